@@ -1,0 +1,493 @@
+/*
+ * psfft_oracle.c -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT.
+ *
+ * A plain, slow, obviously-correct double-precision implementation of what the hot path
+ * of arxiv 1808.01309 computes: the unnormalised 3D real-to-complex DFT of PAPER.md:62
+ * (Sec. 2, Eq. 8), its complex-to-real inverse, and one pseudospectral
+ * Navier-Stokes / MHD right-hand side (Eqs. 1,3,4-6).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may call this.  It shares no code, header, table or helper with the CUDA path under
+ * paper_1808_01309_b200/csrc/.  No blocking, no fusion, no real-FFT trick: every function
+ * is the definition (or the paper's three-step algorithm) written out.
+ * OpenMP is used only to spread independent pencils / output points over host cores.
+ *
+ * Parity pins (tests/test_oracle_*.py): brute-force O(N^6) DFT, single mode -> exact bin,
+ * Parseval, round trip, numpy pocketfft, closed-form derivative, Taylor-Green closed form,
+ * ABC null test, energy/helicity invariants, mask counts, grid independence.  Every
+ * exported function below is pinned by at least one of them; none is "parity unpinned".
+ *
+ * Conventions: real field [z][y][x], x contiguous; half spectrum
+ * [kz][ky][kx], kx in [0, Nx/2]; forward sign -, unnormalised; inverse sign +, scaled by
+ * 1/(Nx Ny Nz); box 2*pi-periodic so wavenumbers are the integers k = p (p < n/2) or
+ * p - n (p >= n/2).
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+
+static const double TWO_PI = 6.283185307179586476925286766559;
+
+/* ---------------------------------------------------------------------------------------
+ * thread control (bench.py reports the count it used)
+ * ------------------------------------------------------------------------------------- */
+int orc_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
+int orc_get_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* w_n^m = exp(sign * 2 pi i m / n) from the REDUCED integer m (no recurrence). */
+static cplx root(int n, long m, int sign)
+{
+    m %= n;
+    if (m < 0) m += n;
+    double a = TWO_PI * (double)m / (double)n;
+    return cos(a) + I * (sign * sin(a));
+}
+
+/* table of w_n^m, m = 0..n-1, each entry computed directly as above */
+static cplx *root_table(int n, int sign)
+{
+    cplx *t = (cplx *)malloc(sizeof(cplx) * (size_t)n);
+    for (int m = 0; m < n; ++m) t[m] = root(n, m, sign);
+    return t;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O1  dft1d_direct: X[p] = sum_j x[j] w^(p j mod n), w = exp(sign 2 pi i / n).
+ *     Eq. 8 restricted to one axis.  O(n^2).
+ * ------------------------------------------------------------------------------------- */
+void orc_dft1d_direct(int n, int sign, const cplx *x, long xs, cplx *X, long Xs)
+{
+    for (int p = 0; p < n; ++p) {
+        cplx acc = 0.0;
+        for (int j = 0; j < n; ++j) acc += x[j * xs] * root(n, (long)p * j, sign);
+        X[p * Xs] = acc;
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O2  fft1d: recursive decimation in time over the smallest prime factor; the p-point
+ *     combination step is O1 with the root table of the top-level n; prime n falls back
+ *     to O1.  ("naive radix-2 / mixed-radix FFT", BASELINE.json north_star.)
+ *     tab = root_table(ntop, sign); step = ntop / n so that w_n^m = tab[(m*step) % ntop].
+ * ------------------------------------------------------------------------------------- */
+static int smallest_factor(int n)
+{
+    if (n % 2 == 0) return 2;
+    for (int f = 3; (long)f * f <= n; f += 2)
+        if (n % f == 0) return f;
+    return n;
+}
+
+static void fft_rec(int n, const cplx *in, long is, cplx *out, cplx *scratch,
+                    const cplx *tab, int ntop)
+{
+    if (n == 1) { out[0] = in[0]; return; }
+    int p = smallest_factor(n);
+    int m = n / p;
+    long step = ntop / n;
+    if (p == n) { /* prime length: direct definition */
+        for (int q = 0; q < n; ++q) {
+            cplx acc = 0.0;
+            for (int j = 0; j < n; ++j) acc += in[j * is] * tab[(((long)q * j) % n) * step];
+            out[q] = acc;
+        }
+        return;
+    }
+    /* sub-transforms of the p decimated sequences x[r], x[r+p], ... -> scratch[r*m ..] */
+    for (int r = 0; r < p; ++r)
+        fft_rec(m, in + r * is, is * p, scratch + (long)r * m, out + (long)r * m, tab, ntop);
+    /* X[k + m q] = sum_r w_n^{r (k + m q)} T_r[k] */
+    for (int k = 0; k < m; ++k)
+        for (int q = 0; q < p; ++q) {
+            cplx acc = 0.0;
+            long idx = k + (long)m * q;
+            for (int r = 0; r < p; ++r) acc += scratch[(long)r * m + k] * tab[((r * idx) % n) * step];
+            out[idx] = acc;
+        }
+}
+
+/* public O2: strided in, strided out; allocates its own table and scratch */
+void orc_fft1d(int n, int sign, const cplx *x, long xs, cplx *X, long Xs)
+{
+    cplx *tab = root_table(n, sign);
+    cplx *out = (cplx *)malloc(sizeof(cplx) * (size_t)n * 2);
+    fft_rec(n, x, xs, out, out + n, tab, n);
+    for (int i = 0; i < n; ++i) X[i * Xs] = out[i];
+    free(out);
+    free(tab);
+}
+
+/* in-place transform of `count` pencils of length n, element stride es; pencil c starts at
+ * base + off[c] where off is given by (c / inner)*outer_s + (c % inner)*inner_s */
+static void fft_pencils(cplx *base, int n, int sign, long es, long count, long inner,
+                        long inner_s, long outer_s)
+{
+    cplx *tab = root_table(n, sign);
+#pragma omp parallel
+    {
+        cplx *buf = (cplx *)malloc(sizeof(cplx) * (size_t)n * 2);
+#pragma omp for schedule(static)
+        for (long c = 0; c < count; ++c) {
+            cplx *p = base + (c / inner) * outer_s + (c % inner) * inner_s;
+            fft_rec(n, p, es, buf, buf + n, tab, n);
+            for (int i = 0; i < n; ++i) p[i * es] = buf[i];
+        }
+        free(buf);
+    }
+    free(tab);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O3  r2c3d: X[r,q,p] = sum_{k,j,i} x[k,j,i] exp(-2 pi i (p i/Nx + q j/Ny + r k/Nz)),
+ *     p in [0, Nx/2]  (Eq. 8; half spectrum PAPER.md:79).
+ *     The paper's three steps: transform along x and y in every plane,
+ *     then along z.  Real data is promoted to complex; no real-FFT trick.  Only the kept
+ *     columns p <= Nx/2 are carried through the y and z steps.
+ * ------------------------------------------------------------------------------------- */
+void orc_r2c3d(int Nz, int Ny, int Nx, const double *x, cplx *X)
+{
+    int H = Nx / 2 + 1;
+    cplx *tab = root_table(Nx, -1);
+#pragma omp parallel
+    {
+        cplx *row = (cplx *)malloc(sizeof(cplx) * (size_t)Nx * 3);
+#pragma omp for schedule(static)
+        for (long zy = 0; zy < (long)Nz * Ny; ++zy) {
+            const double *src = x + zy * Nx;
+            for (int i = 0; i < Nx; ++i) row[i] = src[i];
+            fft_rec(Nx, row, 1, row + Nx, row + 2 * Nx, tab, Nx);
+            for (int p = 0; p < H; ++p) X[zy * H + p] = row[Nx + p];
+        }
+        free(row);
+    }
+    free(tab);
+    /* y: pencils at fixed (z, p), element stride H */
+    fft_pencils(X, Ny, -1, H, (long)Nz * H, H, 1, (long)Ny * H);
+    /* z: pencils at fixed (q, p), element stride Ny*H */
+    fft_pencils(X, Nz, -1, (long)Ny * H, (long)Ny * H, (long)Ny * H, 1, 0);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O4  c2r3d: inverse along z, then y, on the half spectrum; then per row the real
+ *     synthesis  x[i] = (1/Ntot) [ Re Y0 + (-1)^i Re Y_{Nx/2}
+ *                                   + 2 sum_{p=1}^{Nx/2-1} Re( Y_p e^{+2 pi i p i/Nx} ) ],
+ *     evaluated as the inverse complex transform of the Hermitian-extended row
+ *     (Y_{Nx-p} = conj Y_p, imaginary parts of Y_0 and Y_{Nx/2} dropped), which is the
+ *     same sum term by term.  PAPER.md:79 ("the reverse transform essentially reverses
+ *     these steps to produce a real physical space field"); 1/N^3 from BASELINE.json
+ *     config 1.  Defined for ANY half spectrum, Hermitian-consistent or not.
+ *     X is not modified.
+ * ------------------------------------------------------------------------------------- */
+void orc_c2r3d(int Nz, int Ny, int Nx, const cplx *X, double *x)
+{
+    int H = Nx / 2 + 1;
+    size_t nspec = (size_t)Nz * Ny * H;
+    cplx *Y = (cplx *)malloc(sizeof(cplx) * nspec);
+    memcpy(Y, X, sizeof(cplx) * nspec);
+    fft_pencils(Y, Nz, +1, (long)Ny * H, (long)Ny * H, (long)Ny * H, 1, 0);
+    fft_pencils(Y, Ny, +1, H, (long)Nz * H, H, 1, (long)Ny * H);
+    double scale = 1.0 / ((double)Nx * (double)Ny * (double)Nz);
+    cplx *tab = root_table(Nx, +1);
+#pragma omp parallel
+    {
+        cplx *row = (cplx *)malloc(sizeof(cplx) * (size_t)Nx * 3);
+#pragma omp for schedule(static)
+        for (long zy = 0; zy < (long)Nz * Ny; ++zy) {
+            const cplx *src = Y + zy * H;
+            row[0] = creal(src[0]);
+            for (int p = 1; p < H; ++p) {
+                if (2 * p == Nx) row[p] = creal(src[p]);
+                else { row[p] = src[p]; row[Nx - p] = conj(src[p]); }
+            }
+            fft_rec(Nx, row, 1, row + Nx, row + 2 * Nx, tab, Nx);
+            for (int i = 0; i < Nx; ++i) x[zy * Nx + i] = creal(row[Nx + i]) * scale;
+        }
+        free(row);
+    }
+    free(tab);
+    free(Y);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O5  dft3d_bruteforce: the triple sum of Eq. 8 for every output, O(N^6).
+ *     Full spectrum [r][q][p], p in [0, Nx).  Small grids only.
+ *     orc_r2c3d_mode: the same triple sum for ONE output (sampled parity at full size).
+ * ------------------------------------------------------------------------------------- */
+static cplx dft3d_point(int Nz, int Ny, int Nx, const double *x, int r, int q, int p)
+{
+    cplx acc = 0.0;
+    for (int k = 0; k < Nz; ++k) {
+        cplx wk = root(Nz, (long)r * k, -1);
+        cplx accy = 0.0;
+        for (int j = 0; j < Ny; ++j) {
+            cplx wj = root(Ny, (long)q * j, -1);
+            cplx accx = 0.0;
+            const double *row = x + ((long)k * Ny + j) * Nx;
+            for (int i = 0; i < Nx; ++i) accx += row[i] * root(Nx, (long)p * i, -1);
+            accy += accx * wj;
+        }
+        acc += accy * wk;
+    }
+    return acc;
+}
+
+void orc_r2c3d_mode(int Nz, int Ny, int Nx, const double *x, int r, int q, int p, double *out2)
+{
+    /* same sum as dft3d_point with the x-roots tabulated once (large grids) and the
+     * z-planes spread over threads */
+    cplx *tx = root_table(Nx, -1);
+    double accr = 0.0, acci = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : accr, acci)
+    for (int k = 0; k < Nz; ++k) {
+        cplx wk = root(Nz, (long)r * k, -1);
+        cplx accy = 0.0;
+        for (int j = 0; j < Ny; ++j) {
+            cplx wj = root(Ny, (long)q * j, -1);
+            cplx accx = 0.0;
+            const double *row = x + ((long)k * Ny + j) * Nx;
+            for (int i = 0; i < Nx; ++i) accx += row[i] * tx[((long)p * i) % Nx];
+            accy += accx * wj;
+        }
+        cplx t = accy * wk;
+        accr += creal(t);
+        acci += cimag(t);
+    }
+    free(tx);
+    out2[0] = accr;
+    out2[1] = acci;
+}
+
+void orc_dft3d_bruteforce(int Nz, int Ny, int Nx, const double *x, cplx *X)
+{
+#pragma omp parallel for schedule(static) collapse(2)
+    for (int r = 0; r < Nz; ++r)
+        for (int q = 0; q < Ny; ++q)
+            for (int p = 0; p < Nx; ++p)
+                X[((long)r * Ny + q) * Nx + p] = dft3d_point(Nz, Ny, Nx, x, r, q, p);
+}
+
+/* brute-force inverse for ONE physical point from a FULL complex spectrum [r][q][p]:
+ * x[k,j,i] = (1/Ntot) sum X[r,q,p] e^{+2 pi i (...)}  (Eq. 8 with the sign changed) */
+void orc_idft3d_point(int Nz, int Ny, int Nx, const cplx *X, int k, int j, int i, double *out2)
+{
+    cplx acc = 0.0;
+    for (int r = 0; r < Nz; ++r)
+        for (int q = 0; q < Ny; ++q)
+            for (int p = 0; p < Nx; ++p)
+                acc += X[((long)r * Ny + q) * Nx + p] * root(Nz, (long)r * k, +1) *
+                       root(Ny, (long)q * j, +1) * root(Nx, (long)p * i, +1);
+    acc /= ((double)Nx * Ny * Nz);
+    out2[0] = creal(acc);
+    out2[1] = cimag(acc);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * spectral helpers on a cubic N^3 grid (BASELINE.json configs are cubes)
+ * ------------------------------------------------------------------------------------- */
+static inline int wavenumber(int idx, int n) { return idx < n / 2 ? idx : idx - n; } /* n/2 -> -n/2 (G8) */
+
+/* a9: 2/3-rule spherical truncation, integer arithmetic: keep iff 9 |k|^2 < N^2 (G4) */
+static inline int keep_mode(int N, int kx, int ky, int kz)
+{
+    long k2 = (long)kx * kx + (long)ky * ky + (long)kz * kz;
+    return 9 * k2 < (long)N * N;
+}
+
+void orc_dealias_mask(int N, unsigned char *mask)
+{
+    int H = N / 2 + 1;
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p)
+                mask[((long)r * N + q) * H + p] =
+                    (unsigned char)keep_mode(N, p, wavenumber(q, N), wavenumber(r, N));
+}
+
+/* step 1 / step 6 of O6: f <- M f; masked entries become +0.0 (both parts) */
+void orc_apply_mask(int N, int ncomp, cplx *f)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H;
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p)
+                if (!keep_mode(N, p, wavenumber(q, N), wavenumber(r, N)))
+                    for (int c = 0; c < ncomp; ++c) f[c * nf + ((long)r * N + q) * H + p] = 0.0;
+}
+
+/* a7: w = i k x u  (w_x = i (k_y u_z - k_z u_y), cyclic) */
+void orc_curl(int N, const cplx *u, cplx *w)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H;
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p) {
+                long o = ((long)r * N + q) * H + p;
+                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                cplx ux = u[o], uy = u[nf + o], uz = u[2 * nf + o];
+                w[o] = I * (ky * uz - kz * uy);
+                w[nf + o] = I * (kz * ux - kx * uz);
+                w[2 * nf + o] = I * (kx * uy - ky * ux);
+            }
+}
+
+/* a10: f <- f - k (k.f)/|k|^2 for k != 0; identity at k = 0 (G6, G7) */
+void orc_project(int N, cplx *f)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H;
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p) {
+                long o = ((long)r * N + q) * H + p;
+                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                double k2 = kx * kx + ky * ky + kz * kz;
+                if (k2 == 0.0) continue;
+                cplx d = (kx * f[o] + ky * f[nf + o] + kz * f[2 * nf + o]) / k2;
+                f[o] -= kx * d;
+                f[nf + o] -= ky * d;
+                f[2 * nf + o] -= kz * d;
+            }
+}
+
+/* a11: f <- f - nu |k|^2 u */
+static void add_diffusion(int N, double nu, const cplx *u, cplx *f)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H;
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p) {
+                long o = ((long)r * N + q) * H + p;
+                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                double k2 = kx * kx + ky * ky + kz * kz;
+                for (int c = 0; c < 3; ++c) f[c * nf + o] -= nu * k2 * u[c * nf + o];
+            }
+}
+
+/* a8: c = a x b pointwise on n points, 3-component fields laid out [3][n] */
+static void cross_add(long n, const double *a, const double *b, double *c, int accumulate)
+{
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+        double ax = a[i], ay = a[n + i], az = a[2 * n + i];
+        double bx = b[i], by = b[n + i], bz = b[2 * n + i];
+        double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;
+        if (accumulate) { c[i] += cx; c[n + i] += cy; c[2 * n + i] += cz; }
+        else { c[i] = cx; c[n + i] = cy; c[2 * n + i] = cz; }
+    }
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O6  hd_rhs(uhat, nu) = M P F[ F^-1(M uhat) x F^-1(i k x M uhat) ] - nu |k|^2 M uhat
+ *     (Eq. 1 with theta = 0, Eq. 3; nonlinear term in physical
+ *     space, projection in spectral space; rotational form, 2/3 rule and the transform
+ *     count 6 + 3 from BASELINE.json config 2).  Steps 1-8 of SURVEY.md §8(c) O6.
+ *     uhat, rhs: [3][kz][ky][kx], values = N^3 x Fourier coefficient.
+ * ------------------------------------------------------------------------------------- */
+void orc_hd_rhs(int N, const cplx *uhat, double nu, cplx *rhs)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H, nr = (long)N * N * N;
+    cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    cplx *wh = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    double *u = (double *)malloc(sizeof(double) * 3 * nr);
+    double *w = (double *)malloc(sizeof(double) * 3 * nr);
+    memcpy(um, uhat, sizeof(cplx) * 3 * nf);
+    orc_apply_mask(N, 3, um);                                   /* 1 */
+    orc_curl(N, um, wh);                                        /* 2 */
+    for (int c = 0; c < 3; ++c) {                               /* 3 */
+        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
+        orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);
+    }
+    free(wh);
+    double *n = (double *)malloc(sizeof(double) * 3 * nr);
+    cross_add(nr, u, w, n, 0);                                  /* 4 */
+    free(u);
+    free(w);
+    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, n + c * nr, rhs + c * nf); /* 5 */
+    free(n);
+    orc_apply_mask(N, 3, rhs);                                  /* 6 */
+    orc_project(N, rhs);                                        /* 7 */
+    if (nu != 0.0) add_diffusion(N, nu, um, rhs);               /* 8 */
+    free(um);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O7  mhd_rhs (Eqs. 4-6, "v" in Eq. 5 read as u; BASELINE.json config 5):
+ *     w = curl u, j = curl b;  m = u x w + j x b;  e = u x b;
+ *     R_u = M P F[m] - nu |k|^2 M uhat;   R_b = M i k x F[e] - eta |k|^2 M bhat.
+ *     (B.grad B - grad(p + |B|^2/2) = j x b under the projection, as for u.)
+ * ------------------------------------------------------------------------------------- */
+void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double eta, cplx *ru,
+                 cplx *rb)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H, nr = (long)N * N * N;
+    cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    cplx *bm = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    cplx *th = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    double *u = (double *)malloc(sizeof(double) * 3 * nr);
+    double *b = (double *)malloc(sizeof(double) * 3 * nr);
+    double *t = (double *)malloc(sizeof(double) * 3 * nr);
+    double *m = (double *)malloc(sizeof(double) * 3 * nr);
+    memcpy(um, uhat, sizeof(cplx) * 3 * nf);
+    memcpy(bm, bhat, sizeof(cplx) * 3 * nf);
+    orc_apply_mask(N, 3, um);
+    orc_apply_mask(N, 3, bm);
+    for (int c = 0; c < 3; ++c) {
+        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
+        orc_c2r3d(N, N, N, bm + c * nf, b + c * nr);
+    }
+    orc_curl(N, um, th);                                   /* w^ */
+    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, th + c * nf, t + c * nr);
+    cross_add(nr, u, t, m, 0);                             /* m = u x w */
+    orc_curl(N, bm, th);                                   /* j^ */
+    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, th + c * nf, t + c * nr);
+    cross_add(nr, t, b, m, 1);                             /* m += j x b */
+    cross_add(nr, u, b, t, 0);                             /* e = u x b */
+    free(u);
+    free(b);
+    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, m + c * nr, ru + c * nf);
+    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, t + c * nr, th + c * nf);
+    free(m);
+    free(t);
+    orc_apply_mask(N, 3, ru);
+    orc_project(N, ru);
+    if (nu != 0.0) add_diffusion(N, nu, um, ru);
+    orc_apply_mask(N, 3, th);
+    orc_curl(N, th, rb);
+    if (eta != 0.0) add_diffusion(N, eta, bm, rb);
+    free(th);
+    free(um);
+    free(bm);
+}
