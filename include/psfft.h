@@ -1,0 +1,150 @@
+/*
+ * psfft.h -- C ABI of libpsfft: the single-GPU hot path of arxiv 1808.01309 on B200 (sm_100a).
+ *
+ *   N^3 real-to-complex / complex-to-real 3D FFT on a periodic grid (Sec. 2,
+ *   Eq. 8 and the three transform steps) and one pseudospectral Navier-Stokes (HD) or MHD
+ *   right-hand-side evaluation (Eqs. 1, 3, 4-6).
+ *
+ * The calls follow the paper's plan concept -- create / execute forward / execute backward /
+ * clean up, sizes derived from grid size and datatype, an integer return code from every call
+ * (PAPER.md:146-159 Listing 1, :176-212 Sec. 3.2) -- but nothing else of its design: there is no
+ * host staging, no cuFFT, no stream-chunking.  Every execute call is a handful of hand-written
+ * kernels enqueued on the caller's stream.
+ *
+ * CONVENTIONS (all calls)
+ *   Layout   real field      [b][z][y][x], x contiguous            (N^3 reals per field)
+ *            half spectrum   [b][kz][ky][kx], kx in [0, N/2] contiguous, row stride ldk = N/2+1
+ *                            (ldk*N*N complex per field); index q along y/z is wavenumber q for
+ *                            q < N/2 and q-N otherwise; the box is 2*pi-periodic (integer k).
+ *            complex = interleaved (re, im) of the plan's dtype.
+ *   Values   forward: X[r,q,p] = sum x[k,j,i] exp(-2 pi i (p i + q j + r k)/N), unnormalised
+ *            (Eq. 8); inverse: sign +, scaled by 1/N^3 so c2r(r2c(x)) = x.
+ *            Spectral fields handed to / returned by the RHS calls are such unnormalised
+ *            spectra (N^3 x Fourier coefficient).
+ *   Memory   "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  The caller owns
+ *            every buffer (inputs, outputs, workspace, tables); the library never allocates or
+ *            frees device memory.  Device pointers must be 16-byte aligned (256 recommended).
+ *            Inputs are never modified.  Input and output of one call must not overlap; the
+ *            workspace must overlap neither.
+ *   Streams  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Execute
+ *            calls only enqueue work and return without synchronising; they are CUDA-graph
+ *            capturable.  A plan may be used on one stream at a time.
+ *   Errors   0 = success.  Negative = PSFFT_E_* argument errors detected on the host before
+ *            anything is enqueued.  Positive = the cudaError_t of a failed CUDA call.
+ *            There is no CPU fallback: without a CUDA device every execute call fails.
+ */
+#ifndef PSFFT_H
+#define PSFFT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PSFFT_F32 0
+#define PSFFT_F64 1
+
+#define PSFFT_OK 0
+#define PSFFT_E_NULL (-1)        /* a required pointer is NULL */
+#define PSFFT_E_SIZE (-2)        /* unsupported N (see psfft_plan_query) or batch < 1 */
+#define PSFFT_E_DTYPE (-3)       /* dtype is not PSFFT_F32 / PSFFT_F64 */
+#define PSFFT_E_ALIGN (-4)       /* a device pointer is not 16-byte aligned */
+#define PSFFT_E_TABLE (-5)       /* table buffer smaller than layout.table_bytes */
+#define PSFFT_E_PLAN (-6)        /* invalid or destroyed plan handle */
+#define PSFFT_E_BATCH (-7)       /* call needs more fields than the plan's batch provides workspace for */
+
+typedef struct psfft_plan_s *psfft_plan;
+
+/* Sizes implied by (N, dtype, batch); all element counts are per field. */
+typedef struct psfft_layout {
+    int N;                       /* grid points per direction */
+    int dtype;                   /* PSFFT_F32 / PSFFT_F64 */
+    int batch;                   /* fields per fft3d call */
+    int ldk;                     /* leading dimension of the half spectrum (= N/2 + 1) */
+    size_t real_elems;           /* N^3            reals   per real field */
+    size_t spec_elems;           /* ldk * N * N    complex per spectral field */
+    size_t real_bytes;           /* bytes of one real field */
+    size_t spec_bytes;           /* bytes of one spectral field */
+    size_t table_bytes;          /* size of the twiddle-table buffer for psfft_plan_create */
+    size_t work_bytes_fft;       /* workspace for psfft_fft3d_r2c / c2r (batch fields) */
+    size_t work_bytes_hd;        /* workspace for psfft_hd_rhs */
+    size_t work_bytes_mhd;       /* workspace for psfft_mhd_rhs */
+} psfft_layout;
+
+/* Sizes for a prospective plan.  Supported N: 2^a * 3^b with b <= 1 and 8 <= N <= 1024
+ * (8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024).  Host-only. */
+int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out);
+
+/* Create a plan ("create plan": sizes from the input size and datatype).
+ * Computes the root-of-unity table exp(-2 pi i m/N), m = 0..N-1, on the host in long double,
+ * rounds once to the plan dtype and copies it to `d_tables` (>= table_bytes) on `stream`;
+ * returns after that copy has completed.  The plan keeps the pointer; the buffer must outlive
+ * the plan. */
+int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tables,
+                      size_t table_bytes, void *stream);
+
+/* Free host-side state (PAPER.md:187 clean-up).  Never touches caller memory. */
+int psfft_plan_destroy(psfft_plan plan);
+
+/* Fill *out with the plan's layout. */
+int psfft_plan_layout(psfft_plan plan, psfft_layout *out);
+
+/* Forward transform of `batch` real fields (PAPER.md:70-77 steps 1-3; unnormalised, sign -).
+ *   d_real  in   batch * N^3 reals
+ *   d_spec  out  batch * ldk*N*N complex
+ *   d_work       >= work_bytes_fft (may be NULL when that is 0)
+ * Three kernels: x-pass (r2c) -> y-pass -> z-pass; the paper's transpose (step 2) is the
+ * strided tile access of the y/z passes. */
+int psfft_fft3d_r2c(psfft_plan plan, const void *d_real, void *d_spec, void *d_work, void *stream);
+
+/* Inverse transform ("reverses these steps"; sign +, scaled by 1/N^3).
+ * Defined for any half spectrum: imaginary parts of the kx = 0 and kx = N/2 entries that would
+ * break Hermitian symmetry are ignored (x_i = Re Y_0 + (-1)^i Re Y_{N/2} + 2 sum Re(Y_p w^{pi})).
+ *   d_spec  in   batch * ldk*N*N complex (not modified)
+ *   d_real  out  batch * N^3 reals
+ *   d_work       >= work_bytes_fft */
+int psfft_fft3d_c2r(psfft_plan plan, const void *d_spec, void *d_real, void *d_work, void *stream);
+
+/* One Navier-Stokes right-hand side (Eq. 1 with theta = 0, Eq. 3):
+ *     rhs = M P F[ F^-1(M u^) x F^-1(i k x M u^) ] - nu |k|^2 M u^
+ * M = 2/3-rule spherical truncation, keep iff 9 |k|^2 < N^2 (integer test, masked outputs are
+ * exactly +0); P = I - k k^T/|k|^2 (identity at k = 0).  6 inverse + 3 forward transforms.
+ *   d_uhat  in   3 spectral fields [c][kz][ky][kx]
+ *   d_rhs   out  3 spectral fields
+ *   d_work       >= work_bytes_hd
+ * Independent of the plan's batch. */
+int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work,
+                 void *stream);
+
+/* One MHD right-hand side (Eqs. 4-6, v = u in Eq. 5):
+ *     w = curl u, j = curl b;  rhs_u = M P F[u x w + j x b] - nu |k|^2 M u^
+ *                              rhs_b = M i k x F[u x b]     - eta |k|^2 M b^
+ * 12 inverse + 6 forward transforms.  d_work >= work_bytes_mhd. */
+int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u,
+                  void *d_rhs_b, double nu, double eta, void *d_work, void *stream);
+
+/* End-to-end variants with HOST buffers (pinned memory recommended): copy the inputs host->device
+ * into caller-provided device staging, run the call above, copy the result device->host, all on
+ * `stream`, then synchronise the stream.
+ *   d_in / d_out   device staging of the size of the input / output of the corresponding call */
+int psfft_fft3d_r2c_host(psfft_plan plan, const void *h_real, void *h_spec, void *d_in, void *d_out,
+                         void *d_work, void *stream);
+int psfft_fft3d_c2r_host(psfft_plan plan, const void *h_spec, void *h_real, void *d_in, void *d_out,
+                         void *d_work, void *stream);
+int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in,
+                      void *d_out, void *d_work, void *stream);
+
+/* Number of kernels the last execute call on this plan enqueued (bench.py's gpu_launches). */
+int psfft_last_launch_count(psfft_plan plan);
+
+/* Text for a return code (negative: PSFFT_E_*; positive: cudaGetErrorString). */
+const char *psfft_strerror(int code);
+
+/* Library version, "major.minor". */
+const char *psfft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSFFT_H */

@@ -1,0 +1,335 @@
+// psfft_api.cu -- plan object and the extern "C" boundary declared in include/psfft.h.
+// Host logic only; every step of the path runs in the kernels of psfft_kernels.cuh.
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/psfft.h"
+#include "psfft_launch.cuh"
+
+using namespace psfft;
+
+namespace {
+
+const uint32_t PLAN_MAGIC = 0x50534654u;  // "PSFT"
+
+struct Plan {
+    uint32_t magic;
+    psfft_layout lay;
+    void *d_tab;
+    int launches;
+};
+
+bool supported_n(int N)
+{
+    switch (N) {
+#define X(n) case n:
+        PSFFT_FOR_EACH_N(X)
+#undef X
+        return true;
+    }
+    return false;
+}
+
+int fill_layout(int N, int dtype, int batch, psfft_layout *o)
+{
+    if (!o) return PSFFT_E_NULL;
+    if (dtype != PSFFT_F32 && dtype != PSFFT_F64) return PSFFT_E_DTYPE;
+    if (!supported_n(N) || batch < 1) return PSFFT_E_SIZE;
+    const size_t s = dtype == PSFFT_F64 ? 8 : 4;
+    memset(o, 0, sizeof(*o));
+    o->N = N;
+    o->dtype = dtype;
+    o->batch = batch;
+    o->ldk = N / 2 + 1;
+    o->real_elems = (size_t)N * N * N;
+    o->spec_elems = (size_t)o->ldk * N * N;
+    o->real_bytes = o->real_elems * s;
+    o->spec_bytes = o->spec_elems * 2 * s;
+    o->table_bytes = (size_t)N * 2 * s;
+    o->work_bytes_fft = (size_t)batch * o->spec_bytes;
+    o->work_bytes_hd = 12 * o->spec_bytes;
+    o->work_bytes_mhd = 24 * o->spec_bytes;
+    return PSFFT_OK;
+}
+
+inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+Plan *get(psfft_plan p)
+{
+    Plan *pl = reinterpret_cast<Plan *>(p);
+    return (pl && pl->magic == PLAN_MAGIC) ? pl : nullptr;
+}
+
+PassArgs args_of(const Plan *pl, void *stream)
+{
+    PassArgs a;
+    a.tab = pl->d_tab;
+    a.N = pl->lay.N;
+    a.ldk = pl->lay.ldk;
+    a.stream = reinterpret_cast<cudaStream_t>(stream);
+    return a;
+}
+
+#define CU(call)                                   \
+    do {                                           \
+        cudaError_t e__ = (call);                  \
+        if (e__ != cudaSuccess) return (int)e__;   \
+    } while (0)
+
+inline char *off(void *p, size_t bytes) { return static_cast<char *>(p) + bytes; }
+inline const char *off(const void *p, size_t bytes) { return static_cast<const char *>(p) + bytes; }
+
+// ---- transforms ----------------------------------------------------------------------------
+template <typename T> int r2c_fields(Plan *pl, const PassArgs &a, const void *d_real, void *d_spec, int fields)
+{
+    const long nrows = (long)fields * a.N * a.N;
+    CU(launch_xpass_r2c<T>(a, d_real, d_spec, nrows, &pl->launches));
+    CU(launch_cpass<T>(a, -1, 1, d_spec, d_spec, fields, &pl->launches));
+    CU(launch_cpass<T>(a, -1, 2, d_spec, d_spec, fields, &pl->launches));
+    return PSFFT_OK;
+}
+
+// d_spec_work holds the spectra and is overwritten
+template <typename T> int c2r_fields_inplace(Plan *pl, const PassArgs &a, const void *d_spec_in, void *d_spec_work,
+                                             void *d_real, int fields)
+{
+    const long nrows = (long)fields * a.N * a.N;
+    const double scale = 1.0 / ((double)a.N * a.N * a.N);
+    CU(launch_cpass<T>(a, +1, 2, d_spec_in, d_spec_work, fields, &pl->launches));
+    CU(launch_cpass<T>(a, +1, 1, d_spec_work, d_spec_work, fields, &pl->launches));
+    CU(launch_xpass_c2r<T>(a, d_spec_work, d_real, nrows, scale, &pl->launches));
+    return PSFFT_OK;
+}
+
+// ---- right-hand sides (first, unfused composition) -----------------------
+template <typename T> int hd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat, void *rhs, double nu, void *work)
+{
+    const size_t C = pl->lay.spec_bytes, R = pl->lay.real_bytes;
+    void *W0 = work;               // 6 C: (M u^, w^), later 3 R: u x w
+    void *W1 = off(work, 6 * C);   // 6 R: (u, w), later 3 C: F[u x w]
+    CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches));
+    int rc = c2r_fields_inplace<T>(pl, a, W0, W0, W1, 6);
+    if (rc) return rc;
+    CU(launch_cross<T>(a, W1, off(W1, 3 * R), W0, &pl->launches));
+    rc = r2c_fields<T>(pl, a, W0, W1, 3);
+    if (rc) return rc;
+    CU(launch_finish<T>(a, 0, W1, uhat, rhs, nu, &pl->launches));
+    return PSFFT_OK;
+}
+
+template <typename T>
+int mhd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat, const void *bhat, void *ru, void *rb, double nu,
+              double eta, void *work)
+{
+    const size_t C = pl->lay.spec_bytes, R = pl->lay.real_bytes;
+    void *W0 = work;                // 12 C: (M u^, w^, M b^, j^), later 6 R: (m, e)
+    void *W1 = off(work, 12 * C);   // 12 R: (u, w, b, j), later 6 C: (F[m], F[e])
+    CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches));
+    CU(launch_mask_curl<T>(a, bhat, off(W0, 6 * C), &pl->launches));
+    int rc = c2r_fields_inplace<T>(pl, a, W0, W0, W1, 12);
+    if (rc) return rc;
+    CU(launch_cross_mhd<T>(a, W1, off(W1, 6 * R), off(W1, 3 * R), off(W1, 9 * R), W0, off(W0, 3 * R), &pl->launches));
+    rc = r2c_fields<T>(pl, a, W0, W1, 6);
+    if (rc) return rc;
+    CU(launch_finish<T>(a, 0, W1, uhat, ru, nu, &pl->launches));
+    CU(launch_finish<T>(a, 1, off(W1, 3 * C), bhat, rb, eta, &pl->launches));
+    return PSFFT_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out) { return fill_layout(N, dtype, batch, out); }
+
+int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tables, size_t table_bytes, void *stream)
+{
+    if (!plan) return PSFFT_E_NULL;
+    *plan = nullptr;
+    psfft_layout lay;
+    int rc = fill_layout(N, dtype, batch, &lay);
+    if (rc) return rc;
+    if (!d_tables) return PSFFT_E_NULL;
+    if (misaligned(d_tables)) return PSFFT_E_ALIGN;
+    if (table_bytes < lay.table_bytes) return PSFFT_E_TABLE;
+
+    // exp(-2 pi i m / N) from the reduced integer m, evaluated in long double, rounded once
+    std::vector<unsigned char> host(lay.table_bytes);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int m = 0; m < N; ++m) {
+        const long double ang = two_pi * (long double)m / (long double)N;
+        long double c = cosl(ang), s = -sinl(ang);
+        if (4 * m == N) { c = 0; s = -1; }
+        else if (2 * m == N) { c = -1; s = 0; }
+        else if (4 * m == 3 * N) { c = 0; s = 1; }
+        if (dtype == PSFFT_F64) {
+            double *t = reinterpret_cast<double *>(host.data());
+            t[2 * m] = (double)c;
+            t[2 * m + 1] = (double)s;
+        } else {
+            float *t = reinterpret_cast<float *>(host.data());
+            t[2 * m] = (float)c;
+            t[2 * m + 1] = (float)s;
+        }
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    CU(cudaMemcpyAsync(d_tables, host.data(), lay.table_bytes, cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));
+
+    Plan *pl = new (std::nothrow) Plan;
+    if (!pl) return (int)cudaErrorMemoryAllocation;
+    pl->magic = PLAN_MAGIC;
+    pl->lay = lay;
+    pl->d_tab = d_tables;
+    pl->launches = 0;
+    *plan = reinterpret_cast<psfft_plan>(pl);
+    return PSFFT_OK;
+}
+
+int psfft_plan_destroy(psfft_plan plan)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    pl->magic = 0;
+    delete pl;
+    return PSFFT_OK;
+}
+
+int psfft_plan_layout(psfft_plan plan, psfft_layout *out)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!out) return PSFFT_E_NULL;
+    *out = pl->lay;
+    return PSFFT_OK;
+}
+
+int psfft_fft3d_r2c(psfft_plan plan, const void *d_real, void *d_spec, void *d_work, void *stream)
+{
+    (void)d_work;
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_real || !d_spec) return PSFFT_E_NULL;
+    if (misaligned(d_real) || misaligned(d_spec)) return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? r2c_fields<double>(pl, a, d_real, d_spec, pl->lay.batch)
+                                      : r2c_fields<float>(pl, a, d_real, d_spec, pl->lay.batch);
+}
+
+int psfft_fft3d_c2r(psfft_plan plan, const void *d_spec, void *d_real, void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_real || !d_spec || !d_work) return PSFFT_E_NULL;
+    if (misaligned(d_real) || misaligned(d_spec) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? c2r_fields_inplace<double>(pl, a, d_spec, d_work, d_real, pl->lay.batch)
+                                      : c2r_fields_inplace<float>(pl, a, d_spec, d_work, d_real, pl->lay.batch);
+}
+
+int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_uhat || !d_rhs || !d_work) return PSFFT_E_NULL;
+    if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? hd_rhs_t<double>(pl, a, d_uhat, d_rhs, nu, d_work)
+                                      : hd_rhs_t<float>(pl, a, d_uhat, d_rhs, nu, d_work);
+}
+
+int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u, void *d_rhs_b, double nu,
+                  double eta, void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_uhat || !d_bhat || !d_rhs_u || !d_rhs_b || !d_work) return PSFFT_E_NULL;
+    if (misaligned(d_uhat) || misaligned(d_bhat) || misaligned(d_rhs_u) || misaligned(d_rhs_b) || misaligned(d_work))
+        return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? mhd_rhs_t<double>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
+                                      : mhd_rhs_t<float>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work);
+}
+
+int psfft_fft3d_r2c_host(psfft_plan plan, const void *h_real, void *h_spec, void *d_in, void *d_out, void *d_work,
+                         void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!h_real || !h_spec || !d_in || !d_out) return PSFFT_E_NULL;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const size_t nb = (size_t)pl->lay.batch;
+    CU(cudaMemcpyAsync(d_in, h_real, nb * pl->lay.real_bytes, cudaMemcpyHostToDevice, st));
+    int rc = psfft_fft3d_r2c(plan, d_in, d_out, d_work, stream);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h_spec, d_out, nb * pl->lay.spec_bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return PSFFT_OK;
+}
+
+int psfft_fft3d_c2r_host(psfft_plan plan, const void *h_spec, void *h_real, void *d_in, void *d_out, void *d_work,
+                         void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!h_real || !h_spec || !d_in || !d_out) return PSFFT_E_NULL;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const size_t nb = (size_t)pl->lay.batch;
+    CU(cudaMemcpyAsync(d_in, h_spec, nb * pl->lay.spec_bytes, cudaMemcpyHostToDevice, st));
+    int rc = psfft_fft3d_c2r(plan, d_in, d_out, d_work, stream);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h_real, d_out, nb * pl->lay.real_bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return PSFFT_OK;
+}
+
+int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in, void *d_out,
+                      void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!h_uhat || !h_rhs || !d_in || !d_out) return PSFFT_E_NULL;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    CU(cudaMemcpyAsync(d_in, h_uhat, 3 * pl->lay.spec_bytes, cudaMemcpyHostToDevice, st));
+    int rc = psfft_hd_rhs(plan, d_in, d_out, nu, d_work, stream);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h_rhs, d_out, 3 * pl->lay.spec_bytes, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return PSFFT_OK;
+}
+
+int psfft_last_launch_count(psfft_plan plan)
+{
+    Plan *pl = get(plan);
+    return pl ? pl->launches : PSFFT_E_PLAN;
+}
+
+const char *psfft_strerror(int code)
+{
+    switch (code) {
+        case PSFFT_OK: return "success";
+        case PSFFT_E_NULL: return "psfft: required pointer is NULL";
+        case PSFFT_E_SIZE: return "psfft: unsupported grid size or batch";
+        case PSFFT_E_DTYPE: return "psfft: dtype must be PSFFT_F32 or PSFFT_F64";
+        case PSFFT_E_ALIGN: return "psfft: device pointer not 16-byte aligned";
+        case PSFFT_E_TABLE: return "psfft: table buffer too small";
+        case PSFFT_E_PLAN: return "psfft: invalid plan handle";
+        case PSFFT_E_BATCH: return "psfft: plan batch too small for this call";
+    }
+    if (code > 0) return cudaGetErrorString((cudaError_t)code);
+    return "psfft: unknown error code";
+}
+
+const char *psfft_version(void) { return "0.1"; }
+
+}  // extern "C"

@@ -1,0 +1,240 @@
+// psfft_core.cuh -- device-side building blocks of libpsfft (sm_100a).
+//
+// Batched 1D FFTs as register-resident radix-2/3/4/8 butterflies with a shared-memory
+// exchange between stages (Stockham autosort, decimation in time).  One "FFT group" of
+// TPF = L / max_radix threads owns one transform of length L; the first stage reads its
+// inputs straight from a caller-supplied loader (global memory), the last stage hands its
+// outputs to a caller-supplied storer, so a transform costs (stages - 1) shared-memory round
+// trips and exactly one global read and one global write per element.
+//
+// What is computed: Eq. 8 of arxiv 1808.01309 along one axis,
+//   X[p] = sum_j x[j] exp(DIR * 2 pi i p j / L),   DIR = -1 forward, +1 backward,
+// unnormalised in both directions.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace psfft {
+
+// ------------------------------------------------------------------------------------------
+// complex arithmetic on float2 / double2
+// ------------------------------------------------------------------------------------------
+template <typename T> struct CxOf;
+template <> struct CxOf<float> { using type = float2; };
+template <> struct CxOf<double> { using type = double2; };
+template <typename T> using Cx = typename CxOf<T>::type;
+
+template <typename T> __device__ __forceinline__ Cx<T> mk(T re, T im) { Cx<T> r; r.x = re; r.y = im; return r; }
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b)
+{
+    C r;
+    r.x = a.x * b.x - a.y * b.y;
+    r.y = a.x * b.y + a.y * b.x;
+    return r;
+}
+template <typename C> __device__ __forceinline__ C cconj(C a) { a.y = -a.y; return a; }
+// multiply by DIR * i  (DIR = -1: times -i, DIR = +1: times +i)
+template <int DIR, typename C> __device__ __forceinline__ C mul_diri(C a)
+{
+    C r;
+    if (DIR < 0) { r.x = a.y; r.y = -a.x; }
+    else { r.x = -a.y; r.y = a.x; }
+    return r;
+}
+template <typename C, typename T> __device__ __forceinline__ C cscale(C a, T s) { a.x *= s; a.y *= s; return a; }
+
+// ------------------------------------------------------------------------------------------
+// compile-time radix schedule
+// ------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int pow2_part(int n) { int p = 1; while (n % 2 == 0) { n /= 2; p *= 2; } return p; }
+// radix of the stage that starts with `rem` = L / Ns still to be factored
+__host__ __device__ constexpr int pick_radix(int rem)
+{
+    int p2 = pow2_part(rem);
+    return p2 == 16 ? 4 : p2 >= 8 ? 8 : p2 == 4 ? 4 : p2 == 2 ? 2 : 3;
+}
+__host__ __device__ constexpr int max_radix(int L)
+{
+    int m = 1, rem = L;
+    while (rem > 1) { int r = pick_radix(rem); m = r > m ? r : m; rem /= r; }
+    return m;
+}
+__host__ __device__ constexpr int num_stages(int L)
+{
+    int n = 0, rem = L;
+    while (rem > 1) { rem /= pick_radix(rem); ++n; }
+    return n;
+}
+// threads per transform
+__host__ __device__ constexpr int threads_per_fft(int L) { return L / max_radix(L); }
+__host__ __device__ constexpr bool supported_len(int L)
+{
+    int rem = L / pow2_part(L);
+    return L >= 4 && (rem == 1 || rem == 3);
+}
+
+// ------------------------------------------------------------------------------------------
+// in-register butterflies: v[0..R) <- DFT_R(v), natural order out
+// ------------------------------------------------------------------------------------------
+template <int DIR, typename C> __device__ __forceinline__ void bfly2(C &a, C &b)
+{
+    C t = csub(a, b);
+    a = cadd(a, b);
+    b = t;
+}
+
+template <int DIR, typename C> __device__ __forceinline__ void bfly4(C &v0, C &v1, C &v2, C &v3)
+{
+    C t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), t3 = mul_diri<DIR>(csub(v1, v3));
+    v0 = cadd(t0, t2);
+    v2 = csub(t0, t2);
+    v1 = cadd(t1, t3);
+    v3 = csub(t1, t3);
+}
+
+template <int DIR, typename T, typename C> __device__ __forceinline__ void bfly3(C &v0, C &v1, C &v2)
+{
+    const T s = (T)0.86602540378443864676372317075294;  // sqrt(3)/2
+    C t = cadd(v1, v2);
+    C m = mk<T>(v0.x - (T)0.5 * t.x, v0.y - (T)0.5 * t.y);
+    C d = mul_diri<DIR>(cscale(csub(v1, v2), s));
+    v0 = cadd(v0, t);
+    v1 = cadd(m, d);
+    v2 = csub(m, d);
+}
+
+template <int DIR, typename T, typename C> __device__ __forceinline__ void bfly8(C *v)
+{
+    const T h = (T)0.70710678118654752440084436210485;  // 1/sqrt(2)
+    bfly4<DIR>(v[0], v[2], v[4], v[6]);
+    bfly4<DIR>(v[1], v[3], v[5], v[7]);
+    // w8^1 = (1 + DIR i)/sqrt2, w8^2 = DIR i, w8^3 = (-1 + DIR i)/sqrt2
+    C o1, o3;
+    if (DIR < 0) {
+        o1 = mk<T>((v[3].x + v[3].y) * h, (v[3].y - v[3].x) * h);
+        o3 = mk<T>((v[7].y - v[7].x) * h, -(v[7].x + v[7].y) * h);
+    } else {
+        o1 = mk<T>((v[3].x - v[3].y) * h, (v[3].x + v[3].y) * h);
+        o3 = mk<T>(-(v[7].x + v[7].y) * h, (v[7].x - v[7].y) * h);
+    }
+    C o2 = mul_diri<DIR>(v[5]);
+    C e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+    v[0] = cadd(e0, o0);
+    v[4] = csub(e0, o0);
+    v[1] = cadd(e1, o1);
+    v[5] = csub(e1, o1);
+    v[2] = cadd(e2, o2);
+    v[6] = csub(e2, o2);
+    v[3] = cadd(e3, o3);
+    v[7] = csub(e3, o3);
+}
+
+template <int R, int DIR, typename T, typename C> __device__ __forceinline__ void bfly(C *v)
+{
+    if (R == 2) bfly2<DIR>(v[0], v[1]);
+    else if (R == 3) bfly3<DIR, T>(v[0], v[1], v[2]);
+    else if (R == 4) bfly4<DIR>(v[0], v[1], v[2], v[3]);
+    else bfly8<DIR, T>(v);
+}
+
+// ------------------------------------------------------------------------------------------
+// read-only table load (roots of unity): w_N^m = exp(-2 pi i m / N), m in [0, N)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 ldg_c(const double2 *p) { return __ldg(p); }
+__device__ __forceinline__ float2 ldg_c(const float2 *p) { return __ldg(p); }
+
+template <int DIR, typename C> __device__ __forceinline__ C root_of(const C *__restrict__ tab, int m)
+{
+    C w = ldg_c(tab + m);
+    if (DIR > 0) w.y = -w.y;
+    return w;
+}
+
+// ------------------------------------------------------------------------------------------
+// shared-memory index maps.  Elements are whole complex numbers.
+//   ColMap : tile [row][TC columns]; thread column c, rows along the FFT axis.
+//            One padding row of TC elements after every 8 rows when a row is 64 B, so that
+//            the two rows of a 128 B wavefront never share banks in the stride-8 writes.
+//   RowMap : one contiguous transform per group, [c][i]; index i padded by i/8 so that
+//            stride-R writes of 16 B (fp64) / 8 B (fp32) elements are conflict-free.
+// ------------------------------------------------------------------------------------------
+template <int L, int TC, bool PAD> struct ColMap {
+    static constexpr int rows = PAD ? L + (L >> 3) : L;
+    static constexpr int size = rows * TC;
+    __device__ __forceinline__ static int at(int i, int c) { return (PAD ? i + (i >> 3) : i) * TC + c; }
+};
+template <int L> struct RowMap {
+    static constexpr int ld = L + (L >> 3) + 1;
+    __device__ __forceinline__ static int at(int i, int c) { return c * ld + i + (i >> 3); }
+};
+
+// ------------------------------------------------------------------------------------------
+// group-level synchronisation between stages
+// ------------------------------------------------------------------------------------------
+template <bool WARP> __device__ __forceinline__ void group_sync()
+{
+    if (WARP) __syncwarp();
+    else __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------
+// One Stockham stage of radix R on a length-L transform whose earlier stages have radix
+// product Ns.  Butterfly b in [0, L/R): k = b mod Ns,
+//     v[r] = src[b + r L/R] * w_{Ns R}^{r k},  V = DFT_R(v),  dst[(b/Ns) Ns R + k + r Ns] = V[r].
+// src is the loader (SRC_SMEM = false) or shared memory; dst likewise.
+// tws = (table length) / L, so that w_L^m = tab[m * tws].
+// ------------------------------------------------------------------------------------------
+template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
+          class LD, class ST>
+__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tab, int tws, int c, int t,
+                                           LD &ld, ST &st)
+{
+    using C = Cx<T>;
+    constexpr int R = pick_radix(L / Ns);
+    constexpr bool first = (Ns == 1), last = (Ns * R == L);
+    constexpr int NB = L / R;
+    constexpr int ITER = (NB + TPF - 1) / TPF;
+    constexpr bool ragged = (NB % TPF) != 0;
+    constexpr bool from_smem = !first || SRC_SMEM;
+    constexpr bool to_smem = !last || DST_SMEM;
+
+    C v[ITER][R];
+#pragma unroll
+    for (int it = 0; it < ITER; ++it) {
+        const int b = t + it * TPF;
+        if (!ragged || b < NB) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (from_smem) v[it][r] = sm[Map::at(b + r * NB, c)];
+                else v[it][r] = ld(b + r * NB);
+            }
+            if (Ns > 1) {
+                const int k = b % Ns;
+                const int base = k * (L / (Ns * R)) * tws;
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[it][r] = cmul(v[it][r], root_of<DIR>(tab, r * base));
+            }
+            bfly<R, DIR, T>(v[it]);
+        }
+    }
+    if (from_smem && to_smem) group_sync<WARP>();  // in place: every read done before any write
+#pragma unroll
+    for (int it = 0; it < ITER; ++it) {
+        const int b = t + it * TPF;
+        if (!ragged || b < NB) {
+            const int j0 = (b / Ns) * Ns * R + (b % Ns);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (to_smem) sm[Map::at(j0 + r * Ns, c)] = v[it][r];
+                else st(j0 + r * Ns, v[it][r]);
+            }
+        }
+    }
+    if (to_smem) group_sync<WARP>();
+    if constexpr (!last)
+        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST>(sm, tab, tws, c, t, ld, st);
+}
+
+}  // namespace psfft

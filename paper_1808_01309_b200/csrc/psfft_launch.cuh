@@ -1,0 +1,31 @@
+// psfft_launch.cuh -- host-side launchers: pick the kernel instantiation for (dtype, N) and
+// enqueue it.  Declared here, defined (per dtype) in psfft_f32.cu / psfft_f64.cu.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace psfft {
+
+// every supported grid size, in one place (psfft.h: 2^a 3^b, b <= 1, 8 <= N <= 1024)
+#define PSFFT_FOR_EACH_N(X) \
+    X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024)
+
+struct PassArgs {
+    const void *tab;   // roots of unity, N complex of the plan dtype
+    int N;
+    int ldk;
+    cudaStream_t stream;
+};
+
+// Each launcher returns cudaGetLastError() of its launch (or cudaErrorInvalidValue for an
+// unsupported N) and increments *launches.
+template <typename T> cudaError_t launch_xpass_r2c(const PassArgs &a, const void *in, void *out, long nrows, int *launches);
+template <typename T> cudaError_t launch_xpass_c2r(const PassArgs &a, const void *in, void *out, long nrows, double scale, int *launches);
+// dir = -1 forward, +1 backward; axis 1 = y, 2 = z; `fields` contiguous spectral fields
+template <typename T> cudaError_t launch_cpass(const PassArgs &a, int dir, int axis, const void *in, void *out, int fields, int *launches);
+template <typename T> cudaError_t launch_mask_curl(const PassArgs &a, const void *u, void *out6, int *launches);
+template <typename T> cudaError_t launch_cross(const PassArgs &a, const void *pa, const void *pb, void *pc, int *launches);
+template <typename T> cudaError_t launch_cross_mhd(const PassArgs &a, const void *u, const void *b, const void *w, const void *j, void *om, void *oe, int *launches);
+template <typename T> cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void *u, void *out, double nu, int *launches);
+
+}  // namespace psfft

@@ -1,0 +1,237 @@
+"""Thin Python binding of libpsfft (include/psfft.h).  Argument marshalling only.
+
+Same names as the C ABI (``plan_query``, ``plan_create``, ``fft3d_r2c``, ``fft3d_c2r``, ``hd_rhs``,
+``mhd_rhs``, ...).  PyTorch supplies device memory and streams and nothing else: every step of the
+path runs in the library's own kernels.  There is no fallback: if ``libpsfft.so`` is missing or a
+call returns a non-zero code, this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+F32, F64 = 0, 1
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpsfft.so")
+
+EXPORTS = [
+    "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
+    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs",
+    "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
+    "psfft_last_launch_count", "psfft_strerror", "psfft_version",
+]
+
+
+class PsfftError(RuntimeError):
+    pass
+
+
+class Layout(ctypes.Structure):
+    """Mirror of ``psfft_layout``."""
+    _fields_ = [("N", ctypes.c_int), ("dtype", ctypes.c_int), ("batch", ctypes.c_int), ("ldk", ctypes.c_int),
+                ("real_elems", ctypes.c_size_t), ("spec_elems", ctypes.c_size_t),
+                ("real_bytes", ctypes.c_size_t), ("spec_bytes", ctypes.c_size_t),
+                ("table_bytes", ctypes.c_size_t), ("work_bytes_fft", ctypes.c_size_t),
+                ("work_bytes_hd", ctypes.c_size_t), ("work_bytes_mhd", ctypes.c_size_t)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libpsfft.so (built in-tree by ``paper_1808_01309_b200.build``).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise PsfftError(f"{LIB_PATH} not found: run `python -m paper_1808_01309_b200.build` "
+                             "(there is no CPU or PyTorch fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        L.psfft_plan_query.argtypes = [ci, ci, ci, ctypes.POINTER(Layout)]
+        L.psfft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, vp, sz, vp]
+        L.psfft_plan_destroy.argtypes = [vp]
+        L.psfft_plan_layout.argtypes = [vp, ctypes.POINTER(Layout)]
+        L.psfft_fft3d_r2c.argtypes = [vp, vp, vp, vp, vp]
+        L.psfft_fft3d_c2r.argtypes = [vp, vp, vp, vp, vp]
+        L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
+        L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
+        L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.psfft_fft3d_c2r_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.psfft_hd_rhs_host.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
+        L.psfft_last_launch_count.argtypes = [vp]
+        L.psfft_strerror.argtypes = [ci]
+        L.psfft_strerror.restype = ctypes.c_char_p
+        L.psfft_version.restype = ctypes.c_char_p
+        for name in EXPORTS:
+            if getattr(L, name).restype is None:
+                getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().psfft_strerror(int(code)).decode()
+
+
+def _check(code: int, what: str) -> None:
+    if code != 0:
+        raise PsfftError(f"{what} failed with code {code}: {strerror(code)}")
+
+
+def _ptr(t) -> int:
+    if t is None:
+        return 0
+    if isinstance(t, torch.Tensor):
+        return t.data_ptr()
+    return int(t)
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream
+    return int(stream)
+
+
+# ---- the C ABI, one function per entry point ------------------------------------------------------
+
+def plan_query(N: int, dtype: int, batch: int = 1) -> Layout:
+    lay = Layout()
+    _check(lib().psfft_plan_query(N, dtype, batch, ctypes.byref(lay)), "psfft_plan_query")
+    return lay
+
+
+def plan_create(N: int, dtype: int, batch: int, d_tables, table_bytes: int, stream=None) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().psfft_plan_create(ctypes.byref(h), N, dtype, batch, _ptr(d_tables), table_bytes, _stream(stream)),
+           "psfft_plan_create")
+    return h.value
+
+
+def plan_destroy(plan: int) -> None:
+    _check(lib().psfft_plan_destroy(plan), "psfft_plan_destroy")
+
+
+def fft3d_r2c(plan: int, d_real, d_spec, d_work=None, stream=None) -> None:
+    _check(lib().psfft_fft3d_r2c(plan, _ptr(d_real), _ptr(d_spec), _ptr(d_work), _stream(stream)), "psfft_fft3d_r2c")
+
+
+def fft3d_c2r(plan: int, d_spec, d_real, d_work, stream=None) -> None:
+    _check(lib().psfft_fft3d_c2r(plan, _ptr(d_spec), _ptr(d_real), _ptr(d_work), _stream(stream)), "psfft_fft3d_c2r")
+
+
+def hd_rhs(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
+    _check(lib().psfft_hd_rhs(plan, _ptr(d_uhat), _ptr(d_rhs), float(nu), _ptr(d_work), _stream(stream)),
+           "psfft_hd_rhs")
+
+
+def mhd_rhs(plan: int, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu: float, eta: float, d_work, stream=None) -> None:
+    _check(lib().psfft_mhd_rhs(plan, _ptr(d_uhat), _ptr(d_bhat), _ptr(d_rhs_u), _ptr(d_rhs_b), float(nu), float(eta),
+                               _ptr(d_work), _stream(stream)), "psfft_mhd_rhs")
+
+
+def fft3d_r2c_host(plan: int, h_real, h_spec, d_in, d_out, d_work=None, stream=None) -> None:
+    _check(lib().psfft_fft3d_r2c_host(plan, _ptr(h_real), _ptr(h_spec), _ptr(d_in), _ptr(d_out), _ptr(d_work),
+                                      _stream(stream)), "psfft_fft3d_r2c_host")
+
+
+def fft3d_c2r_host(plan: int, h_spec, h_real, d_in, d_out, d_work, stream=None) -> None:
+    _check(lib().psfft_fft3d_c2r_host(plan, _ptr(h_spec), _ptr(h_real), _ptr(d_in), _ptr(d_out), _ptr(d_work),
+                                      _stream(stream)), "psfft_fft3d_c2r_host")
+
+
+def hd_rhs_host(plan: int, h_uhat, h_rhs, nu: float, d_in, d_out, d_work, stream=None) -> None:
+    _check(lib().psfft_hd_rhs_host(plan, _ptr(h_uhat), _ptr(h_rhs), float(nu), _ptr(d_in), _ptr(d_out), _ptr(d_work),
+                                   _stream(stream)), "psfft_hd_rhs_host")
+
+
+def last_launch_count(plan: int) -> int:
+    return int(lib().psfft_last_launch_count(plan))
+
+
+def version() -> str:
+    return lib().psfft_version().decode()
+
+
+# ---- convenience: a plan that owns its torch-allocated tables and workspace -----------------------
+
+class Plan:
+    """Plan + its caller-owned device buffers (allocated with torch; the library allocates nothing).
+
+    >>> p = Plan(512, torch.float64, batch=3)
+    >>> spec = p.r2c(real)          # real: [3, 512, 512, 512] cuda float64 -> [3, 512, 512, 257] complex128
+    >>> back = p.c2r(spec)
+    >>> rhs = p.hd_rhs(uhat)        # uhat: [3, N, N, N/2+1] complex
+    """
+
+    def __init__(self, N: int, dtype=torch.float64, batch: int = 1, device="cuda:0", work: str = "fft"):
+        if not torch.cuda.is_available():
+            raise PsfftError("no CUDA device: libpsfft has no CPU fallback")
+        self.device = torch.device(device)
+        self.rdtype = dtype
+        self.cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
+        code = F64 if dtype == torch.float64 else F32
+        self.layout = plan_query(N, code, batch)
+        self.N, self.batch, self.ldk = N, batch, self.layout.ldk
+        with torch.cuda.device(self.device):
+            self.tables = torch.empty(self.layout.table_bytes, dtype=torch.uint8, device=self.device)
+            self.handle = plan_create(N, code, batch, self.tables, self.layout.table_bytes)
+        self._work = None
+        self._work_kind = None
+        self.ensure_work(work)
+
+    def ensure_work(self, kind: str):
+        need = {"fft": self.layout.work_bytes_fft, "hd": self.layout.work_bytes_hd,
+                "mhd": self.layout.work_bytes_mhd}[kind]
+        if self._work is None or self._work.numel() < need:
+            self._work = None
+            self._work = torch.empty(need, dtype=torch.uint8, device=self.device)
+        return self._work
+
+    def close(self):
+        if getattr(self, "handle", None):
+            plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def spec_shape(self, fields: int):
+        return (fields, self.N, self.N, self.ldk)
+
+    def r2c(self, real: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert real.is_cuda and real.dtype == self.rdtype and real.is_contiguous()
+        assert real.numel() == self.batch * self.N ** 3
+        if out is None:
+            out = torch.empty(self.spec_shape(self.batch), dtype=self.cdtype, device=self.device)
+        fft3d_r2c(self.handle, real, out, self.ensure_work("fft"))
+        return out
+
+    def c2r(self, spec: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert spec.is_cuda and spec.dtype == self.cdtype and spec.is_contiguous()
+        assert spec.numel() == self.batch * self.layout.spec_elems
+        if out is None:
+            out = torch.empty((self.batch, self.N, self.N, self.N), dtype=self.rdtype, device=self.device)
+        fft3d_c2r(self.handle, spec, out, self.ensure_work("fft"))
+        return out
+
+    def hd_rhs(self, uhat: torch.Tensor, nu: float = 0.0, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert uhat.is_cuda and uhat.dtype == self.cdtype and uhat.is_contiguous()
+        assert tuple(uhat.shape) == self.spec_shape(3)
+        if out is None:
+            out = torch.empty_like(uhat)
+        hd_rhs(self.handle, uhat, out, nu, self.ensure_work("hd"))
+        return out
+
+    def mhd_rhs(self, uhat: torch.Tensor, bhat: torch.Tensor, nu: float = 0.0, eta: float = 0.0):
+        for t in (uhat, bhat):
+            assert t.is_cuda and t.dtype == self.cdtype and t.is_contiguous() and tuple(t.shape) == self.spec_shape(3)
+        ru, rb = torch.empty_like(uhat), torch.empty_like(bhat)
+        mhd_rhs(self.handle, uhat, bhat, ru, rb, nu, eta, self.ensure_work("mhd"))
+        return ru, rb

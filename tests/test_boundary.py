@@ -1,0 +1,82 @@
+"""Host-side checks of the C-ABI boundary -- CPU only (no compute calls without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+from paper_1808_01309_b200 import build as psbuild
+from paper_1808_01309_b200 import psfft
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    psbuild.build_library()
+    return psfft.lib()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    """Every function include/psfft.h declares is exported by libpsfft.so, and the binding names them all."""
+    hdr = open(os.path.join(ROOT, "include", "psfft.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(psfft_[a-z0-9_]+)\s*\(", hdr)))
+    assert len(declared) >= 12
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert sorted(psfft.EXPORTS) == declared
+
+
+def test_plan_query_sizes(lib):
+    lay = psfft.plan_query(512, psfft.F64, 3)
+    assert (lay.N, lay.ldk, lay.batch) == (512, 257, 3)
+    assert lay.real_bytes == 1073741824 and lay.spec_bytes == 1077936128      # SURVEY §8 size table
+    assert lay.table_bytes == 512 * 16 and lay.work_bytes_fft == 3 * lay.spec_bytes
+    lay = psfft.plan_query(768, psfft.F32, 1)
+    assert lay.ldk == 385 and lay.real_bytes == 1811939328 and lay.spec_bytes == 1816657920
+    lay = psfft.plan_query(1024, psfft.F32, 1)
+    assert lay.real_bytes == 4294967296 and lay.spec_bytes == 4303355904
+    assert lay.work_bytes_mhd + 12 * lay.spec_bytes < 180e9                    # config 5 fits one B200
+
+
+def test_error_codes(lib):
+    lay = psfft.Layout()
+    assert lib.psfft_plan_query(500, psfft.F64, 1, ctypes.byref(lay)) == -2     # unsupported N
+    assert lib.psfft_plan_query(2048, psfft.F64, 1, ctypes.byref(lay)) == -2
+    assert lib.psfft_plan_query(512, 7, 1, ctypes.byref(lay)) == -3
+    assert lib.psfft_plan_query(512, psfft.F64, 0, ctypes.byref(lay)) == -2
+    assert lib.psfft_plan_query(512, psfft.F64, 1, None) == -1
+    h = ctypes.c_void_p()
+    assert lib.psfft_plan_create(ctypes.byref(h), 64, psfft.F64, 1, None, 1 << 20, None) == -1
+    assert lib.psfft_plan_create(ctypes.byref(h), 64, psfft.F64, 1, ctypes.c_void_p(0x1008), 1 << 20, None) == -4
+    assert lib.psfft_plan_create(ctypes.byref(h), 64, psfft.F64, 1, ctypes.c_void_p(0x1000), 8, None) == -5
+    assert lib.psfft_plan_destroy(None) == -6
+    assert lib.psfft_fft3d_r2c(None, None, None, None, None) == -6
+    for code in (0, -1, -2, -3, -4, -5, -6, -7):
+        assert psfft.strerror(code)
+    assert "psfft" in psfft.strerror(-2)
+    with pytest.raises(psfft.PsfftError):
+        psfft.plan_query(10, psfft.F64, 1)
+    assert psfft.version() == "0.1"
+
+
+def test_every_supported_size_is_accepted(lib):
+    for N in (8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024):
+        for dt in (psfft.F32, psfft.F64):
+            lay = psfft.plan_query(N, dt, 2)
+            assert lay.ldk == N // 2 + 1 and lay.spec_elems == lay.ldk * N * N
+
+
+def test_product_never_imports_the_oracle():
+    """The CUDA path and its binding may not import, read or run anything under oracle/."""
+    pkg = os.path.join(ROOT, "paper_1808_01309_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
+                assert "psfft_oracle" not in src and "liboracle" not in src, f
+    osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "psfft_oracle.c")).read()
+    assert not re.search(r"^\s*(import|from)\s+paper_1808_01309_b200", osrc, flags=re.M)
+    assert "psfft.h" not in osrc and "csrc" not in osrc.replace("paper_1808_01309_b200/csrc/", "")

@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Run on the B200 box:  python -m pytest tests -m gpu
+
+Tolerances (BASELINE.json north_star): relative L2 error <= 1e-12 (fp64), <= 2e-5 (fp32) over the whole
+output; the dealias mask bit-exact (masked outputs exactly +0).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_1808_01309_b200 import psfft, synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float64: 1e-12, torch.float32: 2e-5}
+CDT = {torch.float64: np.complex128, torch.float32: np.complex64}
+RDT = {torch.float64: np.float64, torch.float32: np.float32}
+SMALL = [8, 12, 16, 24, 32, 48, 64, 96, 128]
+
+
+def rel(a, b):
+    a = np.asarray(a).astype(np.complex128 if np.iscomplexobj(a) else np.float64)
+    b = np.asarray(b).astype(a.dtype)
+    return np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.fixture(autouse=True)
+def _sync():
+    yield
+    torch.cuda.synchronize()
+
+
+# ---- config 1 and friends: r2c / c2r -------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", SMALL)
+def test_r2c_matches_oracle(N, dtype):
+    batch = 2 if N <= 48 else 1
+    x = synth.uniform_field(N, batch, 1234, RDT[dtype])
+    p = psfft.Plan(N, dtype, batch)
+    X = p.r2c(dev(x)).cpu().numpy()
+    assert X.shape == (batch, N, N, N // 2 + 1)
+    for b in range(batch):
+        assert rel(X[b], oracle.r2c3d(x[b].astype(np.float64))) < TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", SMALL)
+def test_c2r_matches_oracle_on_non_hermitian_input(N, dtype):
+    """Any half spectrum is a valid input; the imaginary parts at kx = 0, N/2 are ignored as the oracle defines."""
+    rng = np.random.default_rng(N)
+    X = (rng.standard_normal((1, N, N, N // 2 + 1)) + 1j * rng.standard_normal((1, N, N, N // 2 + 1))).astype(CDT[dtype])
+    p = psfft.Plan(N, dtype, 1)
+    Xd = dev(X)
+    x = p.c2r(Xd).cpu().numpy()
+    assert rel(x[0], oracle.c2r3d(X[0].astype(np.complex128), N)) < TOL[dtype]
+    assert np.array_equal(Xd.cpu().numpy(), X)          # input not modified
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_config1_roundtrip_32(dtype):
+    """BASELINE.json config 1: 32^3, uniform [-1,1) from seed, r2c then c2r; spectrum and round trip vs oracle."""
+    N = 32
+    x = synth.uniform_field(N, 1, 1234, RDT[dtype])
+    p = psfft.Plan(N, dtype, 1)
+    X = p.r2c(dev(x))
+    back = p.c2r(X).cpu().numpy()
+    Xo = oracle.r2c3d(x[0].astype(np.float64))
+    assert rel(X.cpu().numpy()[0], Xo) < TOL[dtype]
+    assert rel(back[0], oracle.c2r3d(Xo)) < TOL[dtype]
+    assert rel(back, x) < TOL[dtype]
+
+
+def test_degenerate_inputs():
+    N = 16
+    p = psfft.Plan(N, torch.float64, 1)
+    z = torch.zeros((1, N, N, N), dtype=torch.float64, device="cuda")
+    assert torch.count_nonzero(p.r2c(z)) == 0
+    one = torch.ones_like(z)
+    X = p.r2c(one).cpu().numpy()
+    want = np.zeros_like(X)
+    want[0, 0, 0, 0] = N**3
+    assert np.abs(X - want).max() < 1e-9
+    X = p.r2c(dev(synth.single_mode(N, 3, 2, -1)[None])).cpu().numpy()[0]
+    want = np.zeros_like(X)
+    want[N - 1, 2, 3] = N**3 / 2
+    assert np.abs(X - want).max() < 1e-9
+
+
+def test_streams_and_graph_capture():
+    """Execute calls only enqueue on the given stream and are CUDA-graph capturable."""
+    N = 32
+    x = dev(synth.uniform_field(N, 1, 5))
+    p = psfft.Plan(N, torch.float64, 1)
+    ref = p.r2c(x).clone()
+    out = torch.empty_like(ref)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        psfft.fft3d_r2c(p.handle, x, out, None)          # warm (func attributes) outside capture
+        g = torch.cuda.CUDAGraph()
+        out.zero_()
+        with torch.cuda.graph(g, stream=s):
+            psfft.fft3d_r2c(p.handle, x, out, None, stream=s)
+        g.replay()
+    s.synchronize()
+    assert torch.equal(out, ref)
+    assert psfft.last_launch_count(p.handle) == 3
+
+
+# ---- config 2 and friends: HD right-hand side ------------------------------------------------------
+
+def hd_case(N, k0, kcut, dtype, nu=0.0, seed=1234):
+    uh = synth.solenoidal_spectrum(N, k0, kcut, seed).astype(CDT[dtype])
+    p = psfft.Plan(N, dtype, 1, work="hd")
+    got = p.hd_rhs(dev(uh), nu).cpu().numpy()
+    want = oracle.hd_rhs(uh.astype(np.complex128), nu)
+    return got, want
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,k0,kcut", [(16, 2.0, 7), (24, 2.0, 11), (32, 4.0, 15), (48, 4.0, 23), (64, 4.0, 31), (96, 4.0, 32)])
+def test_hd_rhs_matches_oracle(N, k0, kcut, dtype):
+    """kcut above N/3 on purpose: the input mask of step 1 has to act."""
+    got, want = hd_case(N, k0, kcut, dtype)
+    assert rel(got, want) < TOL[dtype]
+    M = oracle.dealias_mask(N)
+    assert np.all(got[:, ~M] == 0) and not np.any(np.signbit(got[:, ~M].real)) and not np.any(np.signbit(got[:, ~M].imag))
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_config2_hd_rhs_128(dtype):
+    """BASELINE.json config 2: 128^3 HD RHS, E(k) ~ k^4 exp(-2 (k/4)^2), unit energy, seed 1234."""
+    got, want = hd_case(128, 4.0, 32, dtype)
+    assert rel(got, want) < TOL[dtype]
+    M = oracle.dealias_mask(128)
+    assert np.all(got[:, ~M] == 0)
+
+
+def test_hd_rhs_viscous_term():
+    got, want = hd_case(32, 4.0, 12, torch.float64, nu=0.37)
+    assert rel(got, want) < 1e-12
+
+
+def test_hd_rhs_taylor_green_closed_form():
+    """P7 directly on the GPU result: 12 entries +-i N^3/32."""
+    N = 32
+    uh = np.stack([oracle.r2c3d(f) for f in synth.taylor_green(N)])
+    p = psfft.Plan(N, torch.float64, 1, work="hd")
+    got = p.hd_rhs(dev(uh)).cpu().numpy() / N**3
+    assert abs(got[0, 2, 0, 2] - 0.03125j) < 1e-15 and abs(got[0, N - 2, 0, 2] - 0.03125j) < 1e-15
+    assert abs(got[2, 2, 0, 2] + 0.03125j) < 1e-15 and abs(got[2, N - 2, 2, 0] - 0.03125j) < 1e-15
+    assert np.count_nonzero(np.abs(got) > 1e-13) == 12
+
+
+def test_hd_rhs_abc_is_steady_and_input_untouched():
+    N = 16
+    uh = np.stack([oracle.r2c3d(f) for f in synth.abc_flow(N)])
+    d = dev(uh)
+    p = psfft.Plan(N, torch.float64, 1, work="hd")
+    got = p.hd_rhs(d).cpu().numpy()
+    assert np.abs(got).max() / N**3 < 1e-14
+    assert np.array_equal(d.cpu().numpy(), uh)
+
+
+# ---- MHD ----------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [16, 32, 48, 64])
+def test_mhd_rhs_matches_oracle(N, dtype):
+    kcut = N // 2 - 1
+    uh = synth.solenoidal_spectrum(N, 3.0, kcut, 1234, tag=0).astype(CDT[dtype])
+    bh = synth.solenoidal_spectrum(N, 3.0, kcut, 1234, tag=1).astype(CDT[dtype])
+    p = psfft.Plan(N, dtype, 1, work="mhd")
+    ru, rb = p.mhd_rhs(dev(uh), dev(bh), 0.01, 0.02)
+    wu, wb = oracle.mhd_rhs(uh.astype(np.complex128), bh.astype(np.complex128), 0.01, 0.02)
+    assert rel(ru.cpu().numpy(), wu) < TOL[dtype]
+    assert rel(rb.cpu().numpy(), wb) < TOL[dtype]
+    M = oracle.dealias_mask(N)
+    assert np.all(ru.cpu().numpy()[:, ~M] == 0) and np.all(rb.cpu().numpy()[:, ~M] == 0)
+
+
+# ---- host-buffer (end-to-end) entry points -----------------------------------------------------------
+
+def test_host_entry_points():
+    N = 32
+    x = synth.uniform_field(N, 1, 77)
+    p = psfft.Plan(N, torch.float64, 1, work="hd")
+    hx = torch.from_numpy(x).pin_memory()
+    hX = torch.empty((1, N, N, N // 2 + 1), dtype=torch.complex128).pin_memory()
+    d_in = torch.empty(p.layout.spec_bytes * 3, dtype=torch.uint8, device="cuda")
+    d_out = torch.empty(p.layout.spec_bytes * 3, dtype=torch.uint8, device="cuda")
+    psfft.fft3d_r2c_host(p.handle, hx, hX, d_in, d_out, p._work)
+    assert rel(hX.numpy()[0], oracle.r2c3d(x[0])) < 1e-12
+    hb = torch.empty_like(hx)
+    psfft.fft3d_c2r_host(p.handle, hX, hb, d_in, d_out, p._work)
+    assert rel(hb.numpy(), x) < 1e-12
+    uh = synth.solenoidal_spectrum(N, 4.0, 12, 3)
+    hu = torch.from_numpy(uh).pin_memory()
+    hr = torch.empty_like(hu)
+    psfft.hd_rhs_host(p.handle, hu, hr, 0.0, d_in, d_out, p._work)
+    assert rel(hr.numpy(), oracle.hd_rhs(uh, 0.0)) < 1e-12
