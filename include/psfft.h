@@ -135,6 +135,18 @@ int psfft_fft3d_c2r_host(psfft_plan plan, const void *h_spec, void *h_real, void
 int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in,
                       void *d_out, void *d_work, void *stream);
 
+/* Per-launch timing for measurement (bench.py's roofline object).  While enabled, every kernel an
+ * execute call enqueues is bracketed by two CUDA events recorded on the launching stream (so the
+ * call is then NOT graph-capturable).  psfft_profile_get synchronises on record i's stop event and
+ * returns the kernel kind (name via psfft_kernel_name), its device time in ms and the ALGORITHMIC
+ * bytes of that launch (compulsory reads + writes of the pass).
+ * Records accumulate until psfft_profile_reset. */
+int psfft_profile_enable(psfft_plan plan, int on);
+int psfft_profile_reset(psfft_plan plan);
+int psfft_profile_count(psfft_plan plan);
+int psfft_profile_get(psfft_plan plan, int i, int *kind, double *ms, double *bytes);
+const char *psfft_kernel_name(int kind);
+
 /* Number of kernels the last execute call on this plan enqueued (bench.py's gpu_launches). */
 int psfft_last_launch_count(psfft_plan plan);
 

@@ -17,11 +17,52 @@ namespace {
 
 const uint32_t PLAN_MAGIC = 0x50534654u;  // "PSFT"
 
+struct ProfRec {
+    int kind;
+    double bytes;
+    cudaEvent_t start, stop;
+};
+
 struct Plan {
     uint32_t magic;
     psfft_layout lay;
     void *d_tab;
     int launches;
+    bool prof;
+    std::vector<ProfRec> recs;      // records since the last reset
+    std::vector<cudaEvent_t> pool;  // events available for reuse
+};
+
+const char *const KERNEL_NAMES[] = {"xpass_r2c", "xpass_c2r", "cpass_y", "cpass_z", "mask_curl", "cross", "finish"};
+enum { K_XR2C = 0, K_XC2R, K_CPY, K_CPZ, K_MASKCURL, K_CROSS, K_FINISH, K_COUNT };
+
+cudaEvent_t take_event(Plan *pl)
+{
+    cudaEvent_t e = nullptr;
+    if (!pl->pool.empty()) { e = pl->pool.back(); pl->pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+
+// per-launch CUDA events on the launching stream (only when profiling is on)
+struct ProfScope {
+    Plan *pl;
+    cudaStream_t st;
+    ProfScope(Plan *p, cudaStream_t s, int kind, double bytes) : pl(p), st(s)
+    {
+        if (!pl->prof) return;
+        ProfRec r;
+        r.kind = kind;
+        r.bytes = bytes;
+        r.start = take_event(pl);
+        r.stop = take_event(pl);
+        cudaEventRecord(r.start, st);
+        pl->recs.push_back(r);
+    }
+    ~ProfScope()
+    {
+        if (pl->prof) cudaEventRecord(pl->recs.back().stop, st);
+    }
 };
 
 bool supported_n(int N)
@@ -88,9 +129,10 @@ inline const char *off(const void *p, size_t bytes) { return static_cast<const c
 template <typename T> int r2c_fields(Plan *pl, const PassArgs &a, const void *d_real, void *d_spec, int fields)
 {
     const long nrows = (long)fields * a.N * a.N;
-    CU(launch_xpass_r2c<T>(a, d_real, d_spec, nrows, &pl->launches));
-    CU(launch_cpass<T>(a, -1, 1, d_spec, d_spec, fields, &pl->launches));
-    CU(launch_cpass<T>(a, -1, 2, d_spec, d_spec, fields, &pl->launches));
+    const double C = (double)pl->lay.spec_bytes * fields, R = (double)pl->lay.real_bytes * fields;
+    { ProfScope ps(pl, a.stream, K_XR2C, R + C); CU(launch_xpass_r2c<T>(a, d_real, d_spec, nrows, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass<T>(a, -1, 1, d_spec, d_spec, fields, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_CPZ, 2 * C); CU(launch_cpass<T>(a, -1, 2, d_spec, d_spec, fields, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -100,9 +142,10 @@ template <typename T> int c2r_fields_inplace(Plan *pl, const PassArgs &a, const 
 {
     const long nrows = (long)fields * a.N * a.N;
     const double scale = 1.0 / ((double)a.N * a.N * a.N);
-    CU(launch_cpass<T>(a, +1, 2, d_spec_in, d_spec_work, fields, &pl->launches));
-    CU(launch_cpass<T>(a, +1, 1, d_spec_work, d_spec_work, fields, &pl->launches));
-    CU(launch_xpass_c2r<T>(a, d_spec_work, d_real, nrows, scale, &pl->launches));
+    const double C = (double)pl->lay.spec_bytes * fields, R = (double)pl->lay.real_bytes * fields;
+    { ProfScope ps(pl, a.stream, K_CPZ, 2 * C); CU(launch_cpass<T>(a, +1, 2, d_spec_in, d_spec_work, fields, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass<T>(a, +1, 1, d_spec_work, d_spec_work, fields, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_XC2R, R + C); CU(launch_xpass_c2r<T>(a, d_spec_work, d_real, nrows, scale, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -112,13 +155,13 @@ template <typename T> int hd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat
     const size_t C = pl->lay.spec_bytes, R = pl->lay.real_bytes;
     void *W0 = work;               // 6 C: (M u^, w^), later 3 R: u x w
     void *W1 = off(work, 6 * C);   // 6 R: (u, w), later 3 C: F[u x w]
-    CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches));
+    { ProfScope ps(pl, a.stream, K_MASKCURL, 9.0 * C); CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches)); }
     int rc = c2r_fields_inplace<T>(pl, a, W0, W0, W1, 6);
     if (rc) return rc;
-    CU(launch_cross<T>(a, W1, off(W1, 3 * R), W0, &pl->launches));
+    { ProfScope ps(pl, a.stream, K_CROSS, 9.0 * R); CU(launch_cross<T>(a, W1, off(W1, 3 * R), W0, &pl->launches)); }
     rc = r2c_fields<T>(pl, a, W0, W1, 3);
     if (rc) return rc;
-    CU(launch_finish<T>(a, 0, W1, uhat, rhs, nu, &pl->launches));
+    { ProfScope ps(pl, a.stream, K_FINISH, (nu != 0.0 ? 9.0 : 6.0) * C); CU(launch_finish<T>(a, 0, W1, uhat, rhs, nu, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -129,15 +172,16 @@ int mhd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat, const void *bhat, v
     const size_t C = pl->lay.spec_bytes, R = pl->lay.real_bytes;
     void *W0 = work;                // 12 C: (M u^, w^, M b^, j^), later 6 R: (m, e)
     void *W1 = off(work, 12 * C);   // 12 R: (u, w, b, j), later 6 C: (F[m], F[e])
-    CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches));
-    CU(launch_mask_curl<T>(a, bhat, off(W0, 6 * C), &pl->launches));
+    { ProfScope ps(pl, a.stream, K_MASKCURL, 9.0 * C); CU(launch_mask_curl<T>(a, uhat, W0, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_MASKCURL, 9.0 * C); CU(launch_mask_curl<T>(a, bhat, off(W0, 6 * C), &pl->launches)); }
     int rc = c2r_fields_inplace<T>(pl, a, W0, W0, W1, 12);
     if (rc) return rc;
-    CU(launch_cross_mhd<T>(a, W1, off(W1, 6 * R), off(W1, 3 * R), off(W1, 9 * R), W0, off(W0, 3 * R), &pl->launches));
+    { ProfScope ps(pl, a.stream, K_CROSS, 18.0 * R);
+      CU(launch_cross_mhd<T>(a, W1, off(W1, 6 * R), off(W1, 3 * R), off(W1, 9 * R), W0, off(W0, 3 * R), &pl->launches)); }
     rc = r2c_fields<T>(pl, a, W0, W1, 6);
     if (rc) return rc;
-    CU(launch_finish<T>(a, 0, W1, uhat, ru, nu, &pl->launches));
-    CU(launch_finish<T>(a, 1, off(W1, 3 * C), bhat, rb, eta, &pl->launches));
+    { ProfScope ps(pl, a.stream, K_FINISH, (nu != 0.0 ? 9.0 : 6.0) * C); CU(launch_finish<T>(a, 0, W1, uhat, ru, nu, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FINISH, (eta != 0.0 ? 9.0 : 6.0) * C); CU(launch_finish<T>(a, 1, off(W1, 3 * C), bhat, rb, eta, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -188,6 +232,7 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     pl->lay = lay;
     pl->d_tab = d_tables;
     pl->launches = 0;
+    pl->prof = false;
     *plan = reinterpret_cast<psfft_plan>(pl);
     return PSFFT_OK;
 }
@@ -197,6 +242,8 @@ int psfft_plan_destroy(psfft_plan plan)
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
     pl->magic = 0;
+    for (ProfRec &r : pl->recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
+    for (cudaEvent_t e : pl->pool) cudaEventDestroy(e);
     delete pl;
     return PSFFT_OK;
 }
@@ -307,6 +354,47 @@ int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double n
     CU(cudaStreamSynchronize(st));
     return PSFFT_OK;
 }
+
+int psfft_profile_enable(psfft_plan plan, int on)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    pl->prof = on != 0;
+    return PSFFT_OK;
+}
+
+int psfft_profile_reset(psfft_plan plan)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    for (ProfRec &r : pl->recs) { pl->pool.push_back(r.start); pl->pool.push_back(r.stop); }
+    pl->recs.clear();
+    return PSFFT_OK;
+}
+
+int psfft_profile_count(psfft_plan plan)
+{
+    Plan *pl = get(plan);
+    return pl ? (int)pl->recs.size() : PSFFT_E_PLAN;
+}
+
+int psfft_profile_get(psfft_plan plan, int i, int *kind, double *ms, double *bytes)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (i < 0 || i >= (int)pl->recs.size()) return PSFFT_E_SIZE;
+    if (!kind || !ms || !bytes) return PSFFT_E_NULL;
+    const ProfRec &r = pl->recs[i];
+    CU(cudaEventSynchronize(r.stop));
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, r.start, r.stop));
+    *kind = r.kind;
+    *ms = t;
+    *bytes = r.bytes;
+    return PSFFT_OK;
+}
+
+const char *psfft_kernel_name(int kind) { return (kind >= 0 && kind < K_COUNT) ? KERNEL_NAMES[kind] : "?"; }
 
 int psfft_last_launch_count(psfft_plan plan)
 {

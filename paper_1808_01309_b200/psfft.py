@@ -20,7 +20,8 @@ EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
     "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
-    "psfft_last_launch_count", "psfft_strerror", "psfft_version",
+    "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
+    "psfft_kernel_name", "psfft_last_launch_count", "psfft_strerror", "psfft_version",
 ]
 
 
@@ -60,6 +61,12 @@ def lib() -> ctypes.CDLL:
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_hd_rhs_host.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
+        L.psfft_profile_enable.argtypes = [vp, ci]
+        L.psfft_profile_reset.argtypes = [vp]
+        L.psfft_profile_count.argtypes = [vp]
+        L.psfft_profile_get.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd), ctypes.POINTER(cd)]
+        L.psfft_kernel_name.argtypes = [ci]
+        L.psfft_kernel_name.restype = ctypes.c_char_p
         L.psfft_last_launch_count.argtypes = [vp]
         L.psfft_strerror.argtypes = [ci]
         L.psfft_strerror.restype = ctypes.c_char_p
@@ -146,6 +153,25 @@ def fft3d_c2r_host(plan: int, h_spec, h_real, d_in, d_out, d_work, stream=None) 
 def hd_rhs_host(plan: int, h_uhat, h_rhs, nu: float, d_in, d_out, d_work, stream=None) -> None:
     _check(lib().psfft_hd_rhs_host(plan, _ptr(h_uhat), _ptr(h_rhs), float(nu), _ptr(d_in), _ptr(d_out), _ptr(d_work),
                                    _stream(stream)), "psfft_hd_rhs_host")
+
+
+def profile_enable(plan: int, on: bool) -> None:
+    _check(lib().psfft_profile_enable(plan, int(bool(on))), "psfft_profile_enable")
+
+
+def profile_reset(plan: int) -> None:
+    _check(lib().psfft_profile_reset(plan), "psfft_profile_reset")
+
+
+def profile_records(plan: int):
+    """[(kernel name, ms, algorithmic bytes)] for every launch recorded since the last reset."""
+    out = []
+    kind, ms, by = ctypes.c_int(), ctypes.c_double(), ctypes.c_double()
+    for i in range(int(lib().psfft_profile_count(plan))):
+        _check(lib().psfft_profile_get(plan, i, ctypes.byref(kind), ctypes.byref(ms), ctypes.byref(by)),
+               "psfft_profile_get")
+        out.append((lib().psfft_kernel_name(kind.value).decode(), ms.value, by.value))
+    return out
 
 
 def last_launch_count(plan: int) -> int:
