@@ -124,6 +124,17 @@ int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, vo
 int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u,
                   void *d_rhs_b, double nu, double eta, void *d_work, void *stream);
 
+/* The same two right-hand sides computed as the plain composition of the public passes: mask +
+ * curl kernel, 6 (12) three-pass inverse transforms, pointwise product kernel, 3 (6) three-pass
+ * forward transforms, mask + projection kernel.  Nothing is fused or pruned: every pass touches
+ * the dense fields.  Same arguments, same results up to rounding; kept as the second CUDA path that
+ * the full-size tests cross-check the fused one against, and as the "before" of DESIGN.md's
+ * traffic comparison. */
+int psfft_hd_rhs_unfused(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work,
+                         void *stream);
+int psfft_mhd_rhs_unfused(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u,
+                          void *d_rhs_b, double nu, double eta, void *d_work, void *stream);
+
 /* End-to-end variants with HOST buffers (pinned memory recommended): copy the inputs host->device
  * into caller-provided device staging, run the call above, copy the result device->host, all on
  * `stream`, then synchronise the stream.

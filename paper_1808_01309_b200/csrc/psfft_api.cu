@@ -9,9 +9,23 @@
 #include <vector>
 
 #include "../../include/psfft.h"
+#include "psfft_core.cuh"
 #include "psfft_launch.cuh"
 
 using namespace psfft;
+
+namespace psfft {
+// entries are padded to multiples of 16 so that each table starts 256-byte aligned
+size_t table_entries(int N, size_t *off_twN, size_t *off_twM)
+{
+    auto up = [](size_t n) { return (n + 15) / 16 * 16; };
+    const size_t a = up((size_t)N);
+    const size_t b = a + up((size_t)tw_size(N));
+    if (off_twN) *off_twN = a;
+    if (off_twM) *off_twM = b;
+    return b + up((size_t)tw_size(N / 2));
+}
+}  // namespace psfft
 
 namespace {
 
@@ -29,12 +43,14 @@ struct Plan {
     void *d_tab;
     int launches;
     bool prof;
+    double n_disc, n_sphere;        // retained (ky,kx) columns / retained modes of the half spectrum
     std::vector<ProfRec> recs;      // records since the last reset
     std::vector<cudaEvent_t> pool;  // events available for reuse
 };
 
-const char *const KERNEL_NAMES[] = {"xpass_r2c", "xpass_c2r", "cpass_y", "cpass_z", "mask_curl", "cross", "finish"};
-enum { K_XR2C = 0, K_XC2R, K_CPY, K_CPZ, K_MASKCURL, K_CROSS, K_FINISH, K_COUNT };
+const char *const KERNEL_NAMES[] = {"xpass_r2c", "xpass_c2r", "cpass_y", "cpass_z", "mask_curl", "cross", "finish",
+                                    "rhs_inv_z", "rhs_inv_y", "rhs_mid_x", "rhs_fwd_y", "rhs_fwd_z"};
+enum { K_XR2C = 0, K_XC2R, K_CPY, K_CPZ, K_MASKCURL, K_CROSS, K_FINISH, K_INVZ, K_INVY, K_MIDX, K_FWDY, K_FWDZ, K_COUNT };
 
 cudaEvent_t take_event(Plan *pl)
 {
@@ -91,7 +107,7 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     o->spec_elems = (size_t)o->ldk * N * N;
     o->real_bytes = o->real_elems * s;
     o->spec_bytes = o->spec_elems * 2 * s;
-    o->table_bytes = (size_t)N * 2 * s;
+    o->table_bytes = table_entries(N, nullptr, nullptr) * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
     o->work_bytes_hd = 12 * o->spec_bytes;
     o->work_bytes_mhd = 24 * o->spec_bytes;
@@ -109,7 +125,12 @@ Plan *get(psfft_plan p)
 PassArgs args_of(const Plan *pl, void *stream)
 {
     PassArgs a;
+    const size_t cs = pl->lay.dtype == PSFFT_F64 ? 16 : 8;
+    size_t oN, oM;
+    table_entries(pl->lay.N, &oN, &oM);
     a.tab = pl->d_tab;
+    a.twN = static_cast<const char *>(pl->d_tab) + oN * cs;
+    a.twM = static_cast<const char *>(pl->d_tab) + oM * cs;
     a.N = pl->lay.N;
     a.ldk = pl->lay.ldk;
     a.stream = reinterpret_cast<cudaStream_t>(stream);
@@ -149,7 +170,34 @@ template <typename T> int c2r_fields_inplace(Plan *pl, const PassArgs &a, const 
     return PSFFT_OK;
 }
 
-// ---- right-hand sides (first, unfused composition) -----------------------
+// ---- right-hand sides, fused five-pass path (psfft_rhs.cuh) ------------
+// Algorithmic bytes per launch = what the pass must read and write given the known-zero structure
+// of the dealiased spectra: n_disc retained (ky,kx) columns,
+// n_sphere retained modes, KX = kx_count(N) retained kx.
+template <typename T>
+int rhs_fused_t(Plan *pl, const PassArgs &a, int nv, const void *uhat, const void *bhat, void *ru, void *rb, double nu,
+                double eta, void *work)
+{
+    const size_t C = pl->lay.spec_bytes;
+    const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
+    RhsArgs r;
+    r.nv = nv;
+    r.src[0] = uhat; r.src[1] = bhat;
+    r.dst[0] = ru; r.dst[1] = rb;
+    r.diff[0] = nu; r.diff[1] = eta;
+    r.zbuf = work;
+    r.ybuf = off(work, (size_t)5 * nv * C);
+    const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
+    const double ndiff = (nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && eta != 0.0 ? 3.0 : 0.0);
+    { ProfScope ps(pl, a.stream, K_INVZ, nv * (3 * sph + 5 * disc)); CU(launch_rhs_inv_z<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_INVY, nv * (5 * disc + 6 * rows)); CU(launch_rhs_inv_y<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_MIDX, nv * (6 * rows + 3 * rows)); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDY, nv * (3 * rows + 3 * disc)); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, nv * (3 * disc + 3.0 * (double)C) + ndiff * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
+    return PSFFT_OK;
+}
+
+// ---- right-hand sides, unfused composition of the public passes (cross-check path) -------------
 template <typename T> int hd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat, void *rhs, double nu, void *work)
 {
     const size_t C = pl->lay.spec_bytes, R = pl->lay.real_bytes;
@@ -203,25 +251,42 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     if (misaligned(d_tables)) return PSFFT_E_ALIGN;
     if (table_bytes < lay.table_bytes) return PSFFT_E_TABLE;
 
-    // exp(-2 pi i m / N) from the reduced integer m, evaluated in long double, rounded once
+    // Every entry is exp(-2 pi i m / n) from the reduced integer m, evaluated in long double and
+    // rounded once to the plan dtype.  [base: n = N, m = 0..N-1][stage tables, L = N][L = N/2].
     std::vector<unsigned char> host(lay.table_bytes);
-    const long double two_pi = 6.283185307179586476925286766559005768L;
-    for (int m = 0; m < N; ++m) {
-        const long double ang = two_pi * (long double)m / (long double)N;
+    size_t off_twN, off_twM;
+    table_entries(N, &off_twN, &off_twM);
+    auto put = [&](size_t idx, long m, long n) {
+        m %= n;
+        const long double two_pi = 6.283185307179586476925286766559005768L;
+        const long double ang = two_pi * (long double)m / (long double)n;
         long double c = cosl(ang), s = -sinl(ang);
-        if (4 * m == N) { c = 0; s = -1; }
-        else if (2 * m == N) { c = -1; s = 0; }
-        else if (4 * m == 3 * N) { c = 0; s = 1; }
+        if (m == 0) { c = 1; s = 0; }
+        else if (4 * m == n) { c = 0; s = -1; }
+        else if (2 * m == n) { c = -1; s = 0; }
+        else if (4 * m == 3 * n) { c = 0; s = 1; }
         if (dtype == PSFFT_F64) {
             double *t = reinterpret_cast<double *>(host.data());
-            t[2 * m] = (double)c;
-            t[2 * m + 1] = (double)s;
+            t[2 * idx] = (double)c;
+            t[2 * idx + 1] = (double)s;
         } else {
             float *t = reinterpret_cast<float *>(host.data());
-            t[2 * m] = (float)c;
-            t[2 * m + 1] = (float)s;
+            t[2 * idx] = (float)c;
+            t[2 * idx + 1] = (float)s;
         }
-    }
+    };
+    for (int m = 0; m < N; ++m) put(m, m, N);
+    auto stage_tables = [&](size_t base, int L) {   // layout: psfft_core.cuh tw_offset()
+        for (int Ns = 1; Ns < L;) {
+            const int R = pick_radix(L / Ns);
+            if (Ns > 1)
+                for (int r = 1; r < R; ++r)
+                    for (int k = 0; k < Ns; ++k) put(base + tw_offset(L, Ns) + (size_t)(r - 1) * Ns + k, (long)r * k, (long)Ns * R);
+            Ns *= R;
+        }
+    };
+    stage_tables(off_twN, N);
+    stage_tables(off_twM, N / 2);
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     CU(cudaMemcpyAsync(d_tables, host.data(), lay.table_bytes, cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));
@@ -233,6 +298,23 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     pl->d_tab = d_tables;
     pl->launches = 0;
     pl->prof = false;
+    {   // retained columns / modes of the 2/3-rule sphere, by integer enumeration
+        double nd = 0, ns = 0;
+        const long N2 = (long)N * N;
+        for (int q = 0; q < N; ++q) {
+            const long ky = q < N / 2 ? q : q - N;
+            for (long kx = 0; kx <= N / 2; ++kx) {
+                const long kxy2 = kx * kx + ky * ky;
+                if (9 * kxy2 >= N2) continue;
+                nd += 1;
+                long cnt = 0;   // kz = 0, 1, ... retained; each kz > 0 also stands for -kz
+                while (9 * (kxy2 + cnt * cnt) < N2) ++cnt;
+                ns += (double)(2 * cnt - 1);
+            }
+        }
+        pl->n_disc = nd;
+        pl->n_sphere = ns;
+    }
     *plan = reinterpret_cast<psfft_plan>(pl);
     return PSFFT_OK;
 }
@@ -282,7 +364,7 @@ int psfft_fft3d_c2r(psfft_plan plan, const void *d_spec, void *d_real, void *d_w
                                       : c2r_fields_inplace<float>(pl, a, d_spec, d_work, d_real, pl->lay.batch);
 }
 
-int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work, void *stream)
+static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work, void *stream, bool fused)
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
@@ -290,12 +372,15 @@ int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, vo
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
+    if (fused)
+        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, 1, d_uhat, nullptr, d_rhs, nullptr, nu, 0.0, d_work)
+                                          : rhs_fused_t<float>(pl, a, 1, d_uhat, nullptr, d_rhs, nullptr, nu, 0.0, d_work);
     return pl->lay.dtype == PSFFT_F64 ? hd_rhs_t<double>(pl, a, d_uhat, d_rhs, nu, d_work)
                                       : hd_rhs_t<float>(pl, a, d_uhat, d_rhs, nu, d_work);
 }
 
-int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u, void *d_rhs_b, double nu,
-                  double eta, void *d_work, void *stream)
+static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u, void *d_rhs_b, double nu,
+                     double eta, void *d_work, void *stream, bool fused)
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
@@ -304,8 +389,33 @@ int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void 
         return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
+    if (fused)
+        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, 2, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
+                                          : rhs_fused_t<float>(pl, a, 2, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work);
     return pl->lay.dtype == PSFFT_F64 ? mhd_rhs_t<double>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
                                       : mhd_rhs_t<float>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work);
+}
+
+int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work, void *stream)
+{
+    return hd_entry(plan, d_uhat, d_rhs, nu, d_work, stream, true);
+}
+
+int psfft_hd_rhs_unfused(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work, void *stream)
+{
+    return hd_entry(plan, d_uhat, d_rhs, nu, d_work, stream, false);
+}
+
+int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u, void *d_rhs_b, double nu,
+                  double eta, void *d_work, void *stream)
+{
+    return mhd_entry(plan, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work, stream, true);
+}
+
+int psfft_mhd_rhs_unfused(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u, void *d_rhs_b,
+                          double nu, double eta, void *d_work, void *stream)
+{
+    return mhd_entry(plan, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work, stream, false);
 }
 
 int psfft_fft3d_r2c_host(psfft_plan plan, const void *h_real, void *h_spec, void *d_in, void *d_out, void *d_work,

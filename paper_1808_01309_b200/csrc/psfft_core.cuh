@@ -75,6 +75,21 @@ __host__ __device__ constexpr bool supported_len(int L)
     return L >= 4 && (rem == 1 || rem == 3);
 }
 
+// Per-stage twiddle tables.  Stage with earlier radix product Ns (> 1) and radix R needs
+// w_{Ns R}^{r k}, k in [0, Ns), r in [1, R).  They are stored as [r-1][k] (k contiguous, so the
+// lanes of a warp -- consecutive k -- read consecutive 16-byte entries), stage after stage.
+__host__ __device__ constexpr int tw_offset(int L, int Ns_target)
+{
+    int off = 0, Ns = 1;
+    while (Ns < Ns_target) {
+        int r = pick_radix(L / Ns);
+        if (Ns > 1) off += (r - 1) * Ns;
+        Ns *= r;
+    }
+    return off;
+}
+__host__ __device__ constexpr int tw_size(int L) { return tw_offset(L, L); }
+
 // ------------------------------------------------------------------------------------------
 // in-register butterflies: v[0..R) <- DFT_R(v), natural order out
 // ------------------------------------------------------------------------------------------
@@ -145,6 +160,12 @@ template <int R, int DIR, typename T, typename C> __device__ __forceinline__ voi
 __device__ __forceinline__ double2 ldg_c(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg_c(const float2 *p) { return __ldg(p); }
 
+// streaming (touch-once) global access for field data: keeps the twiddle tables resident in L1
+__device__ __forceinline__ double2 ld_stream(const double2 *p) { return __ldcs(p); }
+__device__ __forceinline__ float2 ld_stream(const float2 *p) { return __ldcs(p); }
+__device__ __forceinline__ void st_stream(double2 *p, double2 v) { __stcs(p, v); }
+__device__ __forceinline__ void st_stream(float2 *p, float2 v) { __stcs(p, v); }
+
 template <int DIR, typename C> __device__ __forceinline__ C root_of(const C *__restrict__ tab, int m)
 {
     C w = ldg_c(tab + m);
@@ -184,12 +205,11 @@ template <bool WARP> __device__ __forceinline__ void group_sync()
 // product Ns.  Butterfly b in [0, L/R): k = b mod Ns,
 //     v[r] = src[b + r L/R] * w_{Ns R}^{r k},  V = DFT_R(v),  dst[(b/Ns) Ns R + k + r Ns] = V[r].
 // src is the loader (SRC_SMEM = false) or shared memory; dst likewise.
-// tws = (table length) / L, so that w_L^m = tab[m * tws].
+// tw = per-stage twiddle tables of length L (layout: tw_offset above), forward sign.
 // ------------------------------------------------------------------------------------------
 template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
           class LD, class ST>
-__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tab, int tws, int c, int t,
-                                           LD &ld, ST &st)
+__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st)
 {
     using C = Cx<T>;
     constexpr int R = pick_radix(L / Ns);
@@ -211,10 +231,18 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
                 else v[it][r] = ld(b + r * NB);
             }
             if (Ns > 1) {
-                const int k = b % Ns;
-                const int base = k * (L / (Ns * R)) * tws;
+                const C *__restrict__ ts = tw + tw_offset(L, Ns) + (b % Ns);
+                if (R == 8) {  // three loads, the other four by one or two multiplications
+                    const C w1 = root_of<DIR>(ts, 0), w2 = root_of<DIR>(ts, Ns), w4 = root_of<DIR>(ts, 3 * Ns);
+                    const C w3 = cmul(w1, w2), w5 = cmul(w1, w4), w6 = cmul(w2, w4);
+                    const C w7 = cmul(w3, w4);
+                    v[it][1] = cmul(v[it][1], w1); v[it][2] = cmul(v[it][2], w2); v[it][3] = cmul(v[it][3], w3);
+                    v[it][4] = cmul(v[it][4], w4); v[it][5] = cmul(v[it][5], w5); v[it][6] = cmul(v[it][6], w6);
+                    v[it][7] = cmul(v[it][7], w7);
+                } else {
 #pragma unroll
-                for (int r = 1; r < R; ++r) v[it][r] = cmul(v[it][r], root_of<DIR>(tab, r * base));
+                    for (int r = 1; r < R; ++r) v[it][r] = cmul(v[it][r], root_of<DIR>(ts, (r - 1) * Ns));
+                }
             }
             bfly<R, DIR, T>(v[it]);
         }
@@ -234,7 +262,7 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
     }
     if (to_smem) group_sync<WARP>();
     if constexpr (!last)
-        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST>(sm, tab, tws, c, t, ld, st);
+        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST>(sm, tw, c, t, ld, st);
 }
 
 }  // namespace psfft

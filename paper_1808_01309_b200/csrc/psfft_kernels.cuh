@@ -20,8 +20,8 @@ namespace psfft {
 // ------------------------------------------------------------------------------------------
 template <typename T, int N, int ROWS>
 __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
-    k_xpass_r2c(const T *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab, long nrows,
-                int ldk)
+    k_xpass_r2c(const T *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
+                const Cx<T> *__restrict__ tw, long nrows, int ldk)
 {
     using C = Cx<T>;
     constexpr int M = N / 2;
@@ -38,9 +38,9 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
     const C *src = reinterpret_cast<const C *>(in + row * N);
     C *dst = out + row * (long)ldk;
 
-    auto ld = [&](int i) -> C { return src[i]; };
+    auto ld = [&](int i) -> C { return ld_stream(src + i); };
     auto st = [&](int, C) {};
-    fft_stages<T, M, 1, -1, TPF, false, true, WARP, Map>(sm, tab, 2, c, t, ld, st);
+    fft_stages<T, M, 1, -1, TPF, false, true, WARP, Map>(sm, tw, c, t, ld, st);
 
     if (!valid) return;
 #pragma unroll 2
@@ -51,8 +51,8 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
         const C e = cscale(cadd(zk, zm), (T)0.5);
         const C d = cscale(csub(zk, zm), (T)0.5);
         const C o = mul_diri<-1>(cmul(w, d));  // -(i/2) w (Z[k] - conj Z[M-k])
-        dst[k] = cadd(e, o);
-        if (2 * k != M) dst[M - k] = cconj(csub(e, o));
+        st_stream(dst + k, cadd(e, o));
+        if (2 * k != M) st_stream(dst + (M - k), cconj(csub(e, o)));
     }
 }
 
@@ -63,8 +63,8 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
 // ------------------------------------------------------------------------------------------
 template <typename T, int N, int ROWS>
 __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
-    k_xpass_c2r(const Cx<T> *__restrict__ in, T *__restrict__ out, const Cx<T> *__restrict__ tab, long nrows,
-                int ldk, T scale)
+    k_xpass_c2r(const Cx<T> *__restrict__ in, T *__restrict__ out, const Cx<T> *__restrict__ tab,
+                const Cx<T> *__restrict__ tw, long nrows, int ldk, T scale)
 {
     using C = Cx<T>;
     constexpr int M = N / 2;
@@ -83,8 +83,8 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
 
 #pragma unroll 2
     for (int k = t; k <= M / 2; k += TPF) {
-        C a = src[k];
-        C b = cconj(src[M - k]);
+        C a = ld_stream(src + k);
+        C b = cconj(ld_stream(src + (M - k)));
         if (k == 0) { a.y = (T)0; b.y = (T)0; }
         const C w = root_of<+1>(tab, k);  // exp(+2 pi i k / N)
         const C e = cadd(a, b);
@@ -96,9 +96,9 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
 
     auto ld = [&](int) -> C { return mk<T>(0, 0); };
     auto st = [&](int i, C v) {
-        if (valid) dst[i] = cscale(v, scale);
+        if (valid) st_stream(dst + i, cscale(v, scale));
     };
-    fft_stages<T, M, 1, +1, TPF, true, false, WARP, Map>(sm, tab, 2, c, t, ld, st);
+    fft_stages<T, M, 1, +1, TPF, true, false, WARP, Map>(sm, tw, c, t, ld, st);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -109,13 +109,12 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
 // z-pass: axis_stride = ldk*N, inner = ldk*N, outer = fields,     outer_stride = ldk*N*N
 // In place (in == out) is allowed: a CTA reads all of its columns before it writes any.
 // ------------------------------------------------------------------------------------------
-template <typename T, int N, int DIR, int TC>
-__global__ void __launch_bounds__(TC *threads_per_fft(N))
-    k_cpass(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
-            long axis_stride, long inner, long outer_stride)
+template <typename T, int N, int DIR, int TC, int TPF, int MINB>
+__global__ void __launch_bounds__(TC *TPF, MINB)
+    k_cpass(const Cx<T> *in, Cx<T> *out, const Cx<T> *__restrict__ tw, long axis_stride, long inner,
+            long outer_stride)
 {
     using C = Cx<T>;
-    constexpr int TPF = threads_per_fft(N);
     constexpr bool PAD = (TC * sizeof(C) < 128);
     using Map = ColMap<N, TC, PAD>;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -128,11 +127,11 @@ __global__ void __launch_bounds__(TC *threads_per_fft(N))
     const C *src = in + base;
     C *dst = out + base;
 
-    auto ld = [&](int i) -> C { return valid ? src[i * axis_stride] : mk<T>(0, 0); };
+    auto ld = [&](int i) -> C { return valid ? ld_stream(src + i * axis_stride) : mk<T>(0, 0); };
     auto st = [&](int i, C v) {
-        if (valid) dst[i * axis_stride] = v;
+        if (valid) st_stream(dst + i * axis_stride, v);
     };
-    fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tab, 1, c, t, ld, st);
+    fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tw, c, t, ld, st);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -11,7 +11,9 @@ namespace psfft {
     X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024)
 
 struct PassArgs {
-    const void *tab;   // roots of unity, N complex of the plan dtype
+    const void *tab;   // roots of unity exp(-2 pi i m/N), N complex of the plan dtype
+    const void *twN;   // per-stage twiddle tables of the length-N transforms (y, z passes)
+    const void *twM;   // per-stage twiddle tables of the length-N/2 transforms (x passes)
     int N;
     int ldk;
     cudaStream_t stream;
@@ -27,5 +29,23 @@ template <typename T> cudaError_t launch_mask_curl(const PassArgs &a, const void
 template <typename T> cudaError_t launch_cross(const PassArgs &a, const void *pa, const void *pb, void *pc, int *launches);
 template <typename T> cudaError_t launch_cross_mhd(const PassArgs &a, const void *u, const void *b, const void *w, const void *j, void *om, void *oe, int *launches);
 template <typename T> cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void *u, void *out, double nu, int *launches);
+
+// fused right-hand side (psfft_rhs.cuh); nv = 1 (HD) or 2 (MHD)
+struct RhsArgs {
+    int nv;
+    const void *src[2];   // u^, b^
+    void *dst[2];         // rhs_u, rhs_b
+    double diff[2];       // nu, eta
+    void *zbuf;           // nv x 5 spectral fields (inv_z out; later mid_x out / fwd_y in place, 3 nv fields)
+    void *ybuf;           // nv x 6 spectral fields (inv_y out)
+};
+template <typename T> cudaError_t launch_rhs_inv_z(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T> cudaError_t launch_rhs_inv_y(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T> cudaError_t launch_rhs_mid_x(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T> cudaError_t launch_rhs_fwd_y(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T> cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches);
+
+// complex entries of the three tables (base, twN, twM) for grid size N
+size_t table_entries(int N, size_t *off_twN, size_t *off_twM);
 
 }  // namespace psfft

@@ -2,7 +2,9 @@
 // which instantiate them for one dtype each (two translation units compile in parallel).
 #pragma once
 #include "psfft_kernels.cuh"
+#include "psfft_rhs.cuh"
 #include "psfft_launch.cuh"
+#include <stdlib.h>
 
 namespace psfft {
 
@@ -13,13 +15,17 @@ __host__ __device__ constexpr int xpass_rows(int N)
     int tpf = threads_per_fft(N / 2);
     return tpf >= 256 ? 1 : 256 / tpf;
 }
-// column passes: TC contiguous columns per CTA; at least 64 B per tile row
+// column passes: 16 elements per thread for N >= 128 (two radix-8 butterflies in flight), and TC
+// contiguous columns per CTA: 128-byte tile rows, capped so a tile stays within 64 KB, widened for
+// small N until a CTA has at least 128 threads.  (Measured on B200, 512^3 fp64: 64-byte rows run
+// the z-pass at 3.5 TB/s, 128-byte rows at 5.4 TB/s; profiles/r1_notes.md.)
+__host__ __device__ constexpr int cpass_tpf(int N) { return N >= 128 ? N / 16 : threads_per_fft(N); }
 __host__ __device__ constexpr int cpass_cols(int N, int csize)
 {
-    int tpf = threads_per_fft(N);
-    int tc = tpf >= 256 ? 1 : 256 / tpf;
-    int mn = 64 / csize;
-    return tc < mn ? mn : tc;
+    int tc = 128 / csize;
+    while (tc > 1 && (long)N * tc * csize > 65536) tc /= 2;
+    while (tc * cpass_tpf(N) < 128 && (long)N * tc * 2 * csize <= 65536) tc *= 2;
+    return tc;
 }
 
 template <typename K> static cudaError_t set_smem(K kernel, size_t bytes)
@@ -38,7 +44,8 @@ static cudaError_t xpass_r2c_n(const PassArgs &a, const void *in, void *out, lon
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)((nrows + ROWS - 1) / ROWS);
-    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const T *)in, (Cx<T> *)out, (const Cx<T> *)a.tab, nrows, a.ldk);
+    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const T *)in, (Cx<T> *)out, (const Cx<T> *)a.tab,
+                                                (const Cx<T> *)a.twM, nrows, a.ldk);
     return cudaGetLastError();
 }
 
@@ -52,8 +59,27 @@ static cudaError_t xpass_c2r_n(const PassArgs &a, const void *in, void *out, lon
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     const unsigned grid = (unsigned)((nrows + ROWS - 1) / ROWS);
-    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const Cx<T> *)in, (T *)out, (const Cx<T> *)a.tab, nrows, a.ldk,
-                                                (T)scale);
+    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const Cx<T> *)in, (T *)out, (const Cx<T> *)a.tab,
+                                                (const Cx<T> *)a.twM, nrows, a.ldk, (T)scale);
+    return cudaGetLastError();
+}
+
+template <typename T, int N, int DIR, int TC, int TPF, int MINB>
+static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *out, int fields)
+{
+    using C = Cx<T>;
+    constexpr bool PAD = (TC * sizeof(C) < 128);
+    constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(C);
+    auto kern = k_cpass<T, N, DIR, TC, TPF, MINB>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    const long plane = (long)a.ldk * N;
+    long axis_stride, inner, outer_stride, outer;
+    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)N * fields; }
+    else { axis_stride = plane; inner = plane; outer_stride = plane * N; outer = fields; }
+    dim3 grid((unsigned)((inner + TC - 1) / TC), (unsigned)outer);
+    kern<<<grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)a.twN, axis_stride, inner,
+                                              outer_stride);
     return cudaGetLastError();
 }
 
@@ -62,21 +88,131 @@ static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *ou
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int TPF = threads_per_fft(N);
+    constexpr int TPF = cpass_tpf(N);
+#ifdef PSFFT_EXPERIMENT
+    if constexpr (N == 512 && sizeof(T) == 8) {
+        static const int v = getenv("PSFFT_CPASS_VARIANT") ? atoi(getenv("PSFFT_CPASS_VARIANT")) : 0;
+        const int vv = axis == 1 ? v % 10 : v / 10;   // units digit: y-pass, tens digit: z-pass
+        switch (vv) {
+            case 1: return cpass_v<T, N, DIR, 8, 64, 2>(a, axis, in, out, fields);
+            case 2: return cpass_v<T, N, DIR, 8, 32, 1>(a, axis, in, out, fields);
+            case 3: return cpass_v<T, N, DIR, 4, 32, 1>(a, axis, in, out, fields);
+            case 4: return cpass_v<T, N, DIR, 16, 32, 1>(a, axis, in, out, fields);
+            case 5: return cpass_v<T, N, DIR, 2, 64, 1>(a, axis, in, out, fields);
+            case 6: return cpass_v<T, N, DIR, 8, 64, 1>(a, axis, in, out, fields);
+            default: break;
+        }
+    }
+#endif
+    return cpass_v<T, N, DIR, TC, TPF, 2>(a, axis, in, out, fields);
+}
+
+// ---- fused right-hand side -------------------------------------------------------------------
+template <typename T, int N, int DIR, class Job>
+static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid)
+{
+    using C = Cx<T>;
+    constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    constexpr int TPF = cpass_tpf(N);
     constexpr bool PAD = (TC * sizeof(C) < 128);
     constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(C);
-    auto kern = k_cpass<T, N, DIR, TC>;
+    auto kern = k_cpass_job<T, N, DIR, TC, TPF, 2, Job>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    const long plane = (long)a.ldk * N;
-    long axis_stride, inner, outer_stride, outer;
-    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)N * fields; }
-    else { axis_stride = plane; inner = plane; outer_stride = plane * N; outer = fields; }
-    dim3 grid((unsigned)((inner + TC - 1) / TC), (unsigned)outer);
-    kern<<<grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)a.tab, axis_stride, inner,
-                                              outer_stride);
+    kern<<<grid, TC * TPF, smem, a.stream>>>(job, (const C *)a.twN);
     return cudaGetLastError();
 }
+
+template <typename T, int N, int NV> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
+{
+    using C = Cx<T>;
+    constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    JobInvZ<T, N, TC, NV> job;
+    for (int v = 0; v < NV; ++v) job.src[v] = (const C *)r.src[v];
+    job.dst = (C *)r.zbuf;
+    job.plane = (long)a.ldk * N;
+    job.nf = job.plane * N;
+    job.ldk = a.ldk;
+    return run_job<T, N, +1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)));
+}
+
+template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
+{
+    using C = Cx<T>;
+    constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    JobInvY<T, N, TC, NV> job;
+    job.src = (const C *)r.zbuf;
+    job.dst = (C *)r.ybuf;
+    job.plane = (long)a.ldk * N;
+    job.nf = job.plane * N;
+    job.ldk = a.ldk;
+    return run_job<T, N, +1>(a, job, dim3((unsigned)((kx_count(N) + TC - 1) / TC), (unsigned)N));
+}
+
+template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
+{
+    using C = Cx<T>;
+    constexpr int TPF = threads_per_fft(N / 2);
+    constexpr size_t smem = (size_t)6 * NV * RowMap<N / 2>::ld * sizeof(C);
+    auto kern = k_mid_x<T, N, NV>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    const long nf = (long)a.ldk * N * N;
+    const T scale = (T)(1.0 / ((double)N * N * N));
+    kern<<<(unsigned)(N * N), 6 * NV * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
+                                                               (const C *)a.twM, nf, a.ldk, scale);
+    return cudaGetLastError();
+}
+
+template <typename T, int N, int NV> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)
+{
+    using C = Cx<T>;
+    constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    JobFwdY<T, N, TC> job;
+    job.buf = (C *)r.zbuf;
+    job.plane = (long)a.ldk * N;
+    job.nf = job.plane * N;
+    job.ldk = a.ldk;
+    job.nfields = 3 * NV;
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((kx_count(N) + TC - 1) / TC), (unsigned)N));
+}
+
+template <typename T, int N, int NV> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
+{
+    using C = Cx<T>;
+    constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    JobFwdZ<T, N, TC, NV> job;
+    job.src = (const C *)r.zbuf;
+    for (int v = 0; v < NV; ++v) {
+        job.dst[v] = (C *)r.dst[v];
+        job.aux[v] = (const C *)r.src[v];
+        job.diff[v] = (T)r.diff[v];
+    }
+    job.plane = (long)a.ldk * N;
+    job.nf = job.plane * N;
+    job.ldk = a.ldk;
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)));
+}
+
+#define PSFFT_RHS_LAUNCHER(name)                                                                       \
+    template <typename T> cudaError_t launch_rhs_##name(const PassArgs &a, const RhsArgs &r, int *launches) \
+    {                                                                                                  \
+        ++*launches;                                                                                   \
+        switch (a.N) {                                                                                 \
+            PSFFT_FOR_EACH_N(PSFFT_RHS_CASE_##name)                                                    \
+        }                                                                                              \
+        return cudaErrorInvalidValue;                                                                  \
+    }
+#define PSFFT_RHS_CASE_inv_z(n) case n: return r.nv == 1 ? rhs_inv_z_n<T, n, 1>(a, r) : rhs_inv_z_n<T, n, 2>(a, r);
+#define PSFFT_RHS_CASE_inv_y(n) case n: return r.nv == 1 ? rhs_inv_y_n<T, n, 1>(a, r) : rhs_inv_y_n<T, n, 2>(a, r);
+#define PSFFT_RHS_CASE_mid_x(n) case n: return r.nv == 1 ? rhs_mid_x_n<T, n, 1>(a, r) : rhs_mid_x_n<T, n, 2>(a, r);
+#define PSFFT_RHS_CASE_fwd_y(n) case n: return r.nv == 1 ? rhs_fwd_y_n<T, n, 1>(a, r) : rhs_fwd_y_n<T, n, 2>(a, r);
+#define PSFFT_RHS_CASE_fwd_z(n) case n: return r.nv == 1 ? rhs_fwd_z_n<T, n, 1>(a, r) : rhs_fwd_z_n<T, n, 2>(a, r);
+PSFFT_RHS_LAUNCHER(inv_z)
+PSFFT_RHS_LAUNCHER(inv_y)
+PSFFT_RHS_LAUNCHER(mid_x)
+PSFFT_RHS_LAUNCHER(fwd_y)
+PSFFT_RHS_LAUNCHER(fwd_z)
 
 template <typename T>
 cudaError_t launch_xpass_r2c(const PassArgs &a, const void *in, void *out, long nrows, int *launches)
@@ -163,6 +299,11 @@ cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void
     template cudaError_t launch_cross<T>(const PassArgs &, const void *, const void *, void *, int *);                \
     template cudaError_t launch_cross_mhd<T>(const PassArgs &, const void *, const void *, const void *, const void *, \
                                              void *, void *, int *);                                                  \
-    template cudaError_t launch_finish<T>(const PassArgs &, int, const void *, const void *, void *, double, int *);
+    template cudaError_t launch_finish<T>(const PassArgs &, int, const void *, const void *, void *, double, int *); \
+    template cudaError_t launch_rhs_inv_z<T>(const PassArgs &, const RhsArgs &, int *);                               \
+    template cudaError_t launch_rhs_inv_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
+    template cudaError_t launch_rhs_mid_x<T>(const PassArgs &, const RhsArgs &, int *);                               \
+    template cudaError_t launch_rhs_fwd_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
+    template cudaError_t launch_rhs_fwd_z<T>(const PassArgs &, const RhsArgs &, int *);
 
 }  // namespace psfft

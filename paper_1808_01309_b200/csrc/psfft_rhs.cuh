@@ -1,0 +1,348 @@
+// psfft_rhs.cuh -- the fused right-hand-side passes (HD: NV = 1, MHD: NV = 2).
+//
+// One evaluation is five kernels; physical-space data never reaches HBM and the spectral
+// pointwise work rides on the loads / stores of the transform passes:
+//
+//   inv_z   u^ (masked on load) -> A_c = F_z^-1 u^_c (c = x,y,z),  B_c = F_z^-1 (i kz u^_c) (c = x,y)
+//   inv_y   -> U_c = F_y^-1 A_c,  W_x = F_y^-1 (i ky A_z - B_y),  P = F_y^-1 B_x,  D = F_y^-1 (i ky A_x)
+//   mid_x   per (z,y) row: u_c = c2r U_c, w_x = c2r W_x, w_y = c2r (P - i kx U_z), w_z = c2r (i kx U_y - D);
+//           n = u x w (MHD: m = u x w + j x b, e = u x b);  r2c of n -> kx < N/3 only
+//   fwd_y   in place, kx < N/3
+//   fwd_z   + epilogue on the store: 2/3 mask, projection (or i k x for the induction equation),
+//           diffusion term
+//
+// The curl i k x u^ (a7) is distributed over the three inverse passes: each wavenumber factor is
+// applied in the pass whose FFT runs along that axis (the multiplier is then per-element of the
+// loaded column), everything else commutes with the remaining transforms by linearity.  This
+// needs 5 z-transforms and 6 y-transforms per vector field instead of 6 + 6.
+//
+// Pruning: after the mask of step 1 (and before the mask of step 6) every mode with
+// 9 |k|^2 >= N^2 is zero (does not matter), so columns / rows that are entirely outside the
+// truncation sphere are neither read, transformed nor written, and loads inside a column are
+// predicated on the mode being retained.  Buffers are dense ([kz][ky][ldk]); the skipped
+// entries are simply never touched.
+#pragma once
+#include "psfft_kernels.cuh"
+
+namespace psfft {
+
+// number of kx with 9 kx^2 < N^2
+__host__ __device__ constexpr int kx_count(int N) { return (N - 1) / 3 + 1; }
+
+template <typename C, typename T> __device__ __forceinline__ C mul_ik(C v, T k) { return mk<T>(-k * v.y, k * v.x); }
+
+// ------------------------------------------------------------------------------------------
+// generic multi-round column pass: Job supplies begin(c) / load(r,i) / store(r,i,v)
+// ------------------------------------------------------------------------------------------
+template <typename T, int N, int DIR, int TC, int TPF, int MINB, class Job>
+__global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T> *__restrict__ tw)
+{
+    using C = Cx<T>;
+    constexpr bool PAD = (TC * sizeof(C) < 128);
+    using Map = ColMap<N, TC, PAD>;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    C *sm = reinterpret_cast<C *>(smraw);
+    const int c = threadIdx.x % TC, t = threadIdx.x / TC;
+    typename Job::State s;
+    if (!job.begin(s, c, t)) return;  // CTA-uniform
+#pragma unroll 1
+    for (int r = 0; r < job.rounds(); ++r) {
+        auto ld = [&](int i) -> C { return job.load(s, r, i); };
+        auto st = [&](int i, C v) { job.store(s, r, i, v); };
+        fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tw, c, t, ld, st);
+        __syncthreads();  // the next round's first stage overwrites the tile
+    }
+}
+
+// ---- inv_z -------------------------------------------------------------------------------------
+template <typename T, int N, int TC, int NV> struct JobInvZ {
+    using C = Cx<T>;
+    const C *src[NV];   // NV x 3 spectral fields (u^, b^)
+    C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x, B_y
+    long plane, nf;
+    int ldk;
+    struct State { long col; int kxy2; bool active; };
+
+    __device__ __forceinline__ int rounds() const { return 5 * NV; }
+    __device__ __forceinline__ bool begin(State &s, int c, int) const
+    {
+        s.col = (long)blockIdx.x * TC + c;
+        s.active = false;
+        s.kxy2 = 0;
+        if (s.col < plane) {
+            const int kx = (int)(s.col % ldk), ky = wavenumber((int)(s.col / ldk), N);
+            s.kxy2 = kx * kx + ky * ky;
+            s.active = 9 * s.kxy2 < N * N;
+        }
+        return __syncthreads_or(s.active) != 0;
+    }
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        const int kz = wavenumber(i, N);
+        if (!s.active || 9 * (s.kxy2 + kz * kz) >= N * N) return mk<T>(0, 0);
+        const int v = r / 5, rr = r % 5;
+        const int comp = rr < 3 ? rr : rr - 3;
+        const C *p = (NV == 2 && v == 1) ? src[NV - 1] : src[0];
+        C x = ldg_c(p + comp * nf + i * plane + s.col);
+        if (rr >= 3) x = mul_ik(x, (T)kz);
+        return x;
+    }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (s.active) st_stream(dst + r * nf + i * plane + s.col, v);
+    }
+};
+
+// ---- inv_y -------------------------------------------------------------------------------------
+template <typename T, int N, int TC, int NV> struct JobInvY {
+    using C = Cx<T>;
+    const C *src;  // NV x 5 fields from inv_z
+    C *dst;        // NV x 6 fields: U_x, U_y, U_z, W_x, P, D
+    long plane, nf;
+    int ldk;
+    struct State { long base; int kx; bool active; };
+
+    __device__ __forceinline__ int rounds() const { return 6 * NV; }
+    __device__ __forceinline__ bool begin(State &s, int c, int) const
+    {
+        s.kx = blockIdx.x * TC + c;
+        s.active = s.kx < kx_count(N);
+        s.base = (long)blockIdx.y * plane + s.kx;
+        return true;
+    }
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        const int ky = wavenumber(i, N);
+        if (!s.active || 9 * (s.kx * s.kx + ky * ky) >= N * N) return mk<T>(0, 0);
+        const int v = r / 6, rr = r % 6;
+        // rr: 0 U_x <- A_x | 1 U_y <- A_y | 2 U_z <- A_z | 3 W_x <- i ky A_z - B_y | 4 P <- B_x | 5 D <- i ky A_x
+        const int fa = rr < 3 ? rr : rr == 3 ? 2 : rr == 4 ? 3 : 0;
+        const C *p = src + (long)(v * 5) * nf + s.base + (long)i * ldk;
+        C x = ld_stream(p + fa * nf);
+        if (rr == 3 || rr == 5) x = mul_ik(x, (T)ky);
+        if (rr == 3) x = csub(x, ld_stream(p + 4 * nf));
+        return x;
+    }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (s.active) st_stream(dst + r * nf + s.base + (long)i * ldk, v);
+    }
+};
+
+// ---- fwd_y -------------------------------------------------------------------------------------
+template <typename T, int N, int TC> struct JobFwdY {
+    using C = Cx<T>;
+    C *buf;  // NF fields, in place
+    long plane, nf;
+    int ldk, nfields;
+    struct State { long base; int kx; bool active; };
+
+    __device__ __forceinline__ int rounds() const { return nfields; }
+    __device__ __forceinline__ bool begin(State &s, int c, int) const
+    {
+        s.kx = blockIdx.x * TC + c;
+        s.active = s.kx < kx_count(N);
+        s.base = (long)blockIdx.y * plane + s.kx;
+        return true;
+    }
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        return s.active ? ld_stream(buf + r * nf + s.base + (long)i * ldk) : mk<T>(0, 0);
+    }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        const int ky = wavenumber(i, N);
+        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) st_stream(buf + r * nf + s.base + (long)i * ldk, v);
+    }
+};
+
+// ---- fwd_z + epilogue ----------------------------------------------------------------------------
+// groups of 3 rounds (components x, y, z of one vector field).  Group g: mode[g] = 0 -> P f - d |k|^2 a
+// (momentum), 1 -> i k x f - d |k|^2 a (induction); a = aux[g] (u^ or b^), d = diff[g].
+template <typename T, int N, int TC, int NV> struct JobFwdZ {
+    using C = Cx<T>;
+    const C *src;        // NV x 3 fields (after fwd_y)
+    C *dst[NV];          // NV outputs of 3 fields
+    const C *aux[NV];    // u^, b^ for the diffusion term
+    T diff[NV];
+    long plane, nf;
+    int ldk;
+    struct State { long col; int kx, ky, kxy2; bool active, valid; };
+
+    __device__ __forceinline__ int rounds() const { return 3 * NV; }
+    __device__ __forceinline__ bool begin(State &s, int c, int t) const
+    {
+        s.col = (long)blockIdx.x * TC + c;
+        s.valid = s.col < plane;
+        s.active = false;
+        s.kx = s.ky = s.kxy2 = 0;
+        if (s.valid) {
+            s.kx = (int)(s.col % ldk);
+            s.ky = wavenumber((int)(s.col / ldk), N);
+            s.kxy2 = s.kx * s.kx + s.ky * s.ky;
+            s.active = 9 * s.kxy2 < N * N;
+        }
+        if (__syncthreads_or(s.active)) return true;
+        // nothing retained in this tile: the output is all zeros
+        if (s.valid) {
+            const C z = mk<T>(0, 0);
+            for (int g = 0; g < NV; ++g)
+                for (int comp = 0; comp < 3; ++comp)
+                    for (int i = t; i < N; i += blockDim.x / TC)
+                        st_stream((g == 0 ? dst[0] : dst[NV - 1]) + comp * nf + i * plane + s.col, z);
+        }
+        return false;
+    }
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        return s.active ? ld_stream(src + r * nf + i * plane + s.col) : mk<T>(0, 0);
+    }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (!s.valid) return;
+        const int g = r / 3, comp = r % 3;
+        const int kz = wavenumber(i, N);
+        const int kx = s.kx, ky = s.ky, kxy2 = s.kxy2;
+        C *o = (g == 0 ? dst[0] : dst[NV - 1]) + i * plane + s.col;
+        const bool keep = s.active && 9 * (kxy2 + kz * kz) < N * N;
+        if (!keep) { o[comp * nf] = mk<T>(0, 0); return; }
+        if (comp < 2) { o[comp * nf] = v; return; }   // raw; read back below by this same thread
+        C fx = o[0], fy = o[nf], fz = v;
+        const T qx = (T)kx, qy = (T)ky, qz = (T)kz;
+        const T k2 = (T)(kxy2 + kz * kz);
+        if (g == 0) {            // a10: projection, identity at k = 0
+            if (k2 != (T)0) {
+                const T inv = (T)1 / k2;
+                const T dr = (qx * fx.x + qy * fy.x + qz * fz.x) * inv;
+                const T di = (qx * fx.y + qy * fy.y + qz * fz.y) * inv;
+                fx.x -= qx * dr; fx.y -= qx * di;
+                fy.x -= qy * dr; fy.y -= qy * di;
+                fz.x -= qz * dr; fz.y -= qz * di;
+            }
+        } else {                 // induction: i k x e
+            const C rx = mk<T>(-(qy * fz.y - qz * fy.y), qy * fz.x - qz * fy.x);
+            const C ry = mk<T>(-(qz * fx.y - qx * fz.y), qz * fx.x - qx * fz.x);
+            const C rz = mk<T>(-(qx * fy.y - qy * fx.y), qx * fy.x - qy * fx.x);
+            fx = rx; fy = ry; fz = rz;
+        }
+        const T dg = g == 0 ? diff[0] : diff[NV - 1];
+        if (dg != (T)0) {   // a11
+            const T sc = dg * k2;
+            const C *a = (g == 0 ? aux[0] : aux[NV - 1]) + i * plane + s.col;
+            const C ax = ldg_c(a), ay = ldg_c(a + nf), az = ldg_c(a + 2 * nf);
+            fx.x -= sc * ax.x; fx.y -= sc * ax.y;
+            fy.x -= sc * ay.x; fy.y -= sc * ay.y;
+            fz.x -= sc * az.x; fz.y -= sc * az.y;
+        }
+        o[0] = fx; o[nf] = fy; o[2 * nf] = fz;
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// mid_x: one CTA per (z, y) row; 6 NV groups of TPF threads, one half-length transform each.
+//   in   NV x 6 fields (U_x, U_y, U_z, W_x, P, D), rows of ldk complex, entries kx >= N/3 unused
+//   out  3 NV fields, entries kx < N/3 written
+// ------------------------------------------------------------------------------------------
+template <typename T, int N, int NV>
+__global__ void __launch_bounds__(6 * NV *threads_per_fft(N / 2))
+    k_mid_x(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
+            const Cx<T> *__restrict__ tw, long nf, int ldk, T scale)
+{
+    using C = Cx<T>;
+    constexpr int M = N / 2;
+    constexpr int TPF = threads_per_fft(M);
+    constexpr bool WARP = (TPF <= 32) && (32 % TPF == 0);
+    constexpr int KX = kx_count(N);
+    constexpr int NG = 6 * NV;
+    using Map = RowMap<M>;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    C *sm = reinterpret_cast<C *>(smraw);
+
+    const int g = threadIdx.x / TPF, t = threadIdx.x % TPF;
+    const int v = g / 6, gg = g % 6;
+    const long rowoff = (long)blockIdx.x * ldk;
+    const C *f = in + (long)(v * 6) * nf + rowoff;   // the six fields of this vector
+
+    // spectral row of group gg at index k (0 for k >= KX)
+    auto spec = [&](int k) -> C {
+        if (k >= KX) return mk<T>(0, 0);
+        switch (gg) {
+            case 0: return ld_stream(f + k);
+            case 1: return ld_stream(f + nf + k);
+            case 2: return ld_stream(f + 2 * nf + k);
+            case 3: return ld_stream(f + 3 * nf + k);
+            case 4: return csub(ld_stream(f + 4 * nf + k), mul_ik(ld_stream(f + 2 * nf + k), (T)k));
+            default: return csub(mul_ik(ld_stream(f + nf + k), (T)k), ld_stream(f + 5 * nf + k));
+        }
+    };
+
+    // c2r merge step (see k_xpass_c2r)
+#pragma unroll 2
+    for (int k = t; k <= M / 2; k += TPF) {
+        C a = spec(k);
+        C b = cconj(spec(M - k));
+        if (k == 0) { a.y = (T)0; b.y = (T)0; }
+        const C w = root_of<+1>(tab, k);
+        const C e = cadd(a, b);
+        const C o = mul_diri<+1>(cmul(w, csub(a, b)));
+        sm[Map::at(k, g)] = cadd(e, o);
+        if (k != 0 && 2 * k != M) sm[Map::at(M - k, g)] = cconj(csub(e, o));
+    }
+    group_sync<WARP>();
+    {
+        auto ld = [&](int) -> C { return mk<T>(0, 0); };
+        auto st = [&](int, C) {};
+        fft_stages<T, M, 1, +1, TPF, true, true, WARP, Map>(sm, tw, g, t, ld, st);
+    }
+    __syncthreads();
+
+    // a8: pointwise products; element n of a region holds the grid points (2n, 2n+1)
+    for (int n = threadIdx.x; n < M; n += NG * TPF) {
+        C q[NG];
+#pragma unroll
+        for (int j = 0; j < NG; ++j) q[j] = cscale(sm[Map::at(n, j)], scale);
+        // HD: q0..2 = u, q3..5 = w.   MHD: q0..2 = u, q3..5 = w, q6..8 = b, q9..11 = j
+        C r0, r1, r2;
+        r0.x = q[1].x * q[5].x - q[2].x * q[4].x; r0.y = q[1].y * q[5].y - q[2].y * q[4].y;
+        r1.x = q[2].x * q[3].x - q[0].x * q[5].x; r1.y = q[2].y * q[3].y - q[0].y * q[5].y;
+        r2.x = q[0].x * q[4].x - q[1].x * q[3].x; r2.y = q[0].y * q[4].y - q[1].y * q[3].y;
+        if (NV == 2) {
+            // m = u x w + j x b
+            r0.x += q[10].x * q[8].x - q[11].x * q[7].x; r0.y += q[10].y * q[8].y - q[11].y * q[7].y;
+            r1.x += q[11].x * q[6].x - q[9].x * q[8].x;  r1.y += q[11].y * q[6].y - q[9].y * q[8].y;
+            r2.x += q[9].x * q[7].x - q[10].x * q[6].x;  r2.y += q[9].y * q[7].y - q[10].y * q[6].y;
+            // e = u x b
+            C e0, e1, e2;
+            e0.x = q[1].x * q[8].x - q[2].x * q[7].x; e0.y = q[1].y * q[8].y - q[2].y * q[7].y;
+            e1.x = q[2].x * q[6].x - q[0].x * q[8].x; e1.y = q[2].y * q[6].y - q[0].y * q[8].y;
+            e2.x = q[0].x * q[7].x - q[1].x * q[6].x; e2.y = q[0].y * q[7].y - q[1].y * q[6].y;
+            sm[Map::at(n, 3)] = e0; sm[Map::at(n, 4)] = e1; sm[Map::at(n, 5)] = e2;
+        }
+        sm[Map::at(n, 0)] = r0; sm[Map::at(n, 1)] = r1; sm[Map::at(n, 2)] = r2;
+    }
+    __syncthreads();
+
+    // forward transforms of the 3 NV product rows (the other groups only keep the barriers company)
+    constexpr int NF = 3 * NV;
+    if (WARP && g >= NF) return;
+    {
+        auto ld = [&](int) -> C { return mk<T>(0, 0); };
+        auto st = [&](int, C) {};
+        fft_stages<T, M, 1, -1, TPF, true, true, WARP, Map>(sm, tw, g, t, ld, st);
+    }
+    if (g >= NF) return;
+    C *dst = out + (long)g * nf + rowoff;
+#pragma unroll 2
+    for (int k = t; k <= M / 2; k += TPF) {
+        const C zk = sm[Map::at(k, g)];
+        const C zm = cconj(sm[Map::at((M - k) % M, g)]);
+        const C w = root_of<-1>(tab, k);
+        const C e = cscale(cadd(zk, zm), (T)0.5);
+        const C d = cscale(csub(zk, zm), (T)0.5);
+        const C o = mul_diri<-1>(cmul(w, d));
+        if (k < KX) st_stream(dst + k, cadd(e, o));
+        if (2 * k != M && M - k < KX) st_stream(dst + (M - k), cconj(csub(e, o)));
+    }
+}
+
+}  // namespace psfft

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
     "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs",
+    "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
     "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
     "psfft_kernel_name", "psfft_last_launch_count", "psfft_strerror", "psfft_version",
@@ -58,6 +59,8 @@ def lib() -> ctypes.CDLL:
         L.psfft_fft3d_c2r.argtypes = [vp, vp, vp, vp, vp]
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
+        L.psfft_hd_rhs_unfused.argtypes = [vp, vp, vp, cd, vp, vp]
+        L.psfft_mhd_rhs_unfused.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_hd_rhs_host.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
@@ -138,6 +141,16 @@ def hd_rhs(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
 def mhd_rhs(plan: int, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu: float, eta: float, d_work, stream=None) -> None:
     _check(lib().psfft_mhd_rhs(plan, _ptr(d_uhat), _ptr(d_bhat), _ptr(d_rhs_u), _ptr(d_rhs_b), float(nu), float(eta),
                                _ptr(d_work), _stream(stream)), "psfft_mhd_rhs")
+
+
+def hd_rhs_unfused(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
+    _check(lib().psfft_hd_rhs_unfused(plan, _ptr(d_uhat), _ptr(d_rhs), float(nu), _ptr(d_work), _stream(stream)),
+           "psfft_hd_rhs_unfused")
+
+
+def mhd_rhs_unfused(plan: int, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu: float, eta: float, d_work, stream=None) -> None:
+    _check(lib().psfft_mhd_rhs_unfused(plan, _ptr(d_uhat), _ptr(d_bhat), _ptr(d_rhs_u), _ptr(d_rhs_b), float(nu),
+                                       float(eta), _ptr(d_work), _stream(stream)), "psfft_mhd_rhs_unfused")
 
 
 def fft3d_r2c_host(plan: int, h_real, h_spec, d_in, d_out, d_work=None, stream=None) -> None:

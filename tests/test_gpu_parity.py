@@ -206,3 +206,22 @@ def test_host_entry_points():
     hr = torch.empty_like(hu)
     psfft.hd_rhs_host(p.handle, hu, hr, 0.0, d_in, d_out, p._work)
     assert rel(hr.numpy(), oracle.hd_rhs(uh, 0.0)) < 1e-12
+
+
+# ---- the unfused composition (second CUDA path) ------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [16, 48, 64])
+def test_unfused_rhs_matches_oracle(N, dtype):
+    kcut = N // 2 - 1
+    uh = synth.solenoidal_spectrum(N, 3.0, kcut, 7, tag=0).astype(CDT[dtype])
+    bh = synth.solenoidal_spectrum(N, 3.0, kcut, 7, tag=1).astype(CDT[dtype])
+    p = psfft.Plan(N, dtype, 1, work="mhd")
+    du, db = dev(uh), dev(bh)
+    out = torch.empty_like(du)
+    psfft.hd_rhs_unfused(p.handle, du, out, 0.05, p._work)
+    assert rel(out.cpu().numpy(), oracle.hd_rhs(uh.astype(np.complex128), 0.05)) < TOL[dtype]
+    ru, rb = torch.empty_like(du), torch.empty_like(du)
+    psfft.mhd_rhs_unfused(p.handle, du, db, ru, rb, 0.01, 0.02, p._work)
+    wu, wb = oracle.mhd_rhs(uh.astype(np.complex128), bh.astype(np.complex128), 0.01, 0.02)
+    assert rel(ru.cpu().numpy(), wu) < TOL[dtype] and rel(rb.cpu().numpy(), wb) < TOL[dtype]
