@@ -207,9 +207,16 @@ template <bool WARP> __device__ __forceinline__ void group_sync()
 // src is the loader (SRC_SMEM = false) or shared memory; dst likewise.
 // tw = per-stage twiddle tables of length L (layout: tw_offset above), forward sign.
 // ------------------------------------------------------------------------------------------
+// ld(i) must be a bare (possibly predicated) load so that all loads of a stage issue back to
+// back; px(i, x) is applied to the loaded values afterwards (masking factors, i k multipliers).
+struct NoPost {
+    template <typename C> __device__ __forceinline__ C operator()(int, C x) const { return x; }
+};
+
 template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
-          class LD, class ST>
-__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st)
+          class LD, class ST, class PX>
+__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st,
+                                           PX &px)
 {
     using C = Cx<T>;
     constexpr int R = pick_radix(L / Ns);
@@ -229,6 +236,16 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
             for (int r = 0; r < R; ++r) {
                 if (from_smem) v[it][r] = sm[Map::at(b + r * NB, c)];
                 else v[it][r] = ld(b + r * NB);
+            }
+        }
+    }
+#pragma unroll
+    for (int it = 0; it < ITER; ++it) {
+        const int b = t + it * TPF;
+        if (!ragged || b < NB) {
+            if (!from_smem) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) v[it][r] = px(b + r * NB, v[it][r]);
             }
             if (Ns > 1) {
                 const C *__restrict__ ts = tw + tw_offset(L, Ns) + (b % Ns);
@@ -262,7 +279,15 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
     }
     if (to_smem) group_sync<WARP>();
     if constexpr (!last)
-        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST>(sm, tw, c, t, ld, st);
+        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, PX>(sm, tw, c, t, ld, st, px);
+}
+
+template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
+          class LD, class ST>
+__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st)
+{
+    NoPost px;
+    fft_stages<T, L, Ns, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, NoPost>(sm, tw, c, t, ld, st, px);
 }
 
 }  // namespace psfft

@@ -3,8 +3,9 @@
 // One evaluation is five kernels; physical-space data never reaches HBM and the spectral
 // pointwise work rides on the loads / stores of the transform passes:
 //
-//   inv_z   u^ (masked on load) -> A_c = F_z^-1 u^_c (c = x,y,z),  B_c = F_z^-1 (i kz u^_c) (c = x,y)
-//   inv_y   -> U_c = F_y^-1 A_c,  W_x = F_y^-1 (i ky A_z - B_y),  P = F_y^-1 B_x,  D = F_y^-1 (i ky A_x)
+//   inv_z   u^ (masked on load) -> A_c = F_z^-1 u^_c (c = x,y,z),  B_x = F_z^-1 (i kz u^_x),
+//           G_x = F_z^-1 (i (ky u^_z - kz u^_y))  [= w^_x, complete]
+//   inv_y   -> U_c = F_y^-1 A_c,  W_x = F_y^-1 G_x,  P = F_y^-1 B_x,  D = F_y^-1 (i ky A_x)
 //   mid_x   per (z,y) row: u_c = c2r U_c, w_x = c2r W_x, w_y = c2r (P - i kx U_z), w_z = c2r (i kx U_y - D);
 //           n = u x w (MHD: m = u x w + j x b, e = u x b);  r2c of n -> kx < N/3 only
 //   fwd_y   in place, kx < N/3
@@ -48,8 +49,9 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
 #pragma unroll 1
     for (int r = 0; r < job.rounds(); ++r) {
         auto ld = [&](int i) -> C { return job.load(s, r, i); };
+        auto px = [&](int i, C x) -> C { return job.post(s, r, i, x); };
         auto st = [&](int i, C v) { job.store(s, r, i, v); };
-        fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tw, c, t, ld, st);
+        fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tw, c, t, ld, st, px);
         __syncthreads();  // the next round's first stage overwrites the tile
     }
 }
@@ -58,10 +60,10 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
 template <typename T, int N, int TC, int NV> struct JobInvZ {
     using C = Cx<T>;
     const C *src[NV];   // NV x 3 spectral fields (u^, b^)
-    C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x, B_y
+    C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x = F_z^-1(i kz u_x), G_x = F_z^-1(w^_x)
     long plane, nf;
     int ldk;
-    struct State { long col; int kxy2; bool active; };
+    struct State { long col; int kxy2, ky; bool active; };
 
     __device__ __forceinline__ int rounds() const { return 5 * NV; }
     __device__ __forceinline__ bool begin(State &s, int c, int) const
@@ -72,20 +74,36 @@ template <typename T, int N, int TC, int NV> struct JobInvZ {
         if (s.col < plane) {
             const int kx = (int)(s.col % ldk), ky = wavenumber((int)(s.col / ldk), N);
             s.kxy2 = kx * kx + ky * ky;
+            s.ky = ky;
             s.active = 9 * s.kxy2 < N * N;
         }
         return __syncthreads_or(s.active) != 0;
     }
-    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    __device__ __forceinline__ bool keep(const State &s, int i) const
     {
         const int kz = wavenumber(i, N);
-        if (!s.active || 9 * (s.kxy2 + kz * kz) >= N * N) return mk<T>(0, 0);
-        const int v = r / 5, rr = r % 5;
-        const int comp = rr < 3 ? rr : rr - 3;
-        const C *p = (NV == 2 && v == 1) ? src[NV - 1] : src[0];
-        C x = ldg_c(p + comp * nf + i * plane + s.col);
-        if (rr >= 3) x = mul_ik(x, (T)kz);
+        return s.active && 9 * (s.kxy2 + kz * kz) < N * N;
+    }
+    __device__ __forceinline__ const C *field(int r) const { return (NV == 2 && r >= 5) ? src[NV - 1] : src[0]; }
+    // rr: 0..2 A_c <- u_c | 3 B_x <- i kz u_x | 4 G_x <- i (ky u_z - kz u_y)
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        const int rr = r % 5;
+        const int comp = rr < 3 ? rr : rr == 3 ? 0 : 2;
+        C x = mk<T>(0, 0);
+        if (keep(s, i)) x = ldg_c(field(r) + comp * nf + i * plane + s.col);
         return x;
+    }
+    __device__ __forceinline__ C post(const State &s, int r, int i, C x) const
+    {
+        const int rr = r % 5;
+        if (rr < 3) return x;
+        const T kz = (T)wavenumber(i, N);
+        if (rr == 3) return mul_ik(x, kz);
+        C y = mk<T>(0, 0);
+        if (keep(s, i)) y = ldg_c(field(r) + nf + i * plane + s.col);   // u_y (sparse, L1/L2 resident)
+        const T ky = (T)s.ky;
+        return mk<T>(-(ky * x.y - kz * y.y), ky * x.x - kz * y.x);
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
@@ -110,18 +128,20 @@ template <typename T, int N, int TC, int NV> struct JobInvY {
         s.base = (long)blockIdx.y * plane + s.kx;
         return true;
     }
+    // rr: 0 U_x <- A_x | 1 U_y <- A_y | 2 U_z <- A_z | 3 W_x <- G_x | 4 P <- B_x | 5 D <- i ky A_x
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
         const int ky = wavenumber(i, N);
-        if (!s.active || 9 * (s.kx * s.kx + ky * ky) >= N * N) return mk<T>(0, 0);
         const int v = r / 6, rr = r % 6;
-        // rr: 0 U_x <- A_x | 1 U_y <- A_y | 2 U_z <- A_z | 3 W_x <- i ky A_z - B_y | 4 P <- B_x | 5 D <- i ky A_x
-        const int fa = rr < 3 ? rr : rr == 3 ? 2 : rr == 4 ? 3 : 0;
-        const C *p = src + (long)(v * 5) * nf + s.base + (long)i * ldk;
-        C x = ld_stream(p + fa * nf);
-        if (rr == 3 || rr == 5) x = mul_ik(x, (T)ky);
-        if (rr == 3) x = csub(x, ld_stream(p + 4 * nf));
+        const int fa = rr < 3 ? rr : rr == 3 ? 4 : rr == 4 ? 3 : 0;
+        C x = mk<T>(0, 0);
+        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N)
+            x = ld_stream(src + (long)(v * 5 + fa) * nf + s.base + (long)i * ldk);
         return x;
+    }
+    __device__ __forceinline__ C post(const State &, int r, int i, C x) const
+    {
+        return (r % 6 == 5) ? mul_ik(x, (T)wavenumber(i, N)) : x;
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
@@ -147,8 +167,11 @@ template <typename T, int N, int TC> struct JobFwdY {
     }
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
-        return s.active ? ld_stream(buf + r * nf + s.base + (long)i * ldk) : mk<T>(0, 0);
+        C x = mk<T>(0, 0);
+        if (s.active) x = ld_stream(buf + r * nf + s.base + (long)i * ldk);
+        return x;
     }
+    __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
         const int ky = wavenumber(i, N);
@@ -195,8 +218,11 @@ template <typename T, int N, int TC, int NV> struct JobFwdZ {
     }
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
-        return s.active ? ld_stream(src + r * nf + i * plane + s.col) : mk<T>(0, 0);
+        C x = mk<T>(0, 0);
+        if (s.active) x = ld_stream(src + r * nf + i * plane + s.col);
+        return x;
     }
+    __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
         if (!s.valid) return;
