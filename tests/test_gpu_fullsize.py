@@ -1,0 +1,160 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+* 512^3 fp64 (configs[2] and the metric's HD RHS): the oracle is fast enough on the GPU box's host cores
+  for a full element-by-element comparison; sampled O(N^3)-per-mode brute-force sums pin the transform
+  independently of the oracle's FFT.
+* 768^3 fp32 (configs[3]) and 1024^3 fp32 MHD (configs[4]): a full-size fp64 oracle does not fit / takes
+  minutes, so parity uses the grid-independence property P12: the same band-limited
+  coefficients on a 256^3 grid give the same right-hand-side coefficients mode by mode, and everything
+  outside that box must vanish -- plus conservation invariants and the fused-vs-unfused cross-check.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_1808_01309_b200 import psfft, synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    num = np.linalg.norm((a.astype(b.dtype) - b).ravel())
+    return num / max(np.linalg.norm(b.ravel()), 1e-300)
+
+
+def half_weights(N):
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = w[-1] = 1.0
+    return w[None, None, :]
+
+
+def box_compare(G, N, g, n, K):
+    """P12: compare G/N^3 (big grid) with g/n^3 (oracle grid) on the box |k_i| <= K; everything of G outside
+    the box counts as error.  Returns the relative L2 error."""
+    idxN = np.r_[0:K + 1, N - K:N]
+    idxn = np.r_[0:K + 1, n - K:n]
+    big = G[:, idxN][:, :, idxN][:, :, :, :K + 1].astype(np.complex128) / float(N) ** 3
+    small = g[:, idxn][:, :, idxn][:, :, :, :K + 1] / float(n) ** 3
+    w = np.full(K + 1, 2.0)
+    w[0] = 1.0
+    num = np.sum(w * np.abs(big - small) ** 2)
+    den = np.sum(w * np.abs(small) ** 2)
+    wN = half_weights(N)
+    for c in range(G.shape[0]):                      # energy of G outside the box, summed directly (no cancellation)
+        A = G[c].astype(np.complex128) / float(N) ** 3
+        A[np.ix_(idxN, idxN, np.arange(K + 1))] = 0.0
+        num += float(np.sum(wN * np.abs(A) ** 2))
+        del A
+    return float(np.sqrt(num / den))
+
+
+# ---- configs[2]: 512^3 fp64 batch 3 -------------------------------------------------------------------
+
+def test_config3_fft_512_fp64_batch3():
+    N, B = 512, 3
+    x = synth.uniform_field(N, B, 1234)
+    p = psfft.Plan(N, torch.float64, B)
+    xd = torch.from_numpy(x).cuda()
+    X = p.r2c(xd)
+    back = p.c2r(X)
+    assert float((back - xd).abs().max()) < 1e-13                                   # P4 at full size, all 3 fields
+    Xh = X.cpu().numpy()
+    # element by element against the oracle, one field
+    assert rel(Xh[1], oracle.r2c3d(x[1])) < 1e-12
+    assert rel(back[1].cpu().numpy(), oracle.c2r3d(Xh[1])) < 1e-12
+    # sampled outputs against the O(N^3) triple sum (independent of any FFT), every field
+    rng = np.random.default_rng(0)
+    scale = np.sqrt(np.mean(np.abs(Xh[0]) ** 2))
+    for b in range(B):
+        for _ in range(4):
+            r, q, pp = int(rng.integers(N)), int(rng.integers(N)), int(rng.integers(N // 2 + 1))
+            assert abs(Xh[b, r, q, pp] - oracle.r2c3d_mode(x[b], r, q, pp)) < 1e-11 * scale
+    # P3 Parseval per field
+    w = half_weights(N)
+    for b in range(B):
+        lhs = float(np.sum(x[b] ** 2))
+        rhs = float(np.sum(w * np.abs(Xh[b]) ** 2)) / N**3
+        assert abs(lhs - rhs) / lhs < 1e-13
+
+
+# ---- the metric's workload: 512^3 fp64 HD RHS ----------------------------------------------------------
+
+def test_metric_hd_rhs_512_fp64():
+    N = 512
+    uh = synth.solenoidal_spectrum(N, 4.0, 32, 1234)
+    p = psfft.Plan(N, torch.float64, 3, work="hd")
+    ud = torch.from_numpy(uh).cuda()
+    got_d = p.hd_rhs(ud)
+    unf = torch.empty_like(got_d)
+    psfft.hd_rhs_unfused(p.handle, ud, unf, 0.0, p._work)
+    assert float((got_d - unf).norm() / unf.norm()) < 1e-13                         # two CUDA paths agree
+    del unf
+    got = got_d.cpu().numpy()
+    want = oracle.hd_rhs(uh, 0.0)                                                   # full size, element by element
+    assert rel(got, want) < 1e-12
+    M = oracle.dealias_mask(N)
+    assert np.all(got[:, ~M] == 0)                                                   # mask bit-exact
+    del want
+    # P12 against the 256^3 oracle and P9 invariants
+    g = oracle.hd_rhs(synth.solenoidal_spectrum(256, 4.0, 32, 1234), 0.0)
+    assert box_compare(got, N, g, 256, 64) < 1e-12
+    w = half_weights(N)
+    assert abs(np.sum(w * (np.conj(uh) * got).real)) / (np.sqrt(np.sum(w * np.abs(uh) ** 2)) * np.sqrt(np.sum(w * np.abs(got) ** 2))) < 1e-13
+
+
+# ---- configs[3]: 768^3 fp32 HD RHS ---------------------------------------------------------------------
+
+def test_config4_hd_rhs_768_fp32():
+    N = 768
+    uh = synth.solenoidal_spectrum(N, 4.0, 32, 1234, dtype=np.complex64)
+    p = psfft.Plan(N, torch.float32, 1, work="hd")
+    ud = torch.from_numpy(uh).cuda()
+    got_d = p.hd_rhs(ud)
+    unf = torch.empty_like(got_d)
+    psfft.hd_rhs_unfused(p.handle, ud, unf, 0.0, p._work)
+    assert float((got_d - unf).norm() / unf.norm()) < 2e-5
+    del unf
+    got = got_d.cpu().numpy()
+    g = oracle.hd_rhs(synth.solenoidal_spectrum(256, 4.0, 32, 1234), 0.0)
+    assert box_compare(got, N, g, 256, 64) < 2e-5
+    # strict '<' of the 2/3 rule matters at N = 768 (3 | N): the axis points |k| = 256 are masked
+    assert np.all(got[:, 0, 0, 256] == 0) and np.all(got[:, 0, 256, 0] == 0) and np.all(got[:, 256, 0, 0] == 0)
+    # masked region exactly zero: every Nyquist plane and the far corner
+    assert np.all(got[:, :, :, 256:] == 0) and np.all(got[:, 256:513] == 0) and np.all(got[:, :, 256:513] == 0)
+
+
+# ---- configs[4]: 1024^3 fp32 MHD RHS -------------------------------------------------------------------
+
+def test_config5_mhd_rhs_1024_fp32():
+    N = 1024
+    free, _ = torch.cuda.mem_get_info()
+    lay = psfft.plan_query(N, psfft.F32, 1)
+    need = lay.work_bytes_mhd + 12 * lay.spec_bytes
+    if free < need + (2 << 30):
+        pytest.skip(f"needs {need / 2**30:.0f} GiB of device memory, {free / 2**30:.0f} GiB free")
+    uh = synth.solenoidal_spectrum(N, 3.0, 24, 1234, tag=0, dtype=np.complex64)
+    bh = synth.solenoidal_spectrum(N, 3.0, 24, 1234, tag=1, dtype=np.complex64)
+    p = psfft.Plan(N, torch.float32, 1, work="mhd")
+    ru, rb = p.mhd_rhs(torch.from_numpy(uh).cuda(), torch.from_numpy(bh).cuda())
+    ru, rb = ru.cpu().numpy(), rb.cpu().numpy()
+    del p
+    torch.cuda.empty_cache()
+    gu, gb = oracle.mhd_rhs(synth.solenoidal_spectrum(256, 3.0, 24, 1234, tag=0),
+                            synth.solenoidal_spectrum(256, 3.0, 24, 1234, tag=1))
+    assert box_compare(ru, N, gu, 256, 48) < 2e-5
+    assert box_compare(rb, N, gb, 256, 48) < 2e-5
+    # P10: total energy and cross helicity (fp32 roundoff level)
+    K = 48
+    idx = np.r_[0:K + 1, N - K:N]
+    sub = lambda a: a[:, idx][:, :, idx][:, :, :, :K + 1].astype(np.complex128)
+    w = np.full(K + 1, 2.0)
+    w[0] = 1.0
+    dot = lambda a, b: float(np.sum(w * (np.conj(a) * b).real))
+    u, b, Ru, Rb = sub(uh), sub(bh), sub(ru), sub(rb)
+    s = np.sqrt(dot(u, u) * dot(Ru, Ru)) + np.sqrt(dot(b, b) * dot(Rb, Rb))
+    assert abs(dot(u, Ru) + dot(b, Rb)) / s < 1e-5
+    assert abs(dot(b, Ru) + dot(u, Rb)) / s < 1e-5
