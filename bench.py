@@ -131,13 +131,18 @@ def hbm_peak():
 
 
 def ncu_traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(kernel)
-        except Exception:
-            return None
+    """dram bytes (read + write) per launch of `kernel` from the committed ncu --set full capture
+    (profiles/traffic.csv: kernel,dram_bytes_per_launch,source), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    try:
+        for line in open(p).read().splitlines()[1:]:
+            cols = line.split(",")
+            if cols and cols[0] == kernel:
+                return float(cols[1])
+    except Exception:
+        return None
     return None
 
 
