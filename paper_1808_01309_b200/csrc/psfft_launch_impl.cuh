@@ -3,6 +3,7 @@
 #pragma once
 #include "psfft_kernels.cuh"
 #include "psfft_rhs.cuh"
+#include "psfft_midx8.cuh"
 #include "psfft_launch.cuh"
 #include <stdlib.h>
 
@@ -152,16 +153,30 @@ template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassAr
 template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TPF = threads_per_fft(N / 2);
-    constexpr size_t smem = (size_t)6 * NV * RowMap<N / 2>::ld * sizeof(C);
-    auto kern = k_mid_x<T, N, NV>;
-    cudaError_t e = set_smem(kern, smem);
-    if (e != cudaSuccess) return e;
     const long nf = (long)a.ldk * N * N;
-    const T scale = (T)(1.0 / ((double)N * N * N));
-    kern<<<(unsigned)(N * N), 6 * NV * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
-                                                               (const C *)a.twM, nf, a.ldk, scale);
-    return cudaGetLastError();
+    if constexpr (N == 64 || N == 512) {
+        // radix-8 two-for-one kernel (psfft_midx8.cuh): one butterfly per thread and stage
+        using L = Mid8<N, (int)sizeof(C)>;
+        constexpr int MINB = (sizeof(T) == 8 ? 4 : 8) / NV;
+        constexpr size_t smem = (size_t)3 * NV * L::BUF * sizeof(C);
+        auto kern = k_mid_x8<T, N, NV, MINB>;
+        cudaError_t e = set_smem(kern, smem);
+        if (e != cudaSuccess) return e;
+        const T scale2 = (T)(1.0 / ((double)N * N * N * (double)N * N * N));   // both c2r factors, applied to the product
+        kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, nf, a.ldk,
+                                                           scale2);
+        return cudaGetLastError();
+    } else {
+        constexpr int TPF = threads_per_fft(N / 2);
+        constexpr size_t smem = (size_t)6 * NV * RowMap<N / 2>::ld * sizeof(C);
+        auto kern = k_mid_x<T, N, NV>;
+        cudaError_t e = set_smem(kern, smem);
+        if (e != cudaSuccess) return e;
+        const T scale = (T)(1.0 / ((double)N * N * N));
+        kern<<<(unsigned)(N * N), 6 * NV * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
+                                                                   (const C *)a.twM, nf, a.ldk, scale);
+        return cudaGetLastError();
+    }
 }
 
 template <typename T, int N, int NV> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)
