@@ -109,8 +109,10 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     o->spec_bytes = o->spec_elems * 2 * s;
     o->table_bytes = table_entries(N, nullptr, nullptr) * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
-    o->work_bytes_hd = 12 * o->spec_bytes;
-    o->work_bytes_mhd = 24 * o->spec_bytes;
+    // fused path: 5 + 6 compact fields [N][N][kx_pitch] per vector field; unfused path: 12 C per vector field
+    const size_t wfield = (size_t)N * N * kx_pitch(N, cpass_cols(N, (int)(2 * s))) * 2 * s;
+    o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
+    o->work_bytes_mhd = 2 * o->work_bytes_hd;
     return PSFFT_OK;
 }
 
@@ -185,8 +187,9 @@ int rhs_fused_t(Plan *pl, const PassArgs &a, int nv, const void *uhat, const voi
     r.src[0] = uhat; r.src[1] = bhat;
     r.dst[0] = ru; r.dst[1] = rb;
     r.diff[0] = nu; r.diff[1] = eta;
-    r.zbuf = work;
-    r.ybuf = off(work, (size_t)5 * nv * C);
+    const size_t W = (size_t)a.N * a.N * kx_pitch(a.N, cpass_cols(a.N, (int)(2 * sizeof(T)))) * 2 * sizeof(T);
+    r.zbuf = work;                              // 5 nv compact fields (later 3 nv: mid_x out, fwd_y in place)
+    r.ybuf = off(work, (size_t)5 * nv * W);     // 6 nv compact fields
     const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
     const double ndiff = (nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && eta != 0.0 ? 3.0 : 0.0);
     { ProfScope ps(pl, a.stream, K_INVZ, nv * (3 * sph + 5 * disc)); CU(launch_rhs_inv_z<T>(a, r, &pl->launches)); }

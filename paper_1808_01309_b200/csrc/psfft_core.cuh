@@ -75,6 +75,24 @@ __host__ __device__ constexpr bool supported_len(int L)
     return L >= 4 && (rem == 1 || rem == 3);
 }
 
+// column passes: 16 elements per thread for N >= 128 (two radix-8 butterflies in flight), and TC
+// contiguous columns per CTA: 128-byte tile rows, capped so a tile stays within 64 KB, widened for
+// small N until a CTA has at least 128 threads.  (Measured on B200, 512^3 fp64: 64-byte rows run
+// the z-pass at 3.5 TB/s, 128-byte rows at 5.4 TB/s; profiles/r1a_summary.md.)
+__host__ __device__ constexpr int cpass_tpf(int N) { return N >= 128 ? N / 16 : threads_per_fft(N); }
+__host__ __device__ constexpr int cpass_cols(int N, int csize)
+{
+    int tc = 128 / csize;
+    while (tc > 1 && (long)N * tc * csize > 65536) tc /= 2;
+    while (tc * cpass_tpf(N) < 128 && (long)N * tc * 2 * csize <= 65536) tc *= 2;
+    return tc;
+}
+
+// number of kx with 9 kx^2 < N^2 (2/3-rule), and the compact row pitch of the RHS workspace fields:
+// kx_count rounded up to whole tiles of TC columns
+__host__ __device__ constexpr int kx_count(int N) { return (N - 1) / 3 + 1; }
+__host__ __device__ constexpr int kx_pitch(int N, int TC) { return (kx_count(N) + TC - 1) / TC * TC; }
+
 // Per-stage twiddle tables.  Stage with earlier radix product Ns (> 1) and radix R needs
 // w_{Ns R}^{r k}, k in [0, Ns), r in [1, R).  They are stored as [r-1][k] (k contiguous, so the
 // lanes of a warp -- consecutive k -- read consecutive 16-byte entries), stage after stage.

@@ -16,19 +16,6 @@ __host__ __device__ constexpr int xpass_rows(int N)
     int tpf = threads_per_fft(N / 2);
     return tpf >= 256 ? 1 : 256 / tpf;
 }
-// column passes: 16 elements per thread for N >= 128 (two radix-8 butterflies in flight), and TC
-// contiguous columns per CTA: 128-byte tile rows, capped so a tile stays within 64 KB, widened for
-// small N until a CTA has at least 128 threads.  (Measured on B200, 512^3 fp64: 64-byte rows run
-// the z-pass at 3.5 TB/s, 128-byte rows at 5.4 TB/s; profiles/r1_notes.md.)
-__host__ __device__ constexpr int cpass_tpf(int N) { return N >= 128 ? N / 16 : threads_per_fft(N); }
-__host__ __device__ constexpr int cpass_cols(int N, int csize)
-{
-    int tc = 128 / csize;
-    while (tc > 1 && (long)N * tc * csize > 65536) tc /= 2;
-    while (tc * cpass_tpf(N) < 128 && (long)N * tc * 2 * csize <= 65536) tc *= 2;
-    return tc;
-}
-
 template <typename K> static cudaError_t set_smem(K kernel, size_t bytes)
 {
     if (bytes <= 48 * 1024) return cudaSuccess;
@@ -109,51 +96,76 @@ static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *ou
 }
 
 // ---- fused right-hand side -------------------------------------------------------------------
-template <typename T, int N, int DIR, class Job>
-static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid)
+template <typename T, int N, int DIR, int TPF, int MINB, class Job>
+static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int TPF = cpass_tpf(N);
     constexpr bool PAD = (TC * sizeof(C) < 128);
     constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(C);
-    auto kern = k_cpass_job<T, N, DIR, TC, TPF, 2, Job>;
+    auto kern = k_cpass_job<T, N, DIR, TC, TPF, MINB, Job>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, TC * TPF, smem, a.stream>>>(job, (const C *)a.twN);
     return cudaGetLastError();
 }
 
+// RHS column passes: 8 elements per thread (one radix-8 butterfly per stage) while the CTA stays within
+// 512 threads -- twice the warps of the 16-element shape for the same two tiles per SM (measured, 512^3
+// fp64: inv_y 1.67 -> 1.50 ms, fwd_y 0.85 -> 0.60 ms; profiles/r1b_summary.md)
+__host__ __device__ constexpr int job_tpf(int N, int TC)
+{
+    return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= 512) ? N / 8 : cpass_tpf(N);
+}
+
+template <typename T, int N, int DIR, class Job>
+static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid, int id = 0)
+{
+    constexpr int TC = cpass_cols(N, (int)sizeof(Cx<T>));
+#ifdef PSFFT_EXPERIMENT
+    if constexpr (N == 512 && sizeof(T) == 8) {
+        static const int v = getenv("PSFFT_JOB_VARIANT") ? atoi(getenv("PSFFT_JOB_VARIANT")) : 0;
+        if ((v >> id) & 1) return run_job_v<T, N, DIR, cpass_tpf(N), 2>(a, job, grid);
+    }
+#endif
+    (void)id;
+    return run_job_v<T, N, DIR, job_tpf(N, TC), 2>(a, job, grid);
+}
+
 template <typename T, int N, int NV> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    constexpr int KXP = kx_pitch(N, TC);
     JobInvZ<T, N, TC, NV> job;
     for (int v = 0; v < NV; ++v) job.src[v] = (const C *)r.src[v];
     job.dst = (C *)r.zbuf;
     job.plane = (long)a.ldk * N;
     job.nf = job.plane * N;
-    job.ldk = a.ldk;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)));
+    job.wplane = (long)KXP * N;
+    job.wnf = job.wplane * N;
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 0);
 }
 
 template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    constexpr int KXP = kx_pitch(N, TC);
     JobInvY<T, N, TC, NV> job;
     job.src = (const C *)r.zbuf;
     job.dst = (C *)r.ybuf;
-    job.plane = (long)a.ldk * N;
-    job.nf = job.plane * N;
-    job.ldk = a.ldk;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)((kx_count(N) + TC - 1) / TC), (unsigned)N));
+    job.wplane = (long)KXP * N;
+    job.wnf = job.wplane * N;
+    job.kxp = KXP;
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 1);
 }
 
 template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    const long nf = (long)a.ldk * N * N;
+    constexpr int KXP = kx_pitch(N, cpass_cols(N, (int)sizeof(C)));
+    const long wnf = (long)KXP * N * N;
     if constexpr (N == 64 || N == 512) {
         // radix-8 two-for-one kernel (psfft_midx8.cuh): one butterfly per thread and stage
         using L = Mid8<N, (int)sizeof(C)>;
@@ -163,7 +175,7 @@ template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassAr
         cudaError_t e = set_smem(kern, smem);
         if (e != cudaSuccess) return e;
         const T scale2 = (T)(1.0 / ((double)N * N * N * (double)N * N * N));   // both c2r factors, applied to the product
-        kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, nf, a.ldk,
+        kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, wnf, KXP,
                                                            scale2);
         return cudaGetLastError();
     } else {
@@ -174,7 +186,7 @@ template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassAr
         if (e != cudaSuccess) return e;
         const T scale = (T)(1.0 / ((double)N * N * N));
         kern<<<(unsigned)(N * N), 6 * NV * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
-                                                                   (const C *)a.twM, nf, a.ldk, scale);
+                                                                   (const C *)a.twM, wnf, KXP, scale);
         return cudaGetLastError();
     }
 }
@@ -183,19 +195,21 @@ template <typename T, int N, int NV> static cudaError_t rhs_fwd_y_n(const PassAr
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    constexpr int KXP = kx_pitch(N, TC);
     JobFwdY<T, N, TC> job;
     job.buf = (C *)r.zbuf;
-    job.plane = (long)a.ldk * N;
-    job.nf = job.plane * N;
-    job.ldk = a.ldk;
+    job.wplane = (long)KXP * N;
+    job.wnf = job.wplane * N;
+    job.kxp = KXP;
     job.nfields = 3 * NV;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)((kx_count(N) + TC - 1) / TC), (unsigned)N));
+    return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 2);
 }
 
 template <typename T, int N, int NV> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
+    constexpr int KXP = kx_pitch(N, TC);
     JobFwdZ<T, N, TC, NV> job;
     job.src = (const C *)r.zbuf;
     for (int v = 0; v < NV; ++v) {
@@ -205,8 +219,10 @@ template <typename T, int N, int NV> static cudaError_t rhs_fwd_z_n(const PassAr
     }
     job.plane = (long)a.ldk * N;
     job.nf = job.plane * N;
+    job.wplane = (long)KXP * N;
+    job.wnf = job.wplane * N;
     job.ldk = a.ldk;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)));
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)), 3);
 }
 
 #define PSFFT_RHS_LAUNCHER(name)                                                                       \

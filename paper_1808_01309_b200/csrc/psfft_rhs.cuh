@@ -20,15 +20,18 @@
 // Pruning: after the mask of step 1 (and before the mask of step 6) every mode with
 // 9 |k|^2 >= N^2 is zero (does not matter), so columns / rows that are entirely outside the
 // truncation sphere are neither read, transformed nor written, and loads inside a column are
-// predicated on the mode being retained.  Buffers are dense ([kz][ky][ldk]); the skipped
-// entries are simply never touched.
+// predicated on the mode being retained.
+//
+// Intermediate layout: every workspace field is [z][y][kxp] with the COMPACT row pitch
+// kxp = kx_pitch(N, TC) >= kx_count(N), a multiple of the tile width TC, so every 128-byte tile
+// row of the y passes, of mid_x and of the z passes' workspace side starts on a 128-byte line
+// (the caller's layout has the odd pitch ldk = N/2+1, whose tile rows straddle two lines).
+// Skipped entries of the workspace are simply never touched.
 #pragma once
 #include "psfft_kernels.cuh"
 
 namespace psfft {
 
-// number of kx with 9 kx^2 < N^2
-__host__ __device__ constexpr int kx_count(int N) { return (N - 1) / 3 + 1; }
 
 template <typename C, typename T> __device__ __forceinline__ C mul_ik(C v, T k) { return mk<T>(-k * v.y, k * v.x); }
 
@@ -57,26 +60,25 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
 }
 
 // ---- inv_z -------------------------------------------------------------------------------------
+// grid (kxp / TC, N): tile = TC consecutive kx at one ky.  Reads the caller's layout (pitch ldk),
+// writes the compact workspace layout (pitch kxp).
 template <typename T, int N, int TC, int NV> struct JobInvZ {
     using C = Cx<T>;
-    const C *src[NV];   // NV x 3 spectral fields (u^, b^)
+    const C *src[NV];   // NV x 3 spectral fields (u^, b^), caller layout
     C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x = F_z^-1(i kz u_x), G_x = F_z^-1(w^_x)
-    long plane, nf;
-    int ldk;
-    struct State { long col; int kxy2, ky; bool active; };
+    long plane, nf;     // caller layout: ldk N, ldk N N
+    long wplane, wnf;   // workspace layout: kxp N, kxp N N
+    struct State { long col, wcol; int kxy2, ky; bool active; };
 
     __device__ __forceinline__ int rounds() const { return 5 * NV; }
     __device__ __forceinline__ bool begin(State &s, int c, int) const
     {
-        s.col = (long)blockIdx.x * TC + c;
-        s.active = false;
-        s.kxy2 = 0;
-        if (s.col < plane) {
-            const int kx = (int)(s.col % ldk), ky = wavenumber((int)(s.col / ldk), N);
-            s.kxy2 = kx * kx + ky * ky;
-            s.ky = ky;
-            s.active = 9 * s.kxy2 < N * N;
-        }
+        const int kx = blockIdx.x * TC + c, ky = wavenumber((int)blockIdx.y, N);
+        s.kxy2 = kx * kx + ky * ky;
+        s.ky = ky;
+        s.active = 9 * s.kxy2 < N * N;
+        s.col = (long)blockIdx.y * (plane / N) + kx;
+        s.wcol = (long)blockIdx.y * (wplane / N) + kx;
         return __syncthreads_or(s.active) != 0;
     }
     __device__ __forceinline__ bool keep(const State &s, int i) const
@@ -107,17 +109,18 @@ template <typename T, int N, int TC, int NV> struct JobInvZ {
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
-        if (s.active) st_stream(dst + r * nf + i * plane + s.col, v);
+        if (s.active) st_stream(dst + r * wnf + i * wplane + s.wcol, v);
     }
 };
 
 // ---- inv_y -------------------------------------------------------------------------------------
+// grid (kxp / TC, N): tile = TC consecutive kx of one z plane, all in the compact layout.
 template <typename T, int N, int TC, int NV> struct JobInvY {
     using C = Cx<T>;
     const C *src;  // NV x 5 fields from inv_z
     C *dst;        // NV x 6 fields: U_x, U_y, U_z, W_x, P, D
-    long plane, nf;
-    int ldk;
+    long wplane, wnf;
+    int kxp;
     struct State { long base; int kx; bool active; };
 
     __device__ __forceinline__ int rounds() const { return 6 * NV; }
@@ -125,36 +128,40 @@ template <typename T, int N, int TC, int NV> struct JobInvY {
     {
         s.kx = blockIdx.x * TC + c;
         s.active = s.kx < kx_count(N);
-        s.base = (long)blockIdx.y * plane + s.kx;
+        s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
-    // rr: 0 U_x <- A_x | 1 U_y <- A_y | 2 U_z <- A_z | 3 W_x <- G_x | 4 P <- B_x | 5 D <- i ky A_x
+    // round order: U_x <- A_x | D <- i ky A_x | U_y | U_z | W_x <- G_x | P <- B_x.  A_x is read in two
+    // consecutive rounds: the first read leaves it in L2 (default policy), the second streams.
+    __device__ __forceinline__ static int src_field(int rr) { return rr == 0 ? 0 : rr == 1 ? 0 : rr == 2 ? 1 : rr == 3 ? 2 : rr == 4 ? 4 : 3; }
+    __device__ __forceinline__ static int dst_field(int rr) { return rr == 0 ? 0 : rr == 1 ? 5 : rr == 2 ? 1 : rr == 3 ? 2 : rr == 4 ? 3 : 4; }
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
         const int ky = wavenumber(i, N);
         const int v = r / 6, rr = r % 6;
-        const int fa = rr < 3 ? rr : rr == 3 ? 4 : rr == 4 ? 3 : 0;
         C x = mk<T>(0, 0);
-        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N)
-            x = ld_stream(src + (long)(v * 5 + fa) * nf + s.base + (long)i * ldk);
+        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) {
+            const C *p = src + (long)(v * 5 + src_field(rr)) * wnf + s.base + (long)i * kxp;
+            x = rr == 0 ? *p : ld_stream(p);
+        }
         return x;
     }
     __device__ __forceinline__ C post(const State &, int r, int i, C x) const
     {
-        return (r % 6 == 5) ? mul_ik(x, (T)wavenumber(i, N)) : x;
+        return (r % 6 == 1) ? mul_ik(x, (T)wavenumber(i, N)) : x;
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
-        if (s.active) st_stream(dst + r * nf + s.base + (long)i * ldk, v);
+        if (s.active) st_stream(dst + (long)((r / 6) * 6 + dst_field(r % 6)) * wnf + s.base + (long)i * kxp, v);
     }
 };
 
 // ---- fwd_y -------------------------------------------------------------------------------------
 template <typename T, int N, int TC> struct JobFwdY {
     using C = Cx<T>;
-    C *buf;  // NF fields, in place
-    long plane, nf;
-    int ldk, nfields;
+    C *buf;  // NF fields, in place, compact layout
+    long wplane, wnf;
+    int kxp, nfields;
     struct State { long base; int kx; bool active; };
 
     __device__ __forceinline__ int rounds() const { return nfields; }
@@ -162,20 +169,20 @@ template <typename T, int N, int TC> struct JobFwdY {
     {
         s.kx = blockIdx.x * TC + c;
         s.active = s.kx < kx_count(N);
-        s.base = (long)blockIdx.y * plane + s.kx;
+        s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
         C x = mk<T>(0, 0);
-        if (s.active) x = ld_stream(buf + r * nf + s.base + (long)i * ldk);
+        if (s.active) x = ld_stream(buf + r * wnf + s.base + (long)i * kxp);
         return x;
     }
     __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
         const int ky = wavenumber(i, N);
-        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) st_stream(buf + r * nf + s.base + (long)i * ldk, v);
+        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) st_stream(buf + r * wnf + s.base + (long)i * kxp, v);
     }
 };
 
@@ -184,26 +191,33 @@ template <typename T, int N, int TC> struct JobFwdY {
 // (momentum), 1 -> i k x f - d |k|^2 a (induction); a = aux[g] (u^ or b^), d = diff[g].
 template <typename T, int N, int TC, int NV> struct JobFwdZ {
     using C = Cx<T>;
-    const C *src;        // NV x 3 fields (after fwd_y)
-    C *dst[NV];          // NV outputs of 3 fields
+    const C *src;        // NV x 3 fields (after fwd_y), compact layout
+    C *dst[NV];          // NV outputs of 3 fields, caller layout
     const C *aux[NV];    // u^, b^ for the diffusion term
     T diff[NV];
-    long plane, nf;
+    long plane, nf;      // caller layout
+    long wplane, wnf;    // workspace layout
     int ldk;
-    struct State { long col; int kx, ky, kxy2; bool active, valid; };
+    struct State { long col, wcol; int kx, ky, kxy2; bool active, valid; };
 
     __device__ __forceinline__ int rounds() const { return 3 * NV; }
+    // grid (ceil(ldk N / TC)): tile = TC consecutive columns of the caller's (ky, kx) plane, whose
+    // 128-byte rows are line-aligned (the plane size ldk N is a multiple of TC); the workspace side
+    // is read at the compact address of the same (ky, kx)
     __device__ __forceinline__ bool begin(State &s, int c, int t) const
     {
         s.col = (long)blockIdx.x * TC + c;
         s.valid = s.col < plane;
         s.active = false;
         s.kx = s.ky = s.kxy2 = 0;
+        s.wcol = 0;
         if (s.valid) {
             s.kx = (int)(s.col % ldk);
-            s.ky = wavenumber((int)(s.col / ldk), N);
+            const int q = (int)(s.col / ldk);
+            s.ky = wavenumber(q, N);
             s.kxy2 = s.kx * s.kx + s.ky * s.ky;
             s.active = 9 * s.kxy2 < N * N;
+            s.wcol = (long)q * (wplane / N) + s.kx;
         }
         if (__syncthreads_or(s.active)) return true;
         // nothing retained in this tile: the output is all zeros
@@ -219,7 +233,7 @@ template <typename T, int N, int TC, int NV> struct JobFwdZ {
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
         C x = mk<T>(0, 0);
-        if (s.active) x = ld_stream(src + r * nf + i * plane + s.col);
+        if (s.active) x = ld_stream(src + r * wnf + i * wplane + s.wcol);
         return x;
     }
     __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
