@@ -180,3 +180,15 @@ def mhd_rhs(uhat, bhat, nu: float = 0.0, eta: float = 0.0):
     _load().orc_mhd_rhs(ctypes.c_int(N), _p(u), _p(b), ctypes.c_double(nu), ctypes.c_double(eta), _p(ru),
                         _p(rb))
     return ru, rb
+
+
+def boussinesq_rhs(uhat, thhat, nu: float = 0.0, kappa: float = 0.0, nbv: float = 0.0):
+    """O8: (R_u, R_theta) of the Boussinesq equations, Eqs. 1-3:
+    R_u = M P (F[u x w] - N_bv theta^ z^) - nu |k|^2 M u^,  R_th = -M F[u . grad theta] + N_bv M u^_z - kappa |k|^2 M theta^."""
+    u, t = _c128(uhat), _c128(thhat)
+    N = u.shape[-2]
+    assert u.shape == (3, N, N, N // 2 + 1) and t.shape == (N, N, N // 2 + 1)
+    ru, rt = np.empty_like(u), np.empty_like(t)
+    _load().orc_boussinesq_rhs(ctypes.c_int(N), _p(u), _p(t), ctypes.c_double(nu), ctypes.c_double(kappa),
+                               ctypes.c_double(nbv), _p(ru), _p(rt))
+    return ru, rt

@@ -4,7 +4,7 @@
  * A plain, slow, obviously-correct double-precision implementation of what the hot path
  * of arxiv 1808.01309 computes: the unnormalised 3D real-to-complex DFT of PAPER.md:62
  * (Sec. 2, Eq. 8), its complex-to-real inverse, and one pseudospectral
- * Navier-Stokes / MHD right-hand side (Eqs. 1,3,4-6).
+ * Navier-Stokes / MHD / Boussinesq right-hand side (Eqs. 1-6).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
  * may call this.  It shares no code, header, table or helper with the CUDA path under
@@ -14,7 +14,9 @@
  *
  * Parity pins (tests/test_oracle_*.py): brute-force O(N^6) DFT, single mode -> exact bin,
  * Parseval, round trip, numpy pocketfft, closed-form derivative, Taylor-Green closed form,
- * ABC null test, energy/helicity invariants, mask counts, grid independence.  Every
+ * ABC null test, energy/helicity invariants, mask counts, grid independence; for the Boussinesq
+ * right-hand side (tests/test_oracle_boussinesq.py): theta = 0 -> O6, Taylor-Green + sin x closed
+ * form, hydrostatic balance, the N_bv w source, total-energy conservation, numpy restatement.  Every
  * exported function below is pinned by at least one of them; none is "parity unpinned".
  *
  * Conventions: real field [z][y][x], x contiguous; half spectrum
@@ -490,4 +492,81 @@ void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double et
     free(th);
     free(um);
     free(bm);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O8  boussinesq_rhs (Eqs. 1-3, the paper's reference equations):
+ *       d_t u     = -grad p - u.grad u - N_bv theta z^ + nu Lap u      (Eq. 1)
+ *       d_t theta = -u.grad theta + N_bv w + kappa Lap theta           (Eq. 2),  div u = 0 (Eq. 3)
+ *     Nonlinear terms in physical space, pressure by projection in spectral space.
+ *     Step by step (rotational form for the momentum term as in O6, reading G5):
+ *       1. um = M u^, tm = M theta^                       (2/3-rule mask on load)
+ *       2. w^ = i k x um;  g^ = i k tm                    (curl and gradient in spectral space)
+ *       3. u, w, g = c2r3d(.)                             (9 inverse transforms)
+ *       4. n = u x w;  s = u . g                          (pointwise)
+ *       5. n^ = r2c3d(n) (3), s^ = r2c3d(s) (1)           (4 forward transforms)
+ *       6. n^ <- M n^, s^ <- M s^
+ *       7. n^_z <- n^_z - N_bv tm;  n^ <- P n^            (buoyancy is inside the projection: Eq. 1)
+ *       8. R_u = n^ - nu |k|^2 um
+ *       9. R_th = -s^ + N_bv um_z - kappa |k|^2 tm
+ *     uhat, ru: [3][kz][ky][kx]; thhat, rt: [kz][ky][kx]; values = N^3 x Fourier coefficient.
+ * ------------------------------------------------------------------------------------- */
+void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, double kappa,
+                        double nbv, cplx *ru, cplx *rt)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H, nr = (long)N * N * N;
+    cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    cplx *tm = (cplx *)malloc(sizeof(cplx) * nf);
+    cplx *wh = (cplx *)malloc(sizeof(cplx) * 3 * nf);
+    double *u = (double *)malloc(sizeof(double) * 3 * nr);
+    double *w = (double *)malloc(sizeof(double) * 3 * nr);
+    memcpy(um, uhat, sizeof(cplx) * 3 * nf);
+    memcpy(tm, thhat, sizeof(cplx) * nf);
+    orc_apply_mask(N, 3, um);                                   /* 1 */
+    orc_apply_mask(N, 1, tm);
+    orc_curl(N, um, wh);                                        /* 2 (curl) */
+    for (int c = 0; c < 3; ++c) {                               /* 3 (u, w) */
+        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
+        orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);
+    }
+    double *n = (double *)malloc(sizeof(double) * 3 * nr);
+    cross_add(nr, u, w, n, 0);                                  /* 4 (n = u x w) */
+#pragma omp parallel for schedule(static)                       /* 2 (gradient), reusing wh */
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p) {
+                long o = ((long)r * N + q) * H + p;
+                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                wh[o] = I * kx * tm[o];
+                wh[nf + o] = I * ky * tm[o];
+                wh[2 * nf + o] = I * kz * tm[o];
+            }
+    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);   /* 3 (g) */
+    free(wh);
+    double *s = (double *)malloc(sizeof(double) * nr);
+#pragma omp parallel for schedule(static)                       /* 4 (s = u . g) */
+    for (long i = 0; i < nr; ++i) s[i] = u[i] * w[i] + u[nr + i] * w[nr + i] + u[2 * nr + i] * w[2 * nr + i];
+    free(u);
+    free(w);
+    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, n + c * nr, ru + c * nf);   /* 5 */
+    orc_r2c3d(N, N, N, s, rt);
+    free(n);
+    free(s);
+    orc_apply_mask(N, 3, ru);                                   /* 6 */
+    orc_apply_mask(N, 1, rt);
+    for (long o = 0; o < nf; ++o) ru[2 * nf + o] -= nbv * tm[o];               /* 7 */
+    orc_project(N, ru);
+    if (nu != 0.0) add_diffusion(N, nu, um, ru);                /* 8 */
+#pragma omp parallel for schedule(static)                       /* 9 */
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int p = 0; p < H; ++p) {
+                long o = ((long)r * N + q) * H + p;
+                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                double k2 = kx * kx + ky * ky + kz * kz;
+                rt[o] = -rt[o] + nbv * um[2 * nf + o] - kappa * k2 * tm[o];
+            }
+    free(um);
+    free(tm);
 }

@@ -161,6 +161,22 @@ template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassAr
     return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 1);
 }
 
+template <typename T, int N, int NV, int MINB>
+static cudaError_t mid_x8_launch(const PassArgs &a, const RhsArgs &r, long wnf, int kxp)
+{
+    using C = Cx<T>;
+    using L = Mid8<N, (int)sizeof(C)>;
+    constexpr size_t smem = (size_t)3 * NV * L::BUF * sizeof(C);
+    auto kern = k_mid_x8<T, N, NV, MINB>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    const T scale2 = (T)(1.0 / ((double)N * N * N * (double)N * N * N));   // both c2r factors, applied to the product
+    kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, wnf, kxp, scale2);
+    return cudaGetLastError();
+}
+
 template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
@@ -168,16 +184,15 @@ template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassAr
     const long wnf = (long)KXP * N * N;
     if constexpr (N == 64 || N == 512) {
         // radix-8 two-for-one kernel (psfft_midx8.cuh): one butterfly per thread and stage
-        using L = Mid8<N, (int)sizeof(C)>;
         constexpr int MINB = (sizeof(T) == 8 ? 4 : 8) / NV;
-        constexpr size_t smem = (size_t)3 * NV * L::BUF * sizeof(C);
-        auto kern = k_mid_x8<T, N, NV, MINB>;
-        cudaError_t e = set_smem(kern, smem);
-        if (e != cudaSuccess) return e;
-        const T scale2 = (T)(1.0 / ((double)N * N * N * (double)N * N * N));   // both c2r factors, applied to the product
-        kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, wnf, KXP,
-                                                           scale2);
-        return cudaGetLastError();
+#ifdef PSFFT_EXPERIMENT
+        if constexpr (N == 512 && sizeof(T) == 8 && NV == 1) {
+            static const int v = getenv("PSFFT_MIDX_VARIANT") ? atoi(getenv("PSFFT_MIDX_VARIANT")) : 0;
+            if (v == 4) return mid_x8_launch<T, N, NV, 4>(a, r, wnf, KXP);
+            if (v == 5) return mid_x8_launch<T, N, NV, 5>(a, r, wnf, KXP);
+        }
+#endif
+        return mid_x8_launch<T, N, NV, MINB>(a, r, wnf, KXP);
     } else {
         constexpr int TPF = threads_per_fft(N / 2);
         constexpr size_t smem = (size_t)6 * NV * RowMap<N / 2>::ld * sizeof(C);

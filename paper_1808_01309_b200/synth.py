@@ -137,6 +137,40 @@ def solenoidal_spectrum(N: int, k0: float = 4.0, kcut: int | None = None, seed: 
     return u.astype(dtype)
 
 
+def scalar_coefficients(k0: float, kcut: int, seed: int = 1234, tag: int = 7):
+    """Grid-independent Fourier coefficients of a random-phase real SCALAR field (the temperature
+    fluctuation theta of the Boussinesq runs): same shell amplitude as the
+    velocity recipe, one uniform phase per canonical wavevector keyed on ``(seed, tag, kx, ky, kz)``,
+    scaled to unit variance-energy 1/2 <theta^2> = 1.  Returns ``(kx, ky, kz, a)``."""
+    r = np.arange(-kcut, kcut + 1)
+    kx, ky, kz = np.meshgrid(np.arange(0, kcut + 1), r, r, indexing="ij")
+    kx, ky, kz = kx.ravel(), ky.ravel(), kz.ravel()
+    k2 = kx * kx + ky * ky + kz * kz
+    canon = (kx > 0) | ((kx == 0) & ((ky > 0) | ((ky == 0) & (kz > 0))))
+    sel = canon & (k2 >= 1) & (k2 <= kcut * kcut)
+    kx, ky, kz, k2 = kx[sel], ky[sel], kz[sel], k2[sel].astype(np.float64)
+    ph = 2.0 * np.pi * _variate(_key(seed, tag, kx, ky, kz), 0)
+    amp = np.sqrt(k2 * k2 * np.exp(-2.0 * k2 / (k0 * k0)) / (4.0 * np.pi * k2))
+    a = amp * np.exp(1j * ph)
+    return kx, ky, kz, a / np.sqrt(np.sum(np.abs(a) ** 2))
+
+
+def scalar_spectrum(N: int, k0: float = 4.0, kcut: int | None = None, seed: int = 1234, tag: int = 7,
+                    dtype=np.complex128) -> np.ndarray:
+    """Half spectrum ``thhat[kz][ky][kx]`` (= N^3 a_k) of the random scalar field."""
+    if kcut is None:
+        kcut = int(8 * k0)
+    if kcut >= N // 2:
+        raise ValueError("kcut must be below the Nyquist wavenumber")
+    kx, ky, kz, a = scalar_coefficients(k0, kcut, seed, tag)
+    t = np.zeros((N, N, N // 2 + 1), dtype=np.complex128)
+    scale = float(N) ** 3
+    t[kz % N, ky % N, kx] = a * scale
+    on0 = kx == 0
+    t[(-kz[on0]) % N, (-ky[on0]) % N, 0] = np.conj(a[on0]) * scale
+    return t.astype(dtype)
+
+
 def grid_axes(N: int):
     """Physical coordinates X_i = 2 pi i / N as broadcastable [z][y][x] arrays (returns x, y, z)."""
     t = 2.0 * np.pi * np.arange(N) / N
