@@ -70,6 +70,7 @@ typedef struct psfft_layout {
     size_t work_bytes_fft;       /* workspace for psfft_fft3d_r2c / c2r (batch fields) */
     size_t work_bytes_hd;        /* workspace for psfft_hd_rhs */
     size_t work_bytes_mhd;       /* workspace for psfft_mhd_rhs */
+    size_t work_bytes_boussinesq; /* workspace for psfft_boussinesq_rhs */
 } psfft_layout;
 
 /* Sizes for a prospective plan.  Supported N: 2^a * 3^b with b <= 1 and 8 <= N <= 1024
@@ -123,6 +124,23 @@ int psfft_hd_rhs(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, vo
  * 12 inverse + 6 forward transforms.  d_work >= work_bytes_mhd. */
 int psfft_mhd_rhs(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u,
                   void *d_rhs_b, double nu, double eta, void *d_work, void *stream);
+
+/* One Boussinesq right-hand side, the paper's reference equations (Eqs. 1-3):
+ *     d_t u     = -grad p - u.grad u - N_bv theta z^ + nu Lap u,   div u = 0
+ *     d_t theta = -u.grad theta + N_bv w + kappa Lap theta          (w = u_z)
+ * evaluated as (rotational form for the momentum term, as in psfft_hd_rhs)
+ *     rhs_u  = M P ( F[u x w] - N_bv M theta^ z^ ) - nu |k|^2 M u^          (w = curl u)
+ *     rhs_th = -M F[u . grad theta] + N_bv M u^_z - kappa |k|^2 M theta^
+ * with u, w, grad theta = F^-1 of (M u^, i k x M u^, i k M theta^): 9 inverse + 4 forward transforms in
+ * the definition; the fused passes need the equivalent of 8 inverse axis-pass sets (theta itself is
+ * never needed in physical space).
+ *   d_uhat    in   3 spectral fields     d_thhat   in   1 spectral field
+ *   d_rhs_u   out  3 spectral fields     d_rhs_th  out  1 spectral field
+ *   d_work         >= work_bytes_boussinesq
+ * Independent of the plan's batch. */
+int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thhat, void *d_rhs_u,
+                         void *d_rhs_th, double nu, double kappa, double nbv, void *d_work,
+                         void *stream);
 
 /* The same two right-hand sides computed as the plain composition of the public passes: mask +
  * curl kernel, 6 (12) three-pass inverse transforms, pointwise product kernel, 3 (6) three-pass

@@ -113,6 +113,7 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     const size_t wfield = (size_t)N * N * kx_pitch(N, cpass_cols(N, (int)(2 * s))) * 2 * s;
     o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
     o->work_bytes_mhd = 2 * o->work_bytes_hd;
+    o->work_bytes_boussinesq = 16 * wfield;   // 5 + 2 z-fields, 6 + 3 y-fields
     return PSFFT_OK;
 }
 
@@ -176,27 +177,40 @@ template <typename T> int c2r_fields_inplace(Plan *pl, const PassArgs &a, const 
 // Algorithmic bytes per launch = what the pass must read and write given the known-zero structure
 // of the dealiased spectra: n_disc retained (ky,kx) columns,
 // n_sphere retained modes, KX = kx_count(N) retained kx.
-template <typename T>
-int rhs_fused_t(Plan *pl, const PassArgs &a, int nv, const void *uhat, const void *bhat, void *ru, void *rb, double nu,
-                double eta, void *work)
+// System: nv vector fields (1 = HD, 2 = MHD) and ns scalars (Boussinesq: nv = 1, ns = 1).
+struct RhsSys {
+    int nv, ns;
+    const void *uhat, *bhat, *thhat;
+    void *ru, *rb, *rt;
+    double nu, eta, kappa, nbv;
+};
+
+template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys &y, void *work)
 {
     const size_t C = pl->lay.spec_bytes;
     const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
+    const int nv = y.nv, ns = y.ns;
     RhsArgs r;
-    r.nv = nv;
-    r.src[0] = uhat; r.src[1] = bhat;
-    r.dst[0] = ru; r.dst[1] = rb;
-    r.diff[0] = nu; r.diff[1] = eta;
+    r.nv = nv; r.ns = ns;
+    r.src[0] = y.uhat; r.src[1] = y.bhat;
+    r.dst[0] = y.ru; r.dst[1] = y.rb;
+    r.diff[0] = y.nu; r.diff[1] = y.eta;
+    r.ssrc = y.thhat; r.sdst = y.rt;
+    r.sdiff = y.kappa; r.nbv = y.nbv;
     const size_t W = (size_t)a.N * a.N * kx_pitch(a.N, cpass_cols(a.N, (int)(2 * sizeof(T)))) * 2 * sizeof(T);
-    r.zbuf = work;                              // 5 nv compact fields (later 3 nv: mid_x out, fwd_y in place)
-    r.ybuf = off(work, (size_t)5 * nv * W);     // 6 nv compact fields
+    r.zbuf = work;                                         // 5 nv + 2 ns compact fields (later 3 nv + ns: mid_x out, fwd_y in place)
+    r.ybuf = off(work, (size_t)(5 * nv + 2 * ns) * W);     // 6 nv + 3 ns compact fields
     const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
-    const double ndiff = (nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && eta != 0.0 ? 3.0 : 0.0);
-    { ProfScope ps(pl, a.stream, K_INVZ, nv * (3 * sph + 5 * disc)); CU(launch_rhs_inv_z<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_INVY, nv * (5 * disc + 6 * rows)); CU(launch_rhs_inv_y<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_MIDX, nv * (6 * rows + 3 * rows)); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_FWDY, nv * (3 * rows + 3 * disc)); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_FWDZ, nv * (3 * disc + 3.0 * (double)C) + ndiff * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
+    // sparse re-reads of the inputs in the fwd_z epilogue: diffusion (3 per vector, 1 per scalar), buoyancy
+    // (theta^ for R_u, u^_z for R_theta)
+    const double nepi = (y.nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && y.eta != 0.0 ? 3.0 : 0.0) +
+                        (ns ? (y.kappa != 0.0 || y.nbv != 0.0 ? 1.0 : 0.0) + (y.nbv != 0.0 && y.nu == 0.0 ? 1.0 : 0.0) : 0.0);
+    const int zin = 3 * nv + ns, zf = 5 * nv + 2 * ns, yf = 6 * nv + 3 * ns, ff = 3 * nv + ns;
+    { ProfScope ps(pl, a.stream, K_INVZ, zin * sph + zf * disc); CU(launch_rhs_inv_z<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_INVY, zf * disc + yf * rows); CU(launch_rhs_inv_y<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_MIDX, yf * rows + ff * rows); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDY, ff * rows + ff * disc); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (double)C + nepi * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -375,9 +389,10 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
-    if (fused)
-        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, 1, d_uhat, nullptr, d_rhs, nullptr, nu, 0.0, d_work)
-                                          : rhs_fused_t<float>(pl, a, 1, d_uhat, nullptr, d_rhs, nullptr, nu, 0.0, d_work);
+    if (fused) {
+        const RhsSys y = {1, 0, d_uhat, nullptr, nullptr, d_rhs, nullptr, nullptr, nu, 0.0, 0.0, 0.0};
+        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
+    }
     return pl->lay.dtype == PSFFT_F64 ? hd_rhs_t<double>(pl, a, d_uhat, d_rhs, nu, d_work)
                                       : hd_rhs_t<float>(pl, a, d_uhat, d_rhs, nu, d_work);
 }
@@ -392,9 +407,10 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
         return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
-    if (fused)
-        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, 2, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
-                                          : rhs_fused_t<float>(pl, a, 2, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work);
+    if (fused) {
+        const RhsSys y = {2, 0, d_uhat, d_bhat, nullptr, d_rhs_u, d_rhs_b, nullptr, nu, eta, 0.0, 0.0};
+        return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
+    }
     return pl->lay.dtype == PSFFT_F64 ? mhd_rhs_t<double>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
                                       : mhd_rhs_t<float>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work);
 }
@@ -419,6 +435,20 @@ int psfft_mhd_rhs_unfused(psfft_plan plan, const void *d_uhat, const void *d_bha
                           double nu, double eta, void *d_work, void *stream)
 {
     return mhd_entry(plan, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work, stream, false);
+}
+
+int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thhat, void *d_rhs_u, void *d_rhs_th,
+                         double nu, double kappa, double nbv, void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_uhat || !d_thhat || !d_rhs_u || !d_rhs_th || !d_work) return PSFFT_E_NULL;
+    if (misaligned(d_uhat) || misaligned(d_thhat) || misaligned(d_rhs_u) || misaligned(d_rhs_th) || misaligned(d_work))
+        return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    const RhsSys y = {1, 1, d_uhat, nullptr, d_thhat, d_rhs_u, nullptr, d_rhs_th, nu, 0.0, kappa, nbv};
+    return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
 }
 
 int psfft_fft3d_r2c_host(psfft_plan plan, const void *h_real, void *h_spec, void *d_in, void *d_out, void *d_work,

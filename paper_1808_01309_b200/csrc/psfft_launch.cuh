@@ -30,14 +30,17 @@ template <typename T> cudaError_t launch_cross(const PassArgs &a, const void *pa
 template <typename T> cudaError_t launch_cross_mhd(const PassArgs &a, const void *u, const void *b, const void *w, const void *j, void *om, void *oe, int *launches);
 template <typename T> cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void *u, void *out, double nu, int *launches);
 
-// fused right-hand side (psfft_rhs.cuh); nv = 1 (HD) or 2 (MHD)
+// fused right-hand side (psfft_rhs.cuh); nv = 1 (HD) or 2 (MHD); ns = 1 with nv = 1: Boussinesq
 struct RhsArgs {
-    int nv;
+    int nv, ns;
     const void *src[2];   // u^, b^
     void *dst[2];         // rhs_u, rhs_b
     double diff[2];       // nu, eta
-    void *zbuf;           // nv x 5 spectral fields (inv_z out; later mid_x out / fwd_y in place, 3 nv fields)
-    void *ybuf;           // nv x 6 spectral fields (inv_y out)
+    const void *ssrc;     // ns = 1: theta^
+    void *sdst;           // ns = 1: rhs_theta
+    double sdiff, nbv;    // kappa, Brunt-Vaisala frequency N_bv
+    void *zbuf;           // 5 nv + 2 ns compact fields (inv_z out; later mid_x out / fwd_y in place, 3 nv + ns fields)
+    void *ybuf;           // 6 nv + 3 ns compact fields (inv_y out)
 };
 template <typename T> cudaError_t launch_rhs_inv_z(const PassArgs &a, const RhsArgs &r, int *launches);
 template <typename T> cudaError_t launch_rhs_inv_y(const PassArgs &a, const RhsArgs &r, int *launches);

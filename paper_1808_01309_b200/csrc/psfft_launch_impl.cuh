@@ -132,13 +132,14 @@ static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid, int id 
     return run_job_v<T, N, DIR, job_tpf(N, TC), 2>(a, job, grid);
 }
 
-template <typename T, int N, int NV> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
+template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
     constexpr int KXP = kx_pitch(N, TC);
-    JobInvZ<T, N, TC, NV> job;
+    JobInvZ<T, N, TC, NV, NS> job;
     for (int v = 0; v < NV; ++v) job.src[v] = (const C *)r.src[v];
+    job.ssrc = (const C *)r.ssrc;
     job.dst = (C *)r.zbuf;
     job.plane = (long)a.ldk * N;
     job.nf = job.plane * N;
@@ -147,12 +148,12 @@ template <typename T, int N, int NV> static cudaError_t rhs_inv_z_n(const PassAr
     return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 0);
 }
 
-template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
+template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
     constexpr int KXP = kx_pitch(N, TC);
-    JobInvY<T, N, TC, NV> job;
+    JobInvY<T, N, TC, NV, NS> job;
     job.src = (const C *)r.zbuf;
     job.dst = (C *)r.ybuf;
     job.wplane = (long)KXP * N;
@@ -161,13 +162,13 @@ template <typename T, int N, int NV> static cudaError_t rhs_inv_y_n(const PassAr
     return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 1);
 }
 
-template <typename T, int N, int NV, int MINB>
+template <typename T, int N, int NV, int NS, int MINB>
 static cudaError_t mid_x8_launch(const PassArgs &a, const RhsArgs &r, long wnf, int kxp)
 {
     using C = Cx<T>;
     using L = Mid8<N, (int)sizeof(C)>;
-    constexpr size_t smem = (size_t)3 * NV * L::BUF * sizeof(C);
-    auto kern = k_mid_x8<T, N, NV, MINB>;
+    constexpr size_t smem = (size_t)(3 * NV + 2 * NS) * L::BUF * sizeof(C);
+    auto kern = k_mid_x8<T, N, NV, NS, MINB>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -177,36 +178,37 @@ static cudaError_t mid_x8_launch(const PassArgs &a, const RhsArgs &r, long wnf, 
     return cudaGetLastError();
 }
 
-template <typename T, int N, int NV> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
+template <typename T, int N, int NV, int NS> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int KXP = kx_pitch(N, cpass_cols(N, (int)sizeof(C)));
     const long wnf = (long)KXP * N * N;
     if constexpr (N == 64 || N == 512) {
         // radix-8 two-for-one kernel (psfft_midx8.cuh): one butterfly per thread and stage
-        constexpr int MINB = (sizeof(T) == 8 ? 4 : 8) / NV;
+        constexpr int MINB = (sizeof(T) == 8 ? 4 : 8) / (NV + NS);
 #ifdef PSFFT_EXPERIMENT
-        if constexpr (N == 512 && sizeof(T) == 8 && NV == 1) {
+        if constexpr (N == 512 && sizeof(T) == 8 && NV == 1 && NS == 0) {
             static const int v = getenv("PSFFT_MIDX_VARIANT") ? atoi(getenv("PSFFT_MIDX_VARIANT")) : 0;
-            if (v == 4) return mid_x8_launch<T, N, NV, 4>(a, r, wnf, KXP);
-            if (v == 5) return mid_x8_launch<T, N, NV, 5>(a, r, wnf, KXP);
+            if (v == 4) return mid_x8_launch<T, N, NV, NS, 4>(a, r, wnf, KXP);
+            if (v == 5) return mid_x8_launch<T, N, NV, NS, 5>(a, r, wnf, KXP);
         }
 #endif
-        return mid_x8_launch<T, N, NV, MINB>(a, r, wnf, KXP);
+        return mid_x8_launch<T, N, NV, NS, MINB>(a, r, wnf, KXP);
     } else {
         constexpr int TPF = threads_per_fft(N / 2);
-        constexpr size_t smem = (size_t)6 * NV * RowMap<N / 2>::ld * sizeof(C);
-        auto kern = k_mid_x<T, N, NV>;
+        constexpr int NG = 6 * NV + 3 * NS;
+        constexpr size_t smem = (size_t)NG * RowMap<N / 2>::ld * sizeof(C);
+        auto kern = k_mid_x<T, N, NV, NS>;
         cudaError_t e = set_smem(kern, smem);
         if (e != cudaSuccess) return e;
         const T scale = (T)(1.0 / ((double)N * N * N));
-        kern<<<(unsigned)(N * N), 6 * NV * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
+        kern<<<(unsigned)(N * N), NG * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
                                                                    (const C *)a.twM, wnf, KXP, scale);
         return cudaGetLastError();
     }
 }
 
-template <typename T, int N, int NV> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)
+template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
@@ -216,16 +218,20 @@ template <typename T, int N, int NV> static cudaError_t rhs_fwd_y_n(const PassAr
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.kxp = KXP;
-    job.nfields = 3 * NV;
+    job.nfields = 3 * NV + NS;
     return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 2);
 }
 
-template <typename T, int N, int NV> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
+template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
     constexpr int KXP = kx_pitch(N, TC);
-    JobFwdZ<T, N, TC, NV> job;
+    JobFwdZ<T, N, TC, NV, NS> job;
+    job.sdst = (C *)r.sdst;
+    job.saux = (const C *)r.ssrc;
+    job.sdiff = (T)r.sdiff;
+    job.nbv = (T)r.nbv;
     job.src = (const C *)r.zbuf;
     for (int v = 0; v < NV; ++v) {
         job.dst[v] = (C *)r.dst[v];
@@ -249,11 +255,11 @@ template <typename T, int N, int NV> static cudaError_t rhs_fwd_z_n(const PassAr
         }                                                                                              \
         return cudaErrorInvalidValue;                                                                  \
     }
-#define PSFFT_RHS_CASE_inv_z(n) case n: return r.nv == 1 ? rhs_inv_z_n<T, n, 1>(a, r) : rhs_inv_z_n<T, n, 2>(a, r);
-#define PSFFT_RHS_CASE_inv_y(n) case n: return r.nv == 1 ? rhs_inv_y_n<T, n, 1>(a, r) : rhs_inv_y_n<T, n, 2>(a, r);
-#define PSFFT_RHS_CASE_mid_x(n) case n: return r.nv == 1 ? rhs_mid_x_n<T, n, 1>(a, r) : rhs_mid_x_n<T, n, 2>(a, r);
-#define PSFFT_RHS_CASE_fwd_y(n) case n: return r.nv == 1 ? rhs_fwd_y_n<T, n, 1>(a, r) : rhs_fwd_y_n<T, n, 2>(a, r);
-#define PSFFT_RHS_CASE_fwd_z(n) case n: return r.nv == 1 ? rhs_fwd_z_n<T, n, 1>(a, r) : rhs_fwd_z_n<T, n, 2>(a, r);
+#define PSFFT_RHS_CASE_inv_z(n) case n: return r.ns == 1 ? rhs_inv_z_n<T, n, 1, 1>(a, r) : r.nv == 1 ? rhs_inv_z_n<T, n, 1, 0>(a, r) : rhs_inv_z_n<T, n, 2, 0>(a, r);
+#define PSFFT_RHS_CASE_inv_y(n) case n: return r.ns == 1 ? rhs_inv_y_n<T, n, 1, 1>(a, r) : r.nv == 1 ? rhs_inv_y_n<T, n, 1, 0>(a, r) : rhs_inv_y_n<T, n, 2, 0>(a, r);
+#define PSFFT_RHS_CASE_mid_x(n) case n: return r.ns == 1 ? rhs_mid_x_n<T, n, 1, 1>(a, r) : r.nv == 1 ? rhs_mid_x_n<T, n, 1, 0>(a, r) : rhs_mid_x_n<T, n, 2, 0>(a, r);
+#define PSFFT_RHS_CASE_fwd_y(n) case n: return r.ns == 1 ? rhs_fwd_y_n<T, n, 1, 1>(a, r) : r.nv == 1 ? rhs_fwd_y_n<T, n, 1, 0>(a, r) : rhs_fwd_y_n<T, n, 2, 0>(a, r);
+#define PSFFT_RHS_CASE_fwd_z(n) case n: return r.ns == 1 ? rhs_fwd_z_n<T, n, 1, 1>(a, r) : r.nv == 1 ? rhs_fwd_z_n<T, n, 1, 0>(a, r) : rhs_fwd_z_n<T, n, 2, 0>(a, r);
 PSFFT_RHS_LAUNCHER(inv_z)
 PSFFT_RHS_LAUNCHER(inv_y)
 PSFFT_RHS_LAUNCHER(mid_x)

@@ -14,6 +14,8 @@
 // products are formed in registers and go straight into the first stage of the forward
 // transforms F1 = n_x + i n_y, F2 = n_z (MHD: m_x + i m_y, m_z + i e_x, e_y + i e_z), whose output
 // is split as n^_x[k] = (F1[k] + conj F1[N-k])/2, n^_y[k] = -i (F1[k] - conj F1[N-k])/2.
+// Boussinesq (NS = 1): two more inverse transforms (g_x + i g_y, g_z) for grad theta and F2 = n_z + i s,
+// s = u . grad theta (Eq. 2).
 //
 // Shared memory: one buffer of N complex per inverse transform; every exchange is conflict-free
 // (Mid8::pad).  The first forward stage writes into the slots its thread has just read, so the
@@ -53,7 +55,7 @@ __device__ __forceinline__ void twiddle8(C *v, const C *__restrict__ ts, int Ns)
     v[5] = cmul(v[5], w5); v[6] = cmul(v[6], w6); v[7] = cmul(v[7], w7);
 }
 
-template <typename T, int N, int NV, int MINB>
+template <typename T, int N, int NV, int NS, int MINB>
 __global__ void __launch_bounds__(N / 8, MINB)
     k_mid_x8(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tw, long nfw, int kxp,
              T scale2)
@@ -61,9 +63,9 @@ __global__ void __launch_bounds__(N / 8, MINB)
     using C = Cx<T>;
     using L = Mid8<N, (int)sizeof(C)>;
     constexpr int NB = L::NB, BUF = L::BUF, KX = kx_count(N);
-    constexpr int NI = 3 * NV;            // inverse complex transforms
-    constexpr int NF = (3 * NV + 1) / 2;  // forward complex transforms
-    constexpr int NSPLIT = (3 * NV) / 2;  // forward transforms that carry two real fields
+    constexpr int NI = 3 * NV + 2 * NS;        // inverse complex transforms: (u_c, w_c) pairs, (g_x, g_y), (g_z, -)
+    constexpr int NF = (3 * NV + NS + 1) / 2;  // forward complex transforms
+    constexpr int NSPLIT = (3 * NV + NS) / 2;  // forward transforms that carry two real fields
     extern __shared__ __align__(16) unsigned char smraw[];
     C *sm = reinterpret_cast<C *>(smraw);
 
@@ -125,6 +127,40 @@ __global__ void __launch_bounds__(N / 8, MINB)
             for (int r = 0; r < 8; ++r) buf[L::pad(8 * b + r)] = v[r];
         }
     }
+    if constexpr (NS > 0) {   // gradient of the scalar: g_x = c2r (i kx Th), g_y = c2r Dt, g_z = c2r Gz
+        const C *f = in + (long)(6 * NV) * nfw + rowoff;
+        C th[6], dt[6], gz[6];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            th[q] = dt[q] = gz[q] = zero;
+            if (pq[q]) {
+                th[q] = ld_stream(f + kq[q]);
+                dt[q] = ld_stream(f + nfw + kq[q]);
+                gz[q] = ld_stream(f + 2 * nfw + kq[q]);
+            }
+        }
+#pragma unroll
+        for (int tt = 0; tt < 2; ++tt) {
+            C v[8];
+            v[3] = zero; v[4] = zero;
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                C a, bb;
+                if (tt == 0) { a = mul_ik(th[q], (T)kq[q]); bb = dt[q]; }
+                else { a = gz[q]; bb = zero; }
+                if (q < 3) {
+                    if (q == 0 && b == 0) { a.y = (T)0; bb.y = (T)0; }
+                    v[q] = mk<T>(a.x - bb.y, a.y + bb.x);
+                } else {
+                    v[q + 2] = mk<T>(a.x + bb.y, bb.x - a.y);
+                }
+            }
+            bfly8<+1, T>(v);
+            C *buf = sm + (3 * NV + tt) * BUF;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) buf[L::pad(8 * b + r)] = v[r];
+        }
+    }
     __syncthreads();
 
     // ---- inverse, middle stage (N = 512): Ns = 8, in place, software-pipelined over the transforms ----
@@ -175,6 +211,9 @@ __global__ void __launch_bounds__(N / 8, MINB)
             const T e0 = uy * bz - uz * by, e1 = uz * bx - ux * bz, e2 = ux * by - uy * bx;
             F[1][r] = mk<T>(m2 * scale2, e0 * scale2);
             F[2][r] = mk<T>(e1 * scale2, e2 * scale2);
+        } else if constexpr (NS > 0) {   // z[3] = g_x + i g_y, z[4] = g_z:  s = u . grad theta
+            const T s = ux * z[3][r].x + uy * z[3][r].y + uz * z[4][r].x;
+            F[1][r] = mk<T>(m2 * scale2, s * scale2);
         } else {
             F[1][r] = mk<T>(m2 * scale2, (T)0);
         }

@@ -1,4 +1,5 @@
-// psfft_rhs.cuh -- the fused right-hand-side passes (HD: NV = 1, MHD: NV = 2).
+// psfft_rhs.cuh -- the fused right-hand-side passes (HD: NV = 1; MHD: NV = 2; Boussinesq: NV = 1 plus
+// NS = 1 scalar field theta, Eqs. 1-3).
 //
 // One evaluation is five kernels; physical-space data never reaches HBM and the spectral
 // pointwise work rides on the loads / stores of the transform passes:
@@ -16,6 +17,15 @@
 // applied in the pass whose FFT runs along that axis (the multiplier is then per-element of the
 // loaded column), everything else commutes with the remaining transforms by linearity.  This
 // needs 5 z-transforms and 6 y-transforms per vector field instead of 6 + 6.
+//
+// Boussinesq (NS = 1): the gradient g = i k theta^ is split over the passes in the same way,
+//   inv_z   T_A = F_z^-1 theta^,  T_B = F_z^-1 (i kz theta^)
+//   inv_y   Th = F_y^-1 T_A,  Dt = F_y^-1 (i ky T_A),  Gz = F_y^-1 T_B
+//   mid_x   g_x = c2r (i kx Th), g_y = c2r Dt, g_z = c2r Gz;  s = u . g;  r2c of s
+//   fwd_z   epilogue: n^_z -= N_bv M theta^ before the projection (Eq. 1: buoyancy is inside the
+//           pressure projection);  R_theta = -s^ + N_bv M u^_z - kappa |k|^2 M theta^ (Eq. 2)
+// i.e. 2 + 3 + 3 inverse and 1 forward axis transforms on top of HD (theta itself is never needed in
+// physical space).
 //
 // Pruning: after the mask of step 1 (and before the mask of step 6) every mode with
 // 9 |k|^2 >= N^2 is zero (does not matter), so columns / rows that are entirely outside the
@@ -62,15 +72,16 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
 // ---- inv_z -------------------------------------------------------------------------------------
 // grid (kxp / TC, N): tile = TC consecutive kx at one ky.  Reads the caller's layout (pitch ldk),
 // writes the compact workspace layout (pitch kxp).
-template <typename T, int N, int TC, int NV> struct JobInvZ {
+template <typename T, int N, int TC, int NV, int NS> struct JobInvZ {
     using C = Cx<T>;
     const C *src[NV];   // NV x 3 spectral fields (u^, b^), caller layout
-    C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x = F_z^-1(i kz u_x), G_x = F_z^-1(w^_x)
+    const C *ssrc;      // NS = 1: theta^, caller layout
+    C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x = F_z^-1(i kz u_x), G_x = F_z^-1(w^_x); then NS x 2: T_A, T_B
     long plane, nf;     // caller layout: ldk N, ldk N N
     long wplane, wnf;   // workspace layout: kxp N, kxp N N
     struct State { long col, wcol; int kxy2, ky; bool active; };
 
-    __device__ __forceinline__ int rounds() const { return 5 * NV; }
+    __device__ __forceinline__ int rounds() const { return 5 * NV + 2 * NS; }
     __device__ __forceinline__ bool begin(State &s, int c, int) const
     {
         const int kx = blockIdx.x * TC + c, ky = wavenumber((int)blockIdx.y, N);
@@ -87,17 +98,22 @@ template <typename T, int N, int TC, int NV> struct JobInvZ {
         return s.active && 9 * (s.kxy2 + kz * kz) < N * N;
     }
     __device__ __forceinline__ const C *field(int r) const { return (NV == 2 && r >= 5) ? src[NV - 1] : src[0]; }
-    // rr: 0..2 A_c <- u_c | 3 B_x <- i kz u_x | 4 G_x <- i (ky u_z - kz u_y)
+    // rr: 0..2 A_c <- u_c | 3 B_x <- i kz u_x | 4 G_x <- i (ky u_z - kz u_y);  scalar: T_A <- th | T_B <- i kz th
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
+        C x = mk<T>(0, 0);
+        if (NS > 0 && r >= 5 * NV) {
+            if (keep(s, i)) x = ldg_c(ssrc + i * plane + s.col);
+            return x;
+        }
         const int rr = r % 5;
         const int comp = rr < 3 ? rr : rr == 3 ? 0 : 2;
-        C x = mk<T>(0, 0);
         if (keep(s, i)) x = ldg_c(field(r) + comp * nf + i * plane + s.col);
         return x;
     }
     __device__ __forceinline__ C post(const State &s, int r, int i, C x) const
     {
+        if (NS > 0 && r >= 5 * NV) return r == 5 * NV ? x : mul_ik(x, (T)wavenumber(i, N));
         const int rr = r % 5;
         if (rr < 3) return x;
         const T kz = (T)wavenumber(i, N);
@@ -115,15 +131,15 @@ template <typename T, int N, int TC, int NV> struct JobInvZ {
 
 // ---- inv_y -------------------------------------------------------------------------------------
 // grid (kxp / TC, N): tile = TC consecutive kx of one z plane, all in the compact layout.
-template <typename T, int N, int TC, int NV> struct JobInvY {
+template <typename T, int N, int TC, int NV, int NS> struct JobInvY {
     using C = Cx<T>;
-    const C *src;  // NV x 5 fields from inv_z
-    C *dst;        // NV x 6 fields: U_x, U_y, U_z, W_x, P, D
+    const C *src;  // NV x 5 (+ NS x 2) fields from inv_z
+    C *dst;        // NV x 6 fields: U_x, U_y, U_z, W_x, P, D;  then NS x 3: Th, Dt, Gz
     long wplane, wnf;
     int kxp;
     struct State { long base; int kx; bool active; };
 
-    __device__ __forceinline__ int rounds() const { return 6 * NV; }
+    __device__ __forceinline__ int rounds() const { return 6 * NV + 3 * NS; }
     __device__ __forceinline__ bool begin(State &s, int c, int) const
     {
         s.kx = blockIdx.x * TC + c;
@@ -131,6 +147,7 @@ template <typename T, int N, int TC, int NV> struct JobInvY {
         s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
+    // scalar rounds (r >= 6 NV): Th <- T_A | Dt <- i ky T_A | Gz <- T_B
     // round order: U_x <- A_x | D <- i ky A_x | U_y | U_z | W_x <- G_x | P <- B_x.  A_x is read in two
     // consecutive rounds: the first read leaves it in L2 (default policy), the second streams.
     __device__ __forceinline__ static int src_field(int rr) { return rr == 0 ? 0 : rr == 1 ? 0 : rr == 2 ? 1 : rr == 3 ? 2 : rr == 4 ? 4 : 3; }
@@ -138,21 +155,25 @@ template <typename T, int N, int TC, int NV> struct JobInvY {
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
         const int ky = wavenumber(i, N);
-        const int v = r / 6, rr = r % 6;
+        const bool sc = NS > 0 && r >= 6 * NV;
+        const int v = r / 6, rr = sc ? r - 6 * NV : r % 6;
         C x = mk<T>(0, 0);
         if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) {
-            const C *p = src + (long)(v * 5 + src_field(rr)) * wnf + s.base + (long)i * kxp;
+            const int f = sc ? 5 * NV + (rr >> 1) : v * 5 + src_field(rr);
+            const C *p = src + (long)f * wnf + s.base + (long)i * kxp;
             x = rr == 0 ? *p : ld_stream(p);
         }
         return x;
     }
     __device__ __forceinline__ C post(const State &, int r, int i, C x) const
     {
-        return (r % 6 == 1) ? mul_ik(x, (T)wavenumber(i, N)) : x;
+        const int rr = (NS > 0 && r >= 6 * NV) ? r - 6 * NV : r % 6;
+        return rr == 1 ? mul_ik(x, (T)wavenumber(i, N)) : x;
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
-        if (s.active) st_stream(dst + (long)((r / 6) * 6 + dst_field(r % 6)) * wnf + s.base + (long)i * kxp, v);
+        const int f = (NS > 0 && r >= 6 * NV) ? r : (r / 6) * 6 + dst_field(r % 6);
+        if (s.active) st_stream(dst + (long)f * wnf + s.base + (long)i * kxp, v);
     }
 };
 
@@ -189,18 +210,24 @@ template <typename T, int N, int TC> struct JobFwdY {
 // ---- fwd_z + epilogue ----------------------------------------------------------------------------
 // groups of 3 rounds (components x, y, z of one vector field).  Group g: mode[g] = 0 -> P f - d |k|^2 a
 // (momentum), 1 -> i k x f - d |k|^2 a (induction); a = aux[g] (u^ or b^), d = diff[g].
-template <typename T, int N, int TC, int NV> struct JobFwdZ {
+// Boussinesq (NS = 1): one more round for s^ = F[u . grad theta]; its store forms
+// R_theta = -s^ + N_bv u^_z - kappa |k|^2 theta^, and the z component of group 0 gets -N_bv theta^
+// before the projection (Eqs. 1-2).
+template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
     using C = Cx<T>;
-    const C *src;        // NV x 3 fields (after fwd_y), compact layout
+    const C *src;        // NV x 3 (+ NS) fields (after fwd_y), compact layout
     C *dst[NV];          // NV outputs of 3 fields, caller layout
     const C *aux[NV];    // u^, b^ for the diffusion term
     T diff[NV];
+    C *sdst;             // NS = 1: R_theta, caller layout
+    const C *saux;       // NS = 1: theta^
+    T sdiff, nbv;        // kappa, N_bv
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
     int ldk;
     struct State { long col, wcol; int kx, ky, kxy2; bool active, valid; };
 
-    __device__ __forceinline__ int rounds() const { return 3 * NV; }
+    __device__ __forceinline__ int rounds() const { return 3 * NV + NS; }
     // grid (ceil(ldk N / TC)): tile = TC consecutive columns of the caller's (ky, kx) plane, whose
     // 128-byte rows are line-aligned (the plane size ldk N is a multiple of TC); the workspace side
     // is read at the compact address of the same (ky, kx)
@@ -227,6 +254,8 @@ template <typename T, int N, int TC, int NV> struct JobFwdZ {
                 for (int comp = 0; comp < 3; ++comp)
                     for (int i = t; i < N; i += blockDim.x / TC)
                         st_stream((g == 0 ? dst[0] : dst[NV - 1]) + comp * nf + i * plane + s.col, z);
+            if (NS > 0)
+                for (int i = t; i < N; i += blockDim.x / TC) st_stream(sdst + i * plane + s.col, z);
         }
         return false;
     }
@@ -243,14 +272,34 @@ template <typename T, int N, int TC, int NV> struct JobFwdZ {
         const int g = r / 3, comp = r % 3;
         const int kz = wavenumber(i, N);
         const int kx = s.kx, ky = s.ky, kxy2 = s.kxy2;
-        C *o = (g == 0 ? dst[0] : dst[NV - 1]) + i * plane + s.col;
         const bool keep = s.active && 9 * (kxy2 + kz * kz) < N * N;
+        if (NS > 0 && r == 3 * NV) {   // Eq. 2: R_theta = -s^ + N_bv u^_z - kappa |k|^2 theta^
+            C *os = sdst + i * plane + s.col;
+            if (!keep) { *os = mk<T>(0, 0); return; }
+            C rt = mk<T>(-v.x, -v.y);
+            if (nbv != (T)0) {
+                const C uz = ldg_c(aux[0] + 2 * nf + i * plane + s.col);
+                rt.x += nbv * uz.x; rt.y += nbv * uz.y;
+            }
+            if (sdiff != (T)0) {
+                const T sc = sdiff * (T)(kxy2 + kz * kz);
+                const C th = ldg_c(saux + i * plane + s.col);
+                rt.x -= sc * th.x; rt.y -= sc * th.y;
+            }
+            *os = rt;
+            return;
+        }
+        C *o = (g == 0 ? dst[0] : dst[NV - 1]) + i * plane + s.col;
         if (!keep) { o[comp * nf] = mk<T>(0, 0); return; }
         if (comp < 2) { o[comp * nf] = v; return; }   // raw; read back below by this same thread
         C fx = o[0], fy = o[nf], fz = v;
         const T qx = (T)kx, qy = (T)ky, qz = (T)kz;
         const T k2 = (T)(kxy2 + kz * kz);
         if (g == 0) {            // a10: projection, identity at k = 0
+            if (NS > 0 && nbv != (T)0) {   // Eq. 1: buoyancy -N_bv theta z^, inside the projection
+                const C th = ldg_c(saux + i * plane + s.col);
+                fz.x -= nbv * th.x; fz.y -= nbv * th.y;
+            }
             if (k2 != (T)0) {
                 const T inv = (T)1 / k2;
                 const T dr = (qx * fx.x + qy * fy.x + qz * fz.x) * inv;
@@ -279,12 +328,13 @@ template <typename T, int N, int TC, int NV> struct JobFwdZ {
 };
 
 // ------------------------------------------------------------------------------------------
-// mid_x: one CTA per (z, y) row; 6 NV groups of TPF threads, one half-length transform each.
-//   in   NV x 6 fields (U_x, U_y, U_z, W_x, P, D), rows of ldk complex, entries kx >= N/3 unused
-//   out  3 NV fields, entries kx < N/3 written
+// mid_x: one CTA per (z, y) row; 6 NV + 3 NS groups of TPF threads, one half-length transform each.
+//   in   NV x 6 fields (U_x, U_y, U_z, W_x, P, D) (+ NS x 3: Th, Dt, Gz), rows of ldk complex,
+//        entries kx >= N/3 unused
+//   out  3 NV + NS fields, entries kx < N/3 written
 // ------------------------------------------------------------------------------------------
-template <typename T, int N, int NV>
-__global__ void __launch_bounds__(6 * NV *threads_per_fft(N / 2))
+template <typename T, int N, int NV, int NS>
+__global__ void __launch_bounds__((6 * NV + 3 * NS) * threads_per_fft(N / 2))
     k_mid_x(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
             const Cx<T> *__restrict__ tw, long nf, int ldk, T scale)
 {
@@ -293,19 +343,21 @@ __global__ void __launch_bounds__(6 * NV *threads_per_fft(N / 2))
     constexpr int TPF = threads_per_fft(M);
     constexpr bool WARP = (TPF <= 32) && (32 % TPF == 0);
     constexpr int KX = kx_count(N);
-    constexpr int NG = 6 * NV;
+    constexpr int NG = 6 * NV + 3 * NS;
     using Map = RowMap<M>;
     extern __shared__ __align__(16) unsigned char smraw[];
     C *sm = reinterpret_cast<C *>(smraw);
 
     const int g = threadIdx.x / TPF, t = threadIdx.x % TPF;
-    const int v = g / 6, gg = g % 6;
+    const bool sc = NS > 0 && g >= 6 * NV;           // gradient groups: g_x, g_y, g_z
+    const int v = sc ? NV : g / 6, gg = sc ? g - 6 * NV : g % 6;
     const long rowoff = (long)blockIdx.x * ldk;
-    const C *f = in + (long)(v * 6) * nf + rowoff;   // the six fields of this vector
+    const C *f = in + (long)(v * 6) * nf + rowoff;   // the six fields of this vector (three of the scalar)
 
     // spectral row of group gg at index k (0 for k >= KX)
     auto spec = [&](int k) -> C {
         if (k >= KX) return mk<T>(0, 0);
+        if (sc) return gg == 0 ? mul_ik(ld_stream(f + k), (T)k) : ld_stream(f + gg * nf + k);
         switch (gg) {
             case 0: return ld_stream(f + k);
             case 1: return ld_stream(f + nf + k);
@@ -346,7 +398,7 @@ __global__ void __launch_bounds__(6 * NV *threads_per_fft(N / 2))
         r0.x = q[1].x * q[5].x - q[2].x * q[4].x; r0.y = q[1].y * q[5].y - q[2].y * q[4].y;
         r1.x = q[2].x * q[3].x - q[0].x * q[5].x; r1.y = q[2].y * q[3].y - q[0].y * q[5].y;
         r2.x = q[0].x * q[4].x - q[1].x * q[3].x; r2.y = q[0].y * q[4].y - q[1].y * q[3].y;
-        if (NV == 2) {
+        if constexpr (NV == 2) {
             // m = u x w + j x b
             r0.x += q[10].x * q[8].x - q[11].x * q[7].x; r0.y += q[10].y * q[8].y - q[11].y * q[7].y;
             r1.x += q[11].x * q[6].x - q[9].x * q[8].x;  r1.y += q[11].y * q[6].y - q[9].y * q[8].y;
@@ -358,12 +410,18 @@ __global__ void __launch_bounds__(6 * NV *threads_per_fft(N / 2))
             e2.x = q[0].x * q[7].x - q[1].x * q[6].x; e2.y = q[0].y * q[7].y - q[1].y * q[6].y;
             sm[Map::at(n, 3)] = e0; sm[Map::at(n, 4)] = e1; sm[Map::at(n, 5)] = e2;
         }
+        if constexpr (NS > 0) {   // s = u . grad theta
+            C d;
+            d.x = q[0].x * q[6].x + q[1].x * q[7].x + q[2].x * q[8].x;
+            d.y = q[0].y * q[6].y + q[1].y * q[7].y + q[2].y * q[8].y;
+            sm[Map::at(n, 3)] = d;
+        }
         sm[Map::at(n, 0)] = r0; sm[Map::at(n, 1)] = r1; sm[Map::at(n, 2)] = r2;
     }
     __syncthreads();
 
     // forward transforms of the 3 NV product rows (the other groups only keep the barriers company)
-    constexpr int NF = 3 * NV;
+    constexpr int NF = 3 * NV + NS;
     if (WARP && g >= NF) return;
     {
         auto ld = [&](int) -> C { return mk<T>(0, 0); };

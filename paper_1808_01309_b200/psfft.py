@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
-    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs",
+    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
     "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
@@ -36,7 +36,8 @@ class Layout(ctypes.Structure):
                 ("real_elems", ctypes.c_size_t), ("spec_elems", ctypes.c_size_t),
                 ("real_bytes", ctypes.c_size_t), ("spec_bytes", ctypes.c_size_t),
                 ("table_bytes", ctypes.c_size_t), ("work_bytes_fft", ctypes.c_size_t),
-                ("work_bytes_hd", ctypes.c_size_t), ("work_bytes_mhd", ctypes.c_size_t)]
+                ("work_bytes_hd", ctypes.c_size_t), ("work_bytes_mhd", ctypes.c_size_t),
+                ("work_bytes_boussinesq", ctypes.c_size_t)]
 
 
 _lib = None
@@ -59,6 +60,7 @@ def lib() -> ctypes.CDLL:
         L.psfft_fft3d_c2r.argtypes = [vp, vp, vp, vp, vp]
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
+        L.psfft_boussinesq_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, cd, vp, vp]
         L.psfft_hd_rhs_unfused.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs_unfused.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -143,6 +145,12 @@ def mhd_rhs(plan: int, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu: float, eta: float, 
                                _ptr(d_work), _stream(stream)), "psfft_mhd_rhs")
 
 
+def boussinesq_rhs(plan: int, d_uhat, d_thhat, d_rhs_u, d_rhs_th, nu: float, kappa: float, nbv: float, d_work,
+                   stream=None) -> None:
+    _check(lib().psfft_boussinesq_rhs(plan, _ptr(d_uhat), _ptr(d_thhat), _ptr(d_rhs_u), _ptr(d_rhs_th), float(nu),
+                                      float(kappa), float(nbv), _ptr(d_work), _stream(stream)), "psfft_boussinesq_rhs")
+
+
 def hd_rhs_unfused(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
     _check(lib().psfft_hd_rhs_unfused(plan, _ptr(d_uhat), _ptr(d_rhs), float(nu), _ptr(d_work), _stream(stream)),
            "psfft_hd_rhs_unfused")
@@ -224,7 +232,7 @@ class Plan:
 
     def ensure_work(self, kind: str):
         need = {"fft": self.layout.work_bytes_fft, "hd": self.layout.work_bytes_hd,
-                "mhd": self.layout.work_bytes_mhd}[kind]
+                "mhd": self.layout.work_bytes_mhd, "boussinesq": self.layout.work_bytes_boussinesq}[kind]
         if self._work is None or self._work.numel() < need:
             self._work = None
             self._work = torch.empty(need, dtype=torch.uint8, device=self.device)
@@ -274,3 +282,12 @@ class Plan:
         ru, rb = torch.empty_like(uhat), torch.empty_like(bhat)
         mhd_rhs(self.handle, uhat, bhat, ru, rb, nu, eta, self.ensure_work("mhd"))
         return ru, rb
+
+    def boussinesq_rhs(self, uhat: torch.Tensor, thhat: torch.Tensor, nu: float = 0.0, kappa: float = 0.0,
+                       nbv: float = 0.0):
+        assert uhat.is_cuda and uhat.dtype == self.cdtype and uhat.is_contiguous()
+        assert thhat.is_cuda and thhat.dtype == self.cdtype and thhat.is_contiguous()
+        assert tuple(uhat.shape) == self.spec_shape(3) and thhat.numel() == self.layout.spec_elems
+        ru, rt = torch.empty_like(uhat), torch.empty_like(thhat)
+        boussinesq_rhs(self.handle, uhat, thhat, ru, rt, nu, kappa, nbv, self.ensure_work("boussinesq"))
+        return ru, rt

@@ -186,6 +186,48 @@ def test_mhd_rhs_matches_oracle(N, dtype):
     assert np.all(ru.cpu().numpy()[:, ~M] == 0) and np.all(rb.cpu().numpy()[:, ~M] == 0)
 
 
+# ---- Boussinesq (Eqs. 1-3) ------------------------------------------
+
+def boussinesq_case(N, k0, kcut, dtype, nu, kappa, nbv):
+    uh = synth.solenoidal_spectrum(N, k0, kcut, 1234).astype(CDT[dtype])
+    th = synth.scalar_spectrum(N, k0, kcut, 1234).astype(CDT[dtype])
+    p = psfft.Plan(N, dtype, 1, work="boussinesq")
+    ud, td = dev(uh), dev(th)
+    ru, rt = p.boussinesq_rhs(ud, td, nu, kappa, nbv)
+    assert np.array_equal(ud.cpu().numpy(), uh) and np.array_equal(td.cpu().numpy(), th)     # inputs untouched
+    wu, wt = oracle.boussinesq_rhs(uh.astype(np.complex128), th.astype(np.complex128), nu, kappa, nbv)
+    return ru.cpu().numpy(), rt.cpu().numpy(), wu, wt
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,k0,kcut", [(16, 2.0, 7), (24, 2.0, 11), (32, 4.0, 15), (48, 4.0, 23), (64, 4.0, 31), (96, 4.0, 32),
+                                       (128, 4.0, 32)])
+def test_boussinesq_rhs_matches_oracle(N, k0, kcut, dtype):
+    """All terms on: nu, kappa, N_bv != 0; kcut above N/3 so that the input mask has to act.  N = 64 runs the
+    radix-8 two-for-one mid_x kernel, the others the generic one."""
+    ru, rt, wu, wt = boussinesq_case(N, k0, kcut, dtype, 0.013, 0.021, 2.5)
+    assert rel(ru, wu) < TOL[dtype]
+    assert rel(rt, wt) < TOL[dtype]
+    M = oracle.dealias_mask(N)
+    assert np.all(ru[:, ~M] == 0) and np.all(rt[~M] == 0)
+
+
+@pytest.mark.parametrize("nu,kappa,nbv", [(0.0, 0.0, 0.0), (0.0, 0.0, 1.7), (0.02, 0.0, 0.0), (0.0, 0.03, 0.0)])
+def test_boussinesq_rhs_term_by_term(nu, kappa, nbv):
+    """Each optional term alone (the epilogue skips the reads of a term whose coefficient is zero)."""
+    ru, rt, wu, wt = boussinesq_case(32, 4.0, 12, torch.float64, nu, kappa, nbv)
+    assert rel(ru, wu) < 1e-12 and rel(rt, wt) < 1e-12
+
+
+def test_boussinesq_reduces_to_hd_when_theta_vanishes():
+    N = 32
+    uh = synth.solenoidal_spectrum(N, 4.0, 12, 1234)
+    p = psfft.Plan(N, torch.float64, 1, work="boussinesq")
+    ru, rt = p.boussinesq_rhs(dev(uh), dev(np.zeros((N, N, N // 2 + 1), np.complex128)), 0.01, 0.02, 0.0)
+    hd = p.hd_rhs(dev(uh), 0.01)
+    assert float((ru - hd).norm() / hd.norm()) < 1e-14 and float(rt.abs().max()) == 0.0
+
+
 # ---- host-buffer (end-to-end) entry points -----------------------------------------------------------
 
 def test_host_entry_points():
