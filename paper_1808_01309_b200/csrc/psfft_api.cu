@@ -16,14 +16,35 @@ using namespace psfft;
 
 namespace psfft {
 // entries are padded to multiples of 16 so that each table starts 256-byte aligned
-size_t table_entries(int N, size_t *off_twN, size_t *off_twM)
+// the symmetric schedule RM, (factors of N / RM^2), RM of psfft_midxg.cuh (XSched) for a runtime N
+int xsched_stages(int N, int *radix)
+{
+    const int RM = (N % 64 == 0) ? 8 : (N % 16 == 0) ? 4 : 2;
+    int n = 0, m = N / (RM * RM);
+    radix[n++] = RM;
+    while (m > 1) {
+        const int r = (m % 8 == 0 && m != 16) ? 8 : (m % 4 == 0) ? 4 : (m % 2 == 0) ? 2 : 3;
+        radix[n++] = r;
+        m /= r;
+    }
+    radix[n++] = RM;
+    return n;
+}
+
+size_t table_entries(int N, size_t *off_twN, size_t *off_twM, size_t *off_twX)
 {
     auto up = [](size_t n) { return (n + 15) / 16 * 16; };
     const size_t a = up((size_t)N);
     const size_t b = a + up((size_t)tw_size(N));
+    const size_t c = b + up((size_t)tw_size(N / 2));
     if (off_twN) *off_twN = a;
     if (off_twM) *off_twM = b;
-    return b + up((size_t)tw_size(N / 2));
+    if (off_twX) *off_twX = c;
+    int radix[8];
+    const int S = xsched_stages(N, radix);
+    size_t x = 0, Ns = radix[0];
+    for (int s = 1; s < S; ++s) { x += (size_t)(radix[s] - 1) * Ns; Ns *= radix[s]; }
+    return c + up(x);
 }
 }  // namespace psfft
 
@@ -107,7 +128,7 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     o->spec_elems = (size_t)o->ldk * N * N;
     o->real_bytes = o->real_elems * s;
     o->spec_bytes = o->spec_elems * 2 * s;
-    o->table_bytes = table_entries(N, nullptr, nullptr) * 2 * s;
+    o->table_bytes = table_entries(N, nullptr, nullptr, nullptr) * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
     // fused path: 5 + 6 compact fields [N][N][kx_pitch] per vector field; unfused path: 12 C per vector field
     const size_t wfield = (size_t)N * N * kx_pitch(N, cpass_cols(N, (int)(2 * s))) * 2 * s;
@@ -129,11 +150,12 @@ PassArgs args_of(const Plan *pl, void *stream)
 {
     PassArgs a;
     const size_t cs = pl->lay.dtype == PSFFT_F64 ? 16 : 8;
-    size_t oN, oM;
-    table_entries(pl->lay.N, &oN, &oM);
+    size_t oN, oM, oX;
+    table_entries(pl->lay.N, &oN, &oM, &oX);
     a.tab = pl->d_tab;
     a.twN = static_cast<const char *>(pl->d_tab) + oN * cs;
     a.twM = static_cast<const char *>(pl->d_tab) + oM * cs;
+    a.twX = static_cast<const char *>(pl->d_tab) + oX * cs;
     a.N = pl->lay.N;
     a.ldk = pl->lay.ldk;
     a.stream = reinterpret_cast<cudaStream_t>(stream);
@@ -271,8 +293,8 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     // Every entry is exp(-2 pi i m / n) from the reduced integer m, evaluated in long double and
     // rounded once to the plan dtype.  [base: n = N, m = 0..N-1][stage tables, L = N][L = N/2].
     std::vector<unsigned char> host(lay.table_bytes);
-    size_t off_twN, off_twM;
-    table_entries(N, &off_twN, &off_twM);
+    size_t off_twN, off_twM, off_twX;
+    table_entries(N, &off_twN, &off_twM, &off_twX);
     auto put = [&](size_t idx, long m, long n) {
         m %= n;
         const long double two_pi = 6.283185307179586476925286766559005768L;
@@ -304,6 +326,19 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     };
     stage_tables(off_twN, N);
     stage_tables(off_twM, N / 2);
+    {   // symmetric schedule of the mid_x transforms: stage s >= 1 with earlier radix product Ns, [r-1][k]
+        int radix[8];
+        const int S = xsched_stages(N, radix);
+        size_t o = off_twX;
+        long Ns = radix[0];
+        for (int s = 1; s < S; ++s) {
+            const int R = radix[s];
+            for (int r = 1; r < R; ++r)
+                for (long k = 0; k < Ns; ++k) put(o + (size_t)(r - 1) * Ns + k, (long)r * k, Ns * R);
+            o += (size_t)(R - 1) * Ns;
+            Ns *= R;
+        }
+    }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     CU(cudaMemcpyAsync(d_tables, host.data(), lay.table_bytes, cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));

@@ -7,13 +7,19 @@
 namespace psfft {
 
 // every supported grid size, in one place (psfft.h: 2^a 3^b, b <= 1, 8 <= N <= 1024)
+// (-D"PSFFT_SIZES(X)=X(32) X(512)" restricts the list for quick experimental builds)
+#ifdef PSFFT_SIZES
+#define PSFFT_FOR_EACH_N(X) PSFFT_SIZES(X)
+#else
 #define PSFFT_FOR_EACH_N(X) \
     X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024)
+#endif
 
 struct PassArgs {
     const void *tab;   // roots of unity exp(-2 pi i m/N), N complex of the plan dtype
     const void *twN;   // per-stage twiddle tables of the length-N transforms (y, z passes)
     const void *twM;   // per-stage twiddle tables of the length-N/2 transforms (x passes)
+    const void *twX;   // per-stage twiddle tables of the length-N transforms in the symmetric schedule (mid_x)
     int N;
     int ldk;
     cudaStream_t stream;
@@ -48,7 +54,9 @@ template <typename T> cudaError_t launch_rhs_mid_x(const PassArgs &a, const RhsA
 template <typename T> cudaError_t launch_rhs_fwd_y(const PassArgs &a, const RhsArgs &r, int *launches);
 template <typename T> cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches);
 
-// complex entries of the three tables (base, twN, twM) for grid size N
-size_t table_entries(int N, size_t *off_twN, size_t *off_twM);
+// complex entries of the four tables (base, twN, twM, twX) for grid size N
+size_t table_entries(int N, size_t *off_twN, size_t *off_twM, size_t *off_twX);
+// symmetric radix schedule of the mid_x transforms (psfft_midxg.cuh): fills radix[], returns the stage count
+int xsched_stages(int N, int *radix);
 
 }  // namespace psfft

@@ -3,7 +3,8 @@
 #pragma once
 #include "psfft_kernels.cuh"
 #include "psfft_rhs.cuh"
-#include "psfft_midx8.cuh"
+#include "psfft_cpipe.cuh"
+#include "psfft_midxg.cuh"
 #include "psfft_launch.cuh"
 #include <stdlib.h>
 
@@ -71,6 +72,29 @@ static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *ou
     return cudaGetLastError();
 }
 
+template <typename T, int N, int DIR, int TC, int TPF, int NBUF>
+static cudaError_t cpass_pipe_v(const PassArgs &a, int axis, const void *in, void *out, int fields)
+{
+    using C = Cx<T>;
+    constexpr bool PAD = (TC * sizeof(C) < 128);
+    constexpr size_t smem = (size_t)NBUF * ColMap<N, TC, PAD>::size * sizeof(C);
+    auto kern = k_cpass_pipe<T, N, DIR, TC, TPF, NBUF>;
+    cudaError_t e = set_smem(kern, smem);
+    if (e != cudaSuccess) return e;
+    const long plane = (long)a.ldk * N;
+    long axis_stride, inner, outer_stride, outer;
+    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)N * fields; }
+    else { axis_stride = plane; inner = plane; outer_stride = plane * N; outer = fields; }
+    const long ntx = (inner + TC - 1) / TC, ntiles = ntx * outer;
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    const int per_sm = (int)(227 * 1024 / (smem + 1024));
+    const long grid = ntiles < (long)sms * per_sm ? ntiles : (long)sms * per_sm;
+    kern<<<(unsigned)grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)a.twN, axis_stride, inner,
+                                                        outer_stride, (int)ntx, ntiles);
+    return cudaGetLastError();
+}
+
 template <typename T, int N, int DIR>
 static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
@@ -88,6 +112,9 @@ static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *ou
             case 4: return cpass_v<T, N, DIR, 16, 32, 1>(a, axis, in, out, fields);
             case 5: return cpass_v<T, N, DIR, 2, 64, 1>(a, axis, in, out, fields);
             case 6: return cpass_v<T, N, DIR, 8, 64, 1>(a, axis, in, out, fields);
+            case 7: return cpass_pipe_v<T, N, DIR, 8, 64, 2>(a, axis, in, out, fields);
+            case 8: return cpass_pipe_v<T, N, DIR, 8, 64, 3>(a, axis, in, out, fields);
+            case 9: return cpass_pipe_v<T, N, DIR, 8, 32, 3>(a, axis, in, out, fields);
             default: break;
         }
     }
@@ -163,18 +190,20 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_y_n(cons
 }
 
 template <typename T, int N, int NV, int NS, int MINB>
-static cudaError_t mid_x8_launch(const PassArgs &a, const RhsArgs &r, long wnf, int kxp)
+static cudaError_t mid_xg_launch(const PassArgs &a, const RhsArgs &r, long wnf, int kxp)
 {
     using C = Cx<T>;
-    using L = Mid8<N, (int)sizeof(C)>;
-    constexpr size_t smem = (size_t)(3 * NV + 2 * NS) * L::BUF * sizeof(C);
-    auto kern = k_mid_x8<T, N, NV, NS, MINB>;
+    using PX = XPad<N, (int)sizeof(C)>;
+    constexpr int ROWS = xg_rows<N>();
+    constexpr size_t smem = (size_t)ROWS * (3 * NV + 2 * NS) * PX::BUF * sizeof(C);
+    auto kern = k_mid_xg<T, N, NV, NS, MINB>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     const T scale2 = (T)(1.0 / ((double)N * N * N * (double)N * N * N));   // both c2r factors, applied to the product
-    kern<<<(unsigned)(N * N), N / 8, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.twN, wnf, kxp, scale2);
+    kern<<<(unsigned)(N * N / ROWS), ROWS * XSched<N>::TPR, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf,
+                                                                               (const C *)a.twX, wnf, kxp, scale2);
     return cudaGetLastError();
 }
 
@@ -183,29 +212,11 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_mid_x_n(cons
     using C = Cx<T>;
     constexpr int KXP = kx_pitch(N, cpass_cols(N, (int)sizeof(C)));
     const long wnf = (long)KXP * N * N;
-    if constexpr (N == 64 || N == 512) {
-        // radix-8 two-for-one kernel (psfft_midx8.cuh): one butterfly per thread and stage
-        constexpr int MINB = (sizeof(T) == 8 ? 4 : 8) / (NV + NS);
-#ifdef PSFFT_EXPERIMENT
-        if constexpr (N == 512 && sizeof(T) == 8 && NV == 1 && NS == 0) {
-            static const int v = getenv("PSFFT_MIDX_VARIANT") ? atoi(getenv("PSFFT_MIDX_VARIANT")) : 0;
-            if (v == 4) return mid_x8_launch<T, N, NV, NS, 4>(a, r, wnf, KXP);
-            if (v == 5) return mid_x8_launch<T, N, NV, NS, 5>(a, r, wnf, KXP);
-        }
-#endif
-        return mid_x8_launch<T, N, NV, NS, MINB>(a, r, wnf, KXP);
-    } else {
-        constexpr int TPF = threads_per_fft(N / 2);
-        constexpr int NG = 6 * NV + 3 * NS;
-        constexpr size_t smem = (size_t)NG * RowMap<N / 2>::ld * sizeof(C);
-        auto kern = k_mid_x<T, N, NV, NS>;
-        cudaError_t e = set_smem(kern, smem);
-        if (e != cudaSuccess) return e;
-        const T scale = (T)(1.0 / ((double)N * N * N));
-        kern<<<(unsigned)(N * N), NG * TPF, smem, a.stream>>>((const C *)r.ybuf, (C *)r.zbuf, (const C *)a.tab,
-                                                                   (const C *)a.twM, wnf, KXP, scale);
-        return cudaGetLastError();
-    }
+    // register budget: about 8 (fp64) / 16 (fp32) warps per SM for HD, half of that for MHD / Boussinesq
+    constexpr int THREADS = xg_rows<N>() * XSched<N>::TPR;
+    constexpr int M0 = (sizeof(T) == 8 ? 256 : 512) / (THREADS * (NV + NS));
+    constexpr int MINB = M0 < 1 ? 1 : M0;
+    return mid_xg_launch<T, N, NV, NS, MINB>(a, r, wnf, KXP);
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)

@@ -7,7 +7,7 @@
 //   inv_z   u^ (masked on load) -> A_c = F_z^-1 u^_c (c = x,y,z),  B_x = F_z^-1 (i kz u^_x),
 //           G_x = F_z^-1 (i (ky u^_z - kz u^_y))  [= w^_x, complete]
 //   inv_y   -> U_c = F_y^-1 A_c,  W_x = F_y^-1 G_x,  P = F_y^-1 B_x,  D = F_y^-1 (i ky A_x)
-//   mid_x   per (z,y) row: u_c = c2r U_c, w_x = c2r W_x, w_y = c2r (P - i kx U_z), w_z = c2r (i kx U_y - D);
+//   mid_x   (psfft_midxg.cuh) per (z,y) row: u_c = c2r U_c, w_x = c2r W_x, w_y = c2r (P - i kx U_z), w_z = c2r (i kx U_y - D);
 //           n = u x w (MHD: m = u x w + j x b, e = u x b);  r2c of n -> kx < N/3 only
 //   fwd_y   in place, kx < N/3
 //   fwd_z   + epilogue on the store: 2/3 mask, projection (or i k x for the induction equation),
@@ -291,8 +291,14 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
         }
         C *o = (g == 0 ? dst[0] : dst[NV - 1]) + i * plane + s.col;
         if (!keep) { o[comp * nf] = mk<T>(0, 0); return; }
-        if (comp < 2) { o[comp * nf] = v; return; }   // raw; read back below by this same thread
-        C fx = o[0], fy = o[nf], fz = v;
+        if (comp < 2) { o[comp * nf] = v; return; }   // raw; read back here by this same thread (same address: ordered)
+        finish(s, g, i, o, __ldcg(o), __ldcg(o + nf), v);
+    }
+    // epilogue of one retained mode: (fx, fy, fz) = raw transform of the three components
+    __device__ __forceinline__ void finish(const State &s, int g, int i, C *o, C fx, C fy, C fz) const
+    {
+        const int kz = wavenumber(i, N);
+        const int kx = s.kx, ky = s.ky, kxy2 = s.kxy2;
         const T qx = (T)kx, qy = (T)ky, qz = (T)kz;
         const T k2 = (T)(kxy2 + kz * kz);
         if (g == 0) {            // a10: projection, identity at k = 0
@@ -326,121 +332,5 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
         o[0] = fx; o[nf] = fy; o[2 * nf] = fz;
     }
 };
-
-// ------------------------------------------------------------------------------------------
-// mid_x: one CTA per (z, y) row; 6 NV + 3 NS groups of TPF threads, one half-length transform each.
-//   in   NV x 6 fields (U_x, U_y, U_z, W_x, P, D) (+ NS x 3: Th, Dt, Gz), rows of ldk complex,
-//        entries kx >= N/3 unused
-//   out  3 NV + NS fields, entries kx < N/3 written
-// ------------------------------------------------------------------------------------------
-template <typename T, int N, int NV, int NS>
-__global__ void __launch_bounds__((6 * NV + 3 * NS) * threads_per_fft(N / 2))
-    k_mid_x(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
-            const Cx<T> *__restrict__ tw, long nf, int ldk, T scale)
-{
-    using C = Cx<T>;
-    constexpr int M = N / 2;
-    constexpr int TPF = threads_per_fft(M);
-    constexpr bool WARP = (TPF <= 32) && (32 % TPF == 0);
-    constexpr int KX = kx_count(N);
-    constexpr int NG = 6 * NV + 3 * NS;
-    using Map = RowMap<M>;
-    extern __shared__ __align__(16) unsigned char smraw[];
-    C *sm = reinterpret_cast<C *>(smraw);
-
-    const int g = threadIdx.x / TPF, t = threadIdx.x % TPF;
-    const bool sc = NS > 0 && g >= 6 * NV;           // gradient groups: g_x, g_y, g_z
-    const int v = sc ? NV : g / 6, gg = sc ? g - 6 * NV : g % 6;
-    const long rowoff = (long)blockIdx.x * ldk;
-    const C *f = in + (long)(v * 6) * nf + rowoff;   // the six fields of this vector (three of the scalar)
-
-    // spectral row of group gg at index k (0 for k >= KX)
-    auto spec = [&](int k) -> C {
-        if (k >= KX) return mk<T>(0, 0);
-        if (sc) return gg == 0 ? mul_ik(ld_stream(f + k), (T)k) : ld_stream(f + gg * nf + k);
-        switch (gg) {
-            case 0: return ld_stream(f + k);
-            case 1: return ld_stream(f + nf + k);
-            case 2: return ld_stream(f + 2 * nf + k);
-            case 3: return ld_stream(f + 3 * nf + k);
-            case 4: return csub(ld_stream(f + 4 * nf + k), mul_ik(ld_stream(f + 2 * nf + k), (T)k));
-            default: return csub(mul_ik(ld_stream(f + nf + k), (T)k), ld_stream(f + 5 * nf + k));
-        }
-    };
-
-    // c2r merge step (see k_xpass_c2r)
-#pragma unroll 2
-    for (int k = t; k <= M / 2; k += TPF) {
-        C a = spec(k);
-        C b = cconj(spec(M - k));
-        if (k == 0) { a.y = (T)0; b.y = (T)0; }
-        const C w = root_of<+1>(tab, k);
-        const C e = cadd(a, b);
-        const C o = mul_diri<+1>(cmul(w, csub(a, b)));
-        sm[Map::at(k, g)] = cadd(e, o);
-        if (k != 0 && 2 * k != M) sm[Map::at(M - k, g)] = cconj(csub(e, o));
-    }
-    group_sync<WARP>();
-    {
-        auto ld = [&](int) -> C { return mk<T>(0, 0); };
-        auto st = [&](int, C) {};
-        fft_stages<T, M, 1, +1, TPF, true, true, WARP, Map>(sm, tw, g, t, ld, st);
-    }
-    __syncthreads();
-
-    // a8: pointwise products; element n of a region holds the grid points (2n, 2n+1)
-    for (int n = threadIdx.x; n < M; n += NG * TPF) {
-        C q[NG];
-#pragma unroll
-        for (int j = 0; j < NG; ++j) q[j] = cscale(sm[Map::at(n, j)], scale);
-        // HD: q0..2 = u, q3..5 = w.   MHD: q0..2 = u, q3..5 = w, q6..8 = b, q9..11 = j
-        C r0, r1, r2;
-        r0.x = q[1].x * q[5].x - q[2].x * q[4].x; r0.y = q[1].y * q[5].y - q[2].y * q[4].y;
-        r1.x = q[2].x * q[3].x - q[0].x * q[5].x; r1.y = q[2].y * q[3].y - q[0].y * q[5].y;
-        r2.x = q[0].x * q[4].x - q[1].x * q[3].x; r2.y = q[0].y * q[4].y - q[1].y * q[3].y;
-        if constexpr (NV == 2) {
-            // m = u x w + j x b
-            r0.x += q[10].x * q[8].x - q[11].x * q[7].x; r0.y += q[10].y * q[8].y - q[11].y * q[7].y;
-            r1.x += q[11].x * q[6].x - q[9].x * q[8].x;  r1.y += q[11].y * q[6].y - q[9].y * q[8].y;
-            r2.x += q[9].x * q[7].x - q[10].x * q[6].x;  r2.y += q[9].y * q[7].y - q[10].y * q[6].y;
-            // e = u x b
-            C e0, e1, e2;
-            e0.x = q[1].x * q[8].x - q[2].x * q[7].x; e0.y = q[1].y * q[8].y - q[2].y * q[7].y;
-            e1.x = q[2].x * q[6].x - q[0].x * q[8].x; e1.y = q[2].y * q[6].y - q[0].y * q[8].y;
-            e2.x = q[0].x * q[7].x - q[1].x * q[6].x; e2.y = q[0].y * q[7].y - q[1].y * q[6].y;
-            sm[Map::at(n, 3)] = e0; sm[Map::at(n, 4)] = e1; sm[Map::at(n, 5)] = e2;
-        }
-        if constexpr (NS > 0) {   // s = u . grad theta
-            C d;
-            d.x = q[0].x * q[6].x + q[1].x * q[7].x + q[2].x * q[8].x;
-            d.y = q[0].y * q[6].y + q[1].y * q[7].y + q[2].y * q[8].y;
-            sm[Map::at(n, 3)] = d;
-        }
-        sm[Map::at(n, 0)] = r0; sm[Map::at(n, 1)] = r1; sm[Map::at(n, 2)] = r2;
-    }
-    __syncthreads();
-
-    // forward transforms of the 3 NV product rows (the other groups only keep the barriers company)
-    constexpr int NF = 3 * NV + NS;
-    if (WARP && g >= NF) return;
-    {
-        auto ld = [&](int) -> C { return mk<T>(0, 0); };
-        auto st = [&](int, C) {};
-        fft_stages<T, M, 1, -1, TPF, true, true, WARP, Map>(sm, tw, g, t, ld, st);
-    }
-    if (g >= NF) return;
-    C *dst = out + (long)g * nf + rowoff;
-#pragma unroll 2
-    for (int k = t; k <= M / 2; k += TPF) {
-        const C zk = sm[Map::at(k, g)];
-        const C zm = cconj(sm[Map::at((M - k) % M, g)]);
-        const C w = root_of<-1>(tab, k);
-        const C e = cscale(cadd(zk, zm), (T)0.5);
-        const C d = cscale(csub(zk, zm), (T)0.5);
-        const C o = mul_diri<-1>(cmul(w, d));
-        if (k < KX) st_stream(dst + k, cadd(e, o));
-        if (2 * k != M && M - k < KX) st_stream(dst + (M - k), cconj(csub(e, o)));
-    }
-}
 
 }  // namespace psfft
