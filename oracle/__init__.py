@@ -192,3 +192,17 @@ def boussinesq_rhs(uhat, thhat, nu: float = 0.0, kappa: float = 0.0, nbv: float 
     _load().orc_boussinesq_rhs(ctypes.c_int(N), _p(u), _p(t), ctypes.c_double(nu), ctypes.c_double(kappa),
                                ctypes.c_double(nbv), _p(ru), _p(rt))
     return ru, rt
+
+
+def rk_step(sys: int, y, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0, nbv: float = 0.0) -> np.ndarray:
+    """O9: one low-storage Runge-Kutta step of `ord` stages (reading G21):
+    y^(ord) = y_n; y^(o-1) = M y_n + (dt/o) R(y^(o)), o = ord..1.  sys 0 = HD (y: 3 fields), 1 = MHD (u^, b^: 6
+    fields; c2 = eta), 2 = Boussinesq (u^, theta^: 4 fields; c2 = kappa)."""
+    y = _c128(y)
+    N = y.shape[-2]
+    assert y.shape == ({0: 3, 1: 6, 2: 4}[sys], N, N, N // 2 + 1)
+    out = np.empty_like(y)
+    par = (ctypes.c_double * 3)(nu, c2, nbv)
+    _load().orc_rk_step(ctypes.c_int(N), ctypes.c_int(sys), ctypes.c_int(ord), ctypes.c_double(dt), par, _p(y),
+                        _p(out))
+    return out

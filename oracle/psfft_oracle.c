@@ -570,3 +570,39 @@ void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, d
     free(um);
     free(tm);
 }
+
+/* ---------------------------------------------------------------------------------------
+ * O9  rk_step: one explicit Runge-Kutta time step around the right-hand sides above.
+ *     "the system of ODEs is solved using an explicit Runge-Kutta scheme (of
+ *     2nd-4th order); explicit time stepping is used to resolve all wave modes".  The paper does
+ *     not print the scheme; reading G21 takes the low-storage form with `ord` stages
+ *         y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0)
+ *     (R = O6 / O7 / O8, M = the 2/3 mask).  For a linear R = L y this is the degree-`ord` Taylor
+ *     polynomial of exp(dt L), i.e. order `ord`; for the nonlinear terms it is second order.
+ *     sys: 0 = HD (y = u^, 3 fields), 1 = MHD (y = u^, b^: 6 fields), 2 = Boussinesq (y = u^, theta^: 4).
+ *     par = { nu, eta (MHD) or kappa (Boussinesq), N_bv }.
+ * ------------------------------------------------------------------------------------- */
+static void rk_rhs(int N, int sys, const double *par, const cplx *y, cplx *r)
+{
+    long nf = (long)N * N * (N / 2 + 1);
+    if (sys == 0) orc_hd_rhs(N, y, par[0], r);
+    else if (sys == 1) orc_mhd_rhs(N, y, y + 3 * nf, par[0], par[1], r, r + 3 * nf);
+    else orc_boussinesq_rhs(N, y, y + 3 * nf, par[0], par[1], par[2], r, r + 3 * nf);
+}
+
+void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cplx *y0, cplx *y1)
+{
+    int nfields = sys == 0 ? 3 : sys == 1 ? 6 : 4;
+    long nf = (long)N * N * (N / 2 + 1), n = nfields * nf;
+    cplx *ym = (cplx *)malloc(sizeof(cplx) * n);   /* M y_n */
+    cplx *r = (cplx *)malloc(sizeof(cplx) * n);
+    memcpy(ym, y0, sizeof(cplx) * n);
+    orc_apply_mask(N, nfields, ym);
+    memcpy(y1, y0, sizeof(cplx) * n);              /* y^(ord) = y_n */
+    for (int o = ord; o >= 1; --o) {
+        rk_rhs(N, sys, par, y1, r);
+        for (long i = 0; i < n; ++i) y1[i] = ym[i] + (dt / o) * r[i];
+    }
+    free(ym);
+    free(r);
+}
