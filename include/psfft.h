@@ -142,6 +142,26 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
                          void *d_rhs_th, double nu, double kappa, double nbv, void *d_work,
                          void *stream);
 
+/* One explicit Runge-Kutta time step around a right-hand side above ("the system of ODEs
+ * is solved using an explicit Runge-Kutta scheme (of 2nd-4th order)"; the paper does not print the
+ * scheme -- DESIGN.md reading G21: the low-storage form with `ord` stages
+ *     y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0) ).
+ * Each stage is one fused right-hand-side evaluation whose last pass writes M y_n + (dt/o) R instead of
+ * R (one more sparse read of y_n in its epilogue); there is no separate update kernel.
+ *   system    PSFFT_SYS_HD (y = u^: 3 fields), PSFFT_SYS_MHD (u^, b^: 6), PSFFT_SYS_BOUSSINESQ (u^, theta^: 4)
+ *   d_y_in    in   the state y_n, fields contiguous in the order above (not modified)
+ *   d_y_out   out  y_{n+1} (dealiased); must not overlap d_y_in
+ *   ord       1..4 stages
+ *   params    HOST pointer to 3 doubles: { nu, eta (MHD) or kappa (Boussinesq), N_bv }
+ *   d_work         >= psfft_rk_work_bytes(plan, system) = one state-sized stage buffer + the RHS workspace
+ * Returns PSFFT_E_SIZE for a bad system / ord or d_y_in == d_y_out. */
+#define PSFFT_SYS_HD 0
+#define PSFFT_SYS_MHD 1
+#define PSFFT_SYS_BOUSSINESQ 2
+size_t psfft_rk_work_bytes(psfft_plan plan, int system);
+int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out, int ord, double dt,
+                  const double *params, void *d_work, void *stream);
+
 /* The same two right-hand sides computed as the plain composition of the public passes: mask +
  * curl kernel, 6 (12) three-pass inverse transforms, pointwise product kernel, 3 (6) three-pass
  * forward transforms, mask + projection kernel.  Nothing is fused or pruned: every pass touches

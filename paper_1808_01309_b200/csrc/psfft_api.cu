@@ -205,6 +205,9 @@ struct RhsSys {
     const void *uhat, *bhat, *thhat;
     void *ru, *rb, *rt;
     double nu, eta, kappa, nbv;
+    // Runge-Kutta stage: outputs are base + cstep * rhs (base_u == NULL: plain right-hand side)
+    const void *base_u, *base_b, *base_t;
+    double cstep;
 };
 
 template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys &y, void *work)
@@ -219,6 +222,7 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     r.diff[0] = y.nu; r.diff[1] = y.eta;
     r.ssrc = y.thhat; r.sdst = y.rt;
     r.sdiff = y.kappa; r.nbv = y.nbv;
+    r.base[0] = y.base_u; r.base[1] = y.base_b; r.sbase = y.base_t; r.cstep = y.cstep;
     const size_t W = (size_t)a.N * a.N * kx_pitch(a.N, cpass_cols(a.N, (int)(2 * sizeof(T)))) * 2 * sizeof(T);
     r.zbuf = work;                                         // 5 nv + 2 ns compact fields (later 3 nv + ns: mid_x out, fwd_y in place)
     r.ybuf = off(work, (size_t)(5 * nv + 2 * ns) * W);     // 6 nv + 3 ns compact fields
@@ -228,11 +232,12 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     const double nepi = (y.nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && y.eta != 0.0 ? 3.0 : 0.0) +
                         (ns ? (y.kappa != 0.0 || y.nbv != 0.0 ? 1.0 : 0.0) + (y.nbv != 0.0 && y.nu == 0.0 ? 1.0 : 0.0) : 0.0);
     const int zin = 3 * nv + ns, zf = 5 * nv + 2 * ns, yf = 6 * nv + 3 * ns, ff = 3 * nv + ns;
+    const double nbase = y.base_u ? (double)ff : 0.0;   // sparse reads of y_n in a Runge-Kutta stage
     { ProfScope ps(pl, a.stream, K_INVZ, zin * sph + zf * disc); CU(launch_rhs_inv_z<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_INVY, zf * disc + yf * rows); CU(launch_rhs_inv_y<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_MIDX, yf * rows + ff * rows); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_FWDY, ff * rows + ff * disc); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (double)C + nepi * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (double)C + (nepi + nbase) * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -425,7 +430,8 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     if (fused) {
-        const RhsSys y = {1, 0, d_uhat, nullptr, nullptr, d_rhs, nullptr, nullptr, nu, 0.0, 0.0, 0.0};
+        const RhsSys y = {1, 0, d_uhat, nullptr, nullptr, d_rhs, nullptr, nullptr, nu, 0.0, 0.0, 0.0,
+                          nullptr, nullptr, nullptr, 0.0};
         return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
     }
     return pl->lay.dtype == PSFFT_F64 ? hd_rhs_t<double>(pl, a, d_uhat, d_rhs, nu, d_work)
@@ -443,7 +449,8 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     if (fused) {
-        const RhsSys y = {2, 0, d_uhat, d_bhat, nullptr, d_rhs_u, d_rhs_b, nullptr, nu, eta, 0.0, 0.0};
+        const RhsSys y = {2, 0, d_uhat, d_bhat, nullptr, d_rhs_u, d_rhs_b, nullptr, nu, eta, 0.0, 0.0,
+                          nullptr, nullptr, nullptr, 0.0};
         return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
     }
     return pl->lay.dtype == PSFFT_F64 ? mhd_rhs_t<double>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
@@ -482,8 +489,60 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
         return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
-    const RhsSys y = {1, 1, d_uhat, nullptr, d_thhat, d_rhs_u, nullptr, d_rhs_th, nu, 0.0, kappa, nbv};
+    const RhsSys y = {1, 1, d_uhat, nullptr, d_thhat, d_rhs_u, nullptr, d_rhs_th, nu, 0.0, kappa, nbv,
+                      nullptr, nullptr, nullptr, 0.0};
     return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
+}
+
+size_t psfft_rk_work_bytes(psfft_plan plan, int system)
+{
+    Plan *pl = get(plan);
+    if (!pl || system < 0 || system > 2) return 0;
+    const size_t rhs = system == PSFFT_SYS_HD ? pl->lay.work_bytes_hd
+                     : system == PSFFT_SYS_MHD ? pl->lay.work_bytes_mhd : pl->lay.work_bytes_boussinesq;
+    const size_t nfields = system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : 4;
+    return nfields * pl->lay.spec_bytes + rhs;
+}
+
+int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out, int ord, double dt,
+                  const double *params, void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_y_in || !d_y_out || !d_work || !params) return PSFFT_E_NULL;
+    if (system < 0 || system > 2 || ord < 1 || ord > 4 || d_y_in == d_y_out) return PSFFT_E_SIZE;
+    if (misaligned(d_y_in) || misaligned(d_y_out) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    const size_t C = pl->lay.spec_bytes;
+    const int nfields = system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : 4;
+    void *stage = d_work;                                  // one state-sized stage buffer
+    void *rhswork = off(d_work, (size_t)nfields * C);
+    const void *cur = d_y_in;
+    for (int j = 1; j <= ord; ++j) {
+        // stage outputs alternate between the stage buffer and d_y_out so that the last one lands in d_y_out
+        void *out = ((ord - j) % 2 == 0) ? d_y_out : stage;
+        RhsSys y;
+        y.nv = system == PSFFT_SYS_MHD ? 2 : 1;
+        y.ns = system == PSFFT_SYS_BOUSSINESQ ? 1 : 0;
+        y.uhat = cur; y.ru = out; y.base_u = d_y_in;
+        y.bhat = y.nv == 2 ? off(cur, 3 * C) : nullptr;
+        y.rb = y.nv == 2 ? off(out, 3 * C) : nullptr;
+        y.base_b = y.nv == 2 ? off(d_y_in, 3 * C) : nullptr;
+        y.thhat = y.ns ? off(cur, 3 * C) : nullptr;
+        y.rt = y.ns ? off(out, 3 * C) : nullptr;
+        y.base_t = y.ns ? off(d_y_in, 3 * C) : nullptr;
+        y.nu = params[0];
+        y.eta = system == PSFFT_SYS_MHD ? params[1] : 0.0;
+        y.kappa = system == PSFFT_SYS_BOUSSINESQ ? params[1] : 0.0;
+        y.nbv = system == PSFFT_SYS_BOUSSINESQ ? params[2] : 0.0;
+        y.cstep = dt / (double)(ord - j + 1);
+        const int rc = pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, rhswork)
+                                                  : rhs_fused_t<float>(pl, a, y, rhswork);
+        if (rc) return rc;
+        cur = out;
+    }
+    return PSFFT_OK;
 }
 
 int psfft_fft3d_r2c_host(psfft_plan plan, const void *h_real, void *h_spec, void *d_in, void *d_out, void *d_work,

@@ -45,6 +45,11 @@ struct RhsArgs {
     const void *ssrc;     // ns = 1: theta^
     void *sdst;           // ns = 1: rhs_theta
     double sdiff, nbv;    // kappa, Brunt-Vaisala frequency N_bv
+    // Runge-Kutta stage (psfft_rk_step): when base[0] != NULL the outputs are base + cstep * rhs on the retained
+    // modes (base = the state y_n at the start of the step, in the same order as src / ssrc)
+    const void *base[2];
+    const void *sbase;
+    double cstep;
     void *zbuf;           // 5 nv + 2 ns compact fields (inv_z out; later mid_x out / fwd_y in place, 3 nv + ns fields)
     void *ybuf;           // 6 nv + 3 ns compact fields (inv_y out)
 };

@@ -243,6 +243,9 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(cons
     job.saux = (const C *)r.ssrc;
     job.sdiff = (T)r.sdiff;
     job.nbv = (T)r.nbv;
+    for (int v = 0; v < NV; ++v) job.base[v] = (const C *)r.base[v];
+    job.sbase = (const C *)r.sbase;
+    job.cstep = (T)r.cstep;
     job.src = (const C *)r.zbuf;
     for (int v = 0; v < NV; ++v) {
         job.dst[v] = (C *)r.dst[v];

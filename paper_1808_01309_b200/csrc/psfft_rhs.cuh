@@ -222,6 +222,9 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
     C *sdst;             // NS = 1: R_theta, caller layout
     const C *saux;       // NS = 1: theta^
     T sdiff, nbv;        // kappa, N_bv
+    const C *base[NV];   // Runge-Kutta stage: y_n (NULL: plain right-hand side); out = base + cstep * rhs
+    const C *sbase;
+    T cstep;
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
     int ldk;
@@ -286,6 +289,10 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
                 const C th = ldg_c(saux + i * plane + s.col);
                 rt.x -= sc * th.x; rt.y -= sc * th.y;
             }
+            if (sbase != nullptr) {   // Runge-Kutta stage
+                const C y0 = ldg_c(sbase + i * plane + s.col);
+                rt.x = y0.x + cstep * rt.x; rt.y = y0.y + cstep * rt.y;
+            }
             *os = rt;
             return;
         }
@@ -328,6 +335,14 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ {
             fx.x -= sc * ax.x; fx.y -= sc * ax.y;
             fy.x -= sc * ay.x; fy.y -= sc * ay.y;
             fz.x -= sc * az.x; fz.y -= sc * az.y;
+        }
+        const C *yb = g == 0 ? base[0] : base[NV - 1];
+        if (yb != nullptr) {   // Runge-Kutta stage: y_n + (dt / o) R
+            yb += i * plane + s.col;
+            const C bx = ldg_c(yb), by = ldg_c(yb + nf), bz = ldg_c(yb + 2 * nf);
+            fx.x = bx.x + cstep * fx.x; fx.y = bx.y + cstep * fx.y;
+            fy.x = by.x + cstep * fy.x; fy.y = by.y + cstep * fy.y;
+            fz.x = bz.x + cstep * fz.x; fz.y = bz.y + cstep * fz.y;
         }
         o[0] = fx; o[nf] = fy; o[2 * nf] = fz;
     }

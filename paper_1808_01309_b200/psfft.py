@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
     "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs",
+    "psfft_rk_work_bytes", "psfft_rk_step",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
     "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
@@ -61,6 +62,9 @@ def lib() -> ctypes.CDLL:
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_boussinesq_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, cd, vp, vp]
+        L.psfft_rk_work_bytes.argtypes = [vp, ci]
+        L.psfft_rk_work_bytes.restype = sz
+        L.psfft_rk_step.argtypes = [vp, ci, vp, vp, ci, cd, ctypes.POINTER(cd), vp, vp]
         L.psfft_hd_rhs_unfused.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs_unfused.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -151,6 +155,20 @@ def boussinesq_rhs(plan: int, d_uhat, d_thhat, d_rhs_u, d_rhs_th, nu: float, kap
                                       float(kappa), float(nbv), _ptr(d_work), _stream(stream)), "psfft_boussinesq_rhs")
 
 
+SYS_HD, SYS_MHD, SYS_BOUSSINESQ = 0, 1, 2
+
+
+def rk_work_bytes(plan: int, system: int) -> int:
+    return int(lib().psfft_rk_work_bytes(plan, system))
+
+
+def rk_step(plan: int, system: int, d_y_in, d_y_out, ord: int, dt: float, params, d_work, stream=None) -> None:
+    """params = (nu, eta | kappa, N_bv), passed as a host array of 3 doubles."""
+    par = (ctypes.c_double * 3)(*[float(x) for x in params])
+    _check(lib().psfft_rk_step(plan, system, _ptr(d_y_in), _ptr(d_y_out), ord, float(dt), par, _ptr(d_work),
+                               _stream(stream)), "psfft_rk_step")
+
+
 def hd_rhs_unfused(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
     _check(lib().psfft_hd_rhs_unfused(plan, _ptr(d_uhat), _ptr(d_rhs), float(nu), _ptr(d_work), _stream(stream)),
            "psfft_hd_rhs_unfused")
@@ -232,7 +250,10 @@ class Plan:
 
     def ensure_work(self, kind: str):
         need = {"fft": self.layout.work_bytes_fft, "hd": self.layout.work_bytes_hd,
-                "mhd": self.layout.work_bytes_mhd, "boussinesq": self.layout.work_bytes_boussinesq}[kind]
+                "mhd": self.layout.work_bytes_mhd, "boussinesq": self.layout.work_bytes_boussinesq,
+                "rk_hd": 3 * self.layout.spec_bytes + self.layout.work_bytes_hd,
+                "rk_mhd": 6 * self.layout.spec_bytes + self.layout.work_bytes_mhd,
+                "rk_boussinesq": 4 * self.layout.spec_bytes + self.layout.work_bytes_boussinesq}[kind]
         if self._work is None or self._work.numel() < need:
             self._work = None
             self._work = torch.empty(need, dtype=torch.uint8, device=self.device)
@@ -291,3 +312,15 @@ class Plan:
         ru, rt = torch.empty_like(uhat), torch.empty_like(thhat)
         boussinesq_rhs(self.handle, uhat, thhat, ru, rt, nu, kappa, nbv, self.ensure_work("boussinesq"))
         return ru, rt
+
+    def rk_step(self, system: int, y: torch.Tensor, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0,
+                nbv: float = 0.0, out: torch.Tensor | None = None) -> torch.Tensor:
+        """One Runge-Kutta step; y: [3 | 6 | 4, N, N, N/2+1] complex (HD | MHD u,b | Boussinesq u,theta)."""
+        nf = {SYS_HD: 3, SYS_MHD: 6, SYS_BOUSSINESQ: 4}[system]
+        assert y.is_cuda and y.dtype == self.cdtype and y.is_contiguous() and tuple(y.shape) == self.spec_shape(nf)
+        if out is None:
+            out = torch.empty_like(y)
+        work = self.ensure_work({SYS_HD: "rk_hd", SYS_MHD: "rk_mhd", SYS_BOUSSINESQ: "rk_boussinesq"}[system])
+        assert rk_work_bytes(self.handle, system) <= work.numel()
+        rk_step(self.handle, system, y, out, ord, dt, (nu, c2, nbv), work)
+        return out

@@ -228,6 +228,52 @@ def test_boussinesq_reduces_to_hd_when_theta_vanishes():
     assert float((ru - hd).norm() / hd.norm()) < 1e-14 and float(rt.abs().max()) == 0.0
 
 
+# ---- Runge-Kutta step -------------------------------------------------
+
+def rk_state(system, N, k0, kcut, dtype):
+    u = synth.solenoidal_spectrum(N, k0, kcut, 1234, tag=0)
+    if system == psfft.SYS_HD:
+        y = u
+    elif system == psfft.SYS_MHD:
+        y = np.concatenate([u, synth.solenoidal_spectrum(N, k0, kcut, 1234, tag=1)])
+    else:
+        y = np.concatenate([u, synth.scalar_spectrum(N, k0, kcut, 1234)[None]])
+    return np.ascontiguousarray(y.astype(CDT[dtype]))
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("system", [0, 1, 2])
+@pytest.mark.parametrize("N,ord", [(16, 1), (24, 2), (32, 3), (48, 4), (64, 2), (96, 4)])
+def test_rk_step_matches_oracle(N, ord, system, dtype):
+    """dt chosen so that dt * |R| is comparable to |y| (CFL-like): the stages feed on each other."""
+    y = rk_state(system, N, 3.0, N // 2 - 1, dtype)
+    dt, nu, c2, nbv = 0.02, 0.013, 0.021, 2.5
+    p = psfft.Plan(N, dtype, 1)
+    yd = dev(y)
+    got = p.rk_step(system, yd, ord, dt, nu, c2, nbv).cpu().numpy()
+    assert np.array_equal(yd.cpu().numpy(), y)                      # y_n untouched
+    want = oracle.rk_step(system, y.astype(np.complex128), ord, dt, nu, c2, nbv)
+    assert rel(got, want) < TOL[dtype]
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+    assert rel(got, y) > 1e-3                                        # the step did something
+
+
+def test_rk_step_beltrami_closed_form_and_argument_checks():
+    """ABC flow under viscosity: one RK4 step multiplies u^ by 1 + x + x^2/2 + x^3/6 + x^4/24, x = -nu dt."""
+    N, nu, dt = 32, 0.7, 0.05
+    uh = np.stack([oracle.r2c3d(f) for f in synth.abc_flow(N)])
+    p = psfft.Plan(N, torch.float64, 1)
+    got = p.rk_step(psfft.SYS_HD, dev(uh), 4, dt, nu).cpu().numpy()
+    x = -nu * dt
+    assert rel(got, (1 + x + x * x / 2 + x ** 3 / 6 + x ** 4 / 24) * uh) < 1e-13
+    yd = dev(uh)
+    work = p.ensure_work("rk_hd")
+    with pytest.raises(psfft.PsfftError):
+        psfft.rk_step(p.handle, psfft.SYS_HD, yd, yd, 2, dt, (nu, 0, 0), work)          # in == out
+    with pytest.raises(psfft.PsfftError):
+        psfft.rk_step(p.handle, psfft.SYS_HD, yd, torch.empty_like(yd), 5, dt, (nu, 0, 0), work)   # ord > 4
+
+
 # ---- host-buffer (end-to-end) entry points -----------------------------------------------------------
 
 def test_host_entry_points():
