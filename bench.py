@@ -336,13 +336,33 @@ def run_ours(args) -> int:
                  "roundtrip_max_abs_err": rt_err}
         del x, X, y
 
+    # ---- the rows SURVEY.md §8(f) marks "next", same size, same protocol (device-resident) --------------
+    next_rows = None
+    if world == 1:
+        th = torch.from_numpy(synth.scalar_spectrum(N, 4.0, kcut, 1234)).to(dev)
+        rt = torch.empty_like(th)
+        bwork = plan.ensure_work("rk_boussinesq")
+        f_b = lambda: psfft.boussinesq_rhs(h, uh, th, rhs, rt, 1e-3, 1e-3, 1.0, bwork)
+        f_rk = lambda: psfft.rk_step(h, psfft.SYS_HD, uh, rhs, 2, 1e-3, (1e-3, 0.0, 0.0), bwork)
+        for f in (f_b, f_rk):
+            for _ in range(3):
+                f()
+        torch.cuda.synchronize()
+        t_b = time_loop(f_b, K, stream)
+        t_rk = time_loop(f_rk, K, stream)
+        next_rows = {"boussinesq_rhs": {"ms": t_b, "evals_per_s": 1e3 / t_b,
+                                        "workload": f"{N}^3 fp64, u as above + random-phase theta, nu = kappa = 1e-3, N_bv = 1"},
+                     "hd_rk2_step": {"ms": t_rk, "steps_per_s": 1e3 / t_rk,
+                                     "workload": f"{N}^3 fp64, two fused RHS stages, nu = 1e-3, dt = 1e-3"}}
+        del th, rt
+
     if rank != 0:
         return 0
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(N, world), "clocks": clk, "e2e": e2e,
             "gpu_launches": launches_per_step * K, "launches_per_step": launches_per_step,
-            "roofline": roofline, "fft3d": fft3d}
+            "roofline": roofline, "fft3d": fft3d, "next_rows": next_rows}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(N)
     print(json.dumps(line), flush=True)
