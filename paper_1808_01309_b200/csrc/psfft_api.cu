@@ -131,7 +131,7 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     o->table_bytes = table_entries(N, nullptr, nullptr, nullptr) * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
     // fused path: 5 + 6 compact fields [N][N][kx_pitch] per vector field; unfused path: 12 C per vector field
-    const size_t wfield = (size_t)N * N * kx_pitch(N, cpass_cols(N, (int)(2 * s))) * 2 * s;
+    const size_t wfield = (size_t)N * N * rhs_pitch(N, (int)(2 * s)) * 2 * s;
     o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
     o->work_bytes_mhd = 2 * o->work_bytes_hd;
     o->work_bytes_boussinesq = 16 * wfield;   // 5 + 2 z-fields, 6 + 3 y-fields
@@ -223,7 +223,7 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     r.ssrc = y.thhat; r.sdst = y.rt;
     r.sdiff = y.kappa; r.nbv = y.nbv;
     r.base[0] = y.base_u; r.base[1] = y.base_b; r.sbase = y.base_t; r.cstep = y.cstep;
-    const size_t W = (size_t)a.N * a.N * kx_pitch(a.N, cpass_cols(a.N, (int)(2 * sizeof(T)))) * 2 * sizeof(T);
+    const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
     r.zbuf = work;                                         // 5 nv + 2 ns compact fields (later 3 nv + ns: mid_x out, fwd_y in place)
     r.ybuf = off(work, (size_t)(5 * nv + 2 * ns) * W);     // 6 nv + 3 ns compact fields
     const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;

@@ -46,6 +46,108 @@ template <int DIR, typename C> __device__ __forceinline__ C mul_diri(C a)
 template <typename C, typename T> __device__ __forceinline__ C cscale(C a, T s) { a.x *= s; a.y *= s; return a; }
 
 // ------------------------------------------------------------------------------------------
+// fp32 column passes: one thread carries TWO adjacent columns as a float2x2 -- two complex numbers
+// (a, b) held component-wise, re = (re_a, re_b), im = (im_a, im_b) -- so that every complex add /
+// multiply of a butterfly is issued once for both columns with Blackwell's packed fp32 instructions
+// (FADD2 / FMUL2 / FFMA2, add/mul/fma.f32x2: sm_100+), twiddles entering as scalar broadcast operands.
+// Ex<T> is the element a column pass works on: double2 (one column) or float2x2 (two columns), 16 bytes
+// either way, so tile shapes, shared-memory maps and thread counts are the same for both precisions.
+// ------------------------------------------------------------------------------------------
+struct __align__(16) float2x2 { float2 re, im; };
+template <typename T> struct ExOf;
+template <> struct ExOf<float> { using type = float2x2; };
+template <> struct ExOf<double> { using type = double2; };
+template <typename T> using Ex = typename ExOf<T>::type;
+template <typename E> struct ElemWidth { static constexpr int value = 1; };
+template <> struct ElemWidth<float2x2> { static constexpr int value = 2; };
+
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+__device__ __forceinline__ float2 bc2(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2x2 cadd(float2x2 a, float2x2 b)
+{
+    float2x2 r;
+    r.re = __fadd2_rn(a.re, b.re);
+    r.im = __fadd2_rn(a.im, b.im);
+    return r;
+}
+__device__ __forceinline__ float2x2 csub(float2x2 a, float2x2 b)
+{
+    float2x2 r;
+    r.re = __fadd2_rn(a.re, neg2(b.re));
+    r.im = __fadd2_rn(a.im, neg2(b.im));
+    return r;
+}
+// both columns times the same complex scalar w
+__device__ __forceinline__ float2x2 cmul(float2x2 a, float2 w)
+{
+    float2x2 r;
+    r.re = __ffma2_rn(a.re, bc2(w.x), neg2(__fmul2_rn(a.im, bc2(w.y))));
+    r.im = __ffma2_rn(a.re, bc2(w.y), __fmul2_rn(a.im, bc2(w.x)));
+    return r;
+}
+template <int DIR> __device__ __forceinline__ float2x2 mul_diri(float2x2 a)
+{
+    float2x2 r;
+    if (DIR < 0) { r.re = a.im; r.im = neg2(a.re); }
+    else { r.re = neg2(a.im); r.im = a.re; }
+    return r;
+}
+__device__ __forceinline__ float2x2 cscale(float2x2 a, float s)
+{
+    a.re = __fmul2_rn(a.re, bc2(s));
+    a.im = __fmul2_rn(a.im, bc2(s));
+    return a;
+}
+template <typename E> __device__ __forceinline__ E ezero();
+template <> __device__ __forceinline__ double2 ezero<double2>() { return make_double2(0.0, 0.0); }
+template <> __device__ __forceinline__ float2 ezero<float2>() { return make_float2(0.f, 0.f); }
+template <> __device__ __forceinline__ float2x2 ezero<float2x2>()
+{
+    float2x2 r;
+    r.re = make_float2(0.f, 0.f);
+    r.im = r.re;
+    return r;
+}
+// column j of an element / set column j
+__device__ __forceinline__ double2 ecol(double2 e, int) { return e; }
+__device__ __forceinline__ float2 ecol(float2 e, int) { return e; }
+__device__ __forceinline__ float2 ecol(float2x2 e, int j) { return j == 0 ? make_float2(e.re.x, e.im.x) : make_float2(e.re.y, e.im.y); }
+__device__ __forceinline__ void ecol_set(double2 &e, int, double2 v) { e = v; }
+__device__ __forceinline__ void ecol_set(float2 &e, int, float2 v) { e = v; }
+__device__ __forceinline__ void ecol_set(float2x2 &e, int j, float2 v)
+{
+    if (j == 0) { e.re.x = v.x; e.im.x = v.y; }
+    else { e.re.y = v.x; e.im.y = v.y; }
+}
+// v (1 + DIR i)/sqrt 2  and  v (-1 + DIR i)/sqrt 2  (the odd eighth roots of a radix-8 butterfly)
+template <int DIR, typename T, typename C> __device__ __forceinline__ C mul_w8_1(C v)
+{
+    const T h = (T)0.70710678118654752440084436210485;
+    return DIR < 0 ? mk<T>((v.x + v.y) * h, (v.y - v.x) * h) : mk<T>((v.x - v.y) * h, (v.x + v.y) * h);
+}
+template <int DIR, typename T, typename C> __device__ __forceinline__ C mul_w8_3(C v)
+{
+    const T h = (T)0.70710678118654752440084436210485;
+    return DIR < 0 ? mk<T>((v.y - v.x) * h, -(v.x + v.y) * h) : mk<T>(-(v.x + v.y) * h, (v.x - v.y) * h);
+}
+template <int DIR, typename T> __device__ __forceinline__ float2x2 mul_w8_1(float2x2 v)
+{
+    const float h = 0.70710678118654752440f;
+    float2x2 r;
+    if (DIR < 0) { r.re = __fmul2_rn(__fadd2_rn(v.re, v.im), bc2(h)); r.im = __fmul2_rn(__fadd2_rn(v.im, neg2(v.re)), bc2(h)); }
+    else { r.re = __fmul2_rn(__fadd2_rn(v.re, neg2(v.im)), bc2(h)); r.im = __fmul2_rn(__fadd2_rn(v.re, v.im), bc2(h)); }
+    return r;
+}
+template <int DIR, typename T> __device__ __forceinline__ float2x2 mul_w8_3(float2x2 v)
+{
+    const float h = 0.70710678118654752440f;
+    float2x2 r;
+    if (DIR < 0) { r.re = __fmul2_rn(__fadd2_rn(v.im, neg2(v.re)), bc2(h)); r.im = __fmul2_rn(__fadd2_rn(v.re, v.im), bc2(-h)); }
+    else { r.re = __fmul2_rn(__fadd2_rn(v.re, v.im), bc2(-h)); r.im = __fmul2_rn(__fadd2_rn(v.re, neg2(v.im)), bc2(h)); }
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
 // compile-time radix schedule
 // ------------------------------------------------------------------------------------------
 __host__ __device__ constexpr int pow2_part(int n) { int p = 1; while (n % 2 == 0) { n /= 2; p *= 2; } return p; }
@@ -93,6 +195,11 @@ __host__ __device__ constexpr int cpass_cols(int N, int csize)
 __host__ __device__ constexpr int kx_count(int N) { return (N - 1) / 3 + 1; }
 __host__ __device__ constexpr int kx_pitch(int N, int TC) { return (kx_count(N) + TC - 1) / TC * TC; }
 
+// RHS column passes work on 16-byte elements Ex<T> (one fp64 column or two packed fp32 columns, below):
+// tile = [N rows] x [job_cols(N) elements]; the workspace row pitch is a whole number of tiles.
+__host__ __device__ constexpr int job_cols(int N) { return cpass_cols(N, 16); }
+__host__ __device__ constexpr int rhs_pitch(int N, int csize) { return kx_pitch(N, job_cols(N) * (16 / csize)); }
+
 // Per-stage twiddle tables.  Stage with earlier radix product Ns (> 1) and radix R needs
 // w_{Ns R}^{r k}, k in [0, Ns), r in [1, R).  They are stored as [r-1][k] (k contiguous, so the
 // lanes of a warp -- consecutive k -- read consecutive 16-byte entries), stage after stage.
@@ -131,7 +238,7 @@ template <int DIR, typename T, typename C> __device__ __forceinline__ void bfly3
 {
     const T s = (T)0.86602540378443864676372317075294;  // sqrt(3)/2
     C t = cadd(v1, v2);
-    C m = mk<T>(v0.x - (T)0.5 * t.x, v0.y - (T)0.5 * t.y);
+    C m = csub(v0, cscale(t, (T)0.5));
     C d = mul_diri<DIR>(cscale(csub(v1, v2), s));
     v0 = cadd(v0, t);
     v1 = cadd(m, d);
@@ -140,18 +247,10 @@ template <int DIR, typename T, typename C> __device__ __forceinline__ void bfly3
 
 template <int DIR, typename T, typename C> __device__ __forceinline__ void bfly8(C *v)
 {
-    const T h = (T)0.70710678118654752440084436210485;  // 1/sqrt(2)
     bfly4<DIR>(v[0], v[2], v[4], v[6]);
     bfly4<DIR>(v[1], v[3], v[5], v[7]);
     // w8^1 = (1 + DIR i)/sqrt2, w8^2 = DIR i, w8^3 = (-1 + DIR i)/sqrt2
-    C o1, o3;
-    if (DIR < 0) {
-        o1 = mk<T>((v[3].x + v[3].y) * h, (v[3].y - v[3].x) * h);
-        o3 = mk<T>((v[7].y - v[7].x) * h, -(v[7].x + v[7].y) * h);
-    } else {
-        o1 = mk<T>((v[3].x - v[3].y) * h, (v[3].x + v[3].y) * h);
-        o3 = mk<T>(-(v[7].x + v[7].y) * h, (v[7].x - v[7].y) * h);
-    }
+    const C o1 = mul_w8_1<DIR, T>(v[3]), o3 = mul_w8_3<DIR, T>(v[7]);
     C o2 = mul_diri<DIR>(v[5]);
     C e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
     v[0] = cadd(e0, o0);
@@ -231,9 +330,11 @@ struct NoPost {
     template <typename C> __device__ __forceinline__ C operator()(int, C x) const { return x; }
 };
 
+// E is the element the transform works on: Cx<T> (one column per thread) or float2x2 (two fp32 columns per
+// thread, packed arithmetic); the twiddles are always scalar complex numbers Cx<T>.
 template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
-          class LD, class ST, class PX>
-__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st,
+          class LD, class ST, class PX, typename E>
+__device__ __forceinline__ void fft_stages(E *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st,
                                            PX &px)
 {
     using C = Cx<T>;
@@ -245,7 +346,7 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
     constexpr bool from_smem = !first || SRC_SMEM;
     constexpr bool to_smem = !last || DST_SMEM;
 
-    C v[ITER][R];
+    E v[ITER][R];
 #pragma unroll
     for (int it = 0; it < ITER; ++it) {
         const int b = t + it * TPF;
@@ -297,15 +398,15 @@ __device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ 
     }
     if (to_smem) group_sync<WARP>();
     if constexpr (!last)
-        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, PX>(sm, tw, c, t, ld, st, px);
+        fft_stages<T, L, Ns * R, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, PX, E>(sm, tw, c, t, ld, st, px);
 }
 
 template <typename T, int L, int Ns, int DIR, int TPF, bool SRC_SMEM, bool DST_SMEM, bool WARP, class Map,
-          class LD, class ST>
-__device__ __forceinline__ void fft_stages(Cx<T> *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st)
+          class LD, class ST, typename E>
+__device__ __forceinline__ void fft_stages(E *sm, const Cx<T> *__restrict__ tw, int c, int t, LD &ld, ST &st)
 {
     NoPost px;
-    fft_stages<T, L, Ns, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, NoPost>(sm, tw, c, t, ld, st, px);
+    fft_stages<T, L, Ns, DIR, TPF, SRC_SMEM, DST_SMEM, WARP, Map, LD, ST, NoPost, E>(sm, tw, c, t, ld, st, px);
 }
 
 }  // namespace psfft

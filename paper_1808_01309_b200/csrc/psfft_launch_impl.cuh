@@ -127,9 +127,10 @@ template <typename T, int N, int DIR, int TPF, int MINB, class Job>
 static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr bool PAD = (TC * sizeof(C) < 128);
-    constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(C);
+    using E = typename Job::Elem;
+    constexpr int TC = cpass_cols(N, (int)sizeof(E));   // elements per tile row
+    constexpr bool PAD = (TC * sizeof(E) < 128);
+    constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(E);
     auto kern = k_cpass_job<T, N, DIR, TC, TPF, MINB, Job>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
@@ -148,7 +149,7 @@ __host__ __device__ constexpr int job_tpf(int N, int TC)
 template <typename T, int N, int DIR, class Job>
 static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid, int id = 0)
 {
-    constexpr int TC = cpass_cols(N, (int)sizeof(Cx<T>));
+    constexpr int TC = cpass_cols(N, (int)sizeof(typename Job::Elem));
 #ifdef PSFFT_EXPERIMENT
     if constexpr (N == 512 && sizeof(T) == 8) {
         static const int v = getenv("PSFFT_JOB_VARIANT") ? atoi(getenv("PSFFT_JOB_VARIANT")) : 0;
@@ -162,8 +163,8 @@ static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid, int id 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int KXP = kx_pitch(N, TC);
+    constexpr int TC = job_cols(N), EW = 16 / (int)sizeof(C);   // element columns per tile, columns per element
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     JobInvZ<T, N, TC, NV, NS> job;
     for (int v = 0; v < NV; ++v) job.src[v] = (const C *)r.src[v];
     job.ssrc = (const C *)r.ssrc;
@@ -172,21 +173,21 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_z_n(cons
     job.nf = job.plane * N;
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 0);
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 0);
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int KXP = kx_pitch(N, TC);
+    constexpr int TC = job_cols(N), EW = 16 / (int)sizeof(C);   // element columns per tile, columns per element
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     JobInvY<T, N, TC, NV, NS> job;
     job.src = (const C *)r.zbuf;
     job.dst = (C *)r.ybuf;
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.kxp = KXP;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 1);
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 1);
 }
 
 template <typename T, int N, int NV, int NS, int MINB>
@@ -210,7 +211,7 @@ static cudaError_t mid_xg_launch(const PassArgs &a, const RhsArgs &r, long wnf, 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_mid_x_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int KXP = kx_pitch(N, cpass_cols(N, (int)sizeof(C)));
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     const long wnf = (long)KXP * N * N;
     // register budget: about 8 (fp64) / 16 (fp32) warps per SM for HD, half of that for MHD / Boussinesq
     constexpr int THREADS = xg_rows<N>() * XSched<N>::TPR;
@@ -222,22 +223,22 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_mid_x_n(cons
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_y_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int KXP = kx_pitch(N, TC);
+    constexpr int TC = job_cols(N), EW = 16 / (int)sizeof(C);   // element columns per tile, columns per element
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     JobFwdY<T, N, TC> job;
     job.buf = (C *)r.zbuf;
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.kxp = KXP;
     job.nfields = 3 * NV + NS;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / TC), (unsigned)N), 2);
+    return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 2);
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int KXP = kx_pitch(N, TC);
+    constexpr int TC = cpass_cols(N, (int)sizeof(C)), EW = 1;   // single columns in both precisions
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     JobFwdZ<T, N, TC, NV, NS> job;
     job.sdst = (C *)r.sdst;
     job.saux = (const C *)r.ssrc;
@@ -257,7 +258,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(cons
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.ldk = a.ldk;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC - 1) / TC)), 3);
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC * EW - 1) / (TC * EW))), 3);
 }
 
 #define PSFFT_RHS_LAUNCHER(name)                                                                       \
