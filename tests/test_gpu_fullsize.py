@@ -158,3 +158,51 @@ def test_config5_mhd_rhs_1024_fp32():
     s = np.sqrt(dot(u, u) * dot(Ru, Ru)) + np.sqrt(dot(b, b) * dot(Rb, Rb))
     assert abs(dot(u, Ru) + dot(b, Rb)) / s < 1e-5
     assert abs(dot(b, Ru) + dot(u, Rb)) / s < 1e-5
+
+
+# ---- the NEXT rows at the bench size: Boussinesq RHS and the Runge-Kutta step, 512^3 fp64 -----------------
+
+def inside_small_mask_compare(G, N, g, n):
+    """P12 for results that legitimately extend beyond the small grid's truncation sphere (a second RK stage
+    multiplies fields that already reach 2 kcut): compare G/N^3 with g/n^3 on the modes the SMALL grid retains
+    (9 |k|^2 < n^2), where both grids are alias-free.  Returns the relative L2 error over those modes."""
+    K = (n - 1) // 3
+    idxN = np.r_[0:K + 1, N - K:N]
+    idxn = np.r_[0:K + 1, n - K:n]
+    big = G[:, idxN][:, :, idxN][:, :, :, :K + 1].astype(np.complex128) / float(N) ** 3
+    small = g[:, idxn][:, :, idxn][:, :, :, :K + 1] / float(n) ** 3
+    m = oracle.dealias_mask(n)[idxn][:, idxn][:, :, :K + 1]
+    w = np.full(K + 1, 2.0)
+    w[0] = 1.0
+    num = np.sum(w * m * np.abs(big - small) ** 2)
+    den = np.sum(w * m * np.abs(small) ** 2)
+    return float(np.sqrt(num / den))
+
+
+def test_boussinesq_rhs_512_fp64():
+    N = 512
+    uh = synth.solenoidal_spectrum(N, 4.0, 32, 1234)
+    th = synth.scalar_spectrum(N, 4.0, 32, 1234)
+    p = psfft.Plan(N, torch.float64, 1, work="boussinesq")
+    ru, rt = p.boussinesq_rhs(torch.from_numpy(uh).cuda(), torch.from_numpy(th).cuda(), 1e-3, 2e-3, 1.5)
+    ru, rt = ru.cpu().numpy(), rt.cpu().numpy()
+    gu, gt = oracle.boussinesq_rhs(synth.solenoidal_spectrum(256, 4.0, 32, 1234), synth.scalar_spectrum(256, 4.0, 32, 1234),
+                                   1e-3, 2e-3, 1.5)
+    assert box_compare(ru, N, gu, 256, 64) < 1e-12
+    assert box_compare(rt[None], N, gt[None], 256, 64) < 1e-12
+    M = oracle.dealias_mask(N)
+    assert np.all(ru[:, ~M] == 0) and np.all(rt[~M] == 0)
+
+
+def test_rk2_step_512_fp64():
+    """bench.py's hd_rk2_step: two fused stages; dt large enough that the second stage matters."""
+    N, dt, nu = 512, 0.05, 1e-3
+    uh = synth.solenoidal_spectrum(N, 4.0, 32, 1234)
+    p = psfft.Plan(N, torch.float64, 1)
+    got = p.rk_step(psfft.SYS_HD, torch.from_numpy(uh).cuda(), 2, dt, nu).cpu().numpy()
+    g = oracle.rk_step(0, synth.solenoidal_spectrum(256, 4.0, 32, 1234), 2, dt, nu)
+    assert inside_small_mask_compare(got, N, g, 256) < 1e-12
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+    assert rel(got, uh) > 1e-2                                           # the step moved the state
+    # the second stage produced modes beyond 2 kcut = 64 (they exist on this grid, not on the 256^3 one)
+    assert np.abs(got[:, :8, :8, 70:120]).max() > 0.0
