@@ -3,10 +3,8 @@
 #pragma once
 #include "psfft_kernels.cuh"
 #include "psfft_rhs.cuh"
-#include "psfft_cpipe.cuh"
 #include "psfft_midxg.cuh"
 #include "psfft_launch.cuh"
-#include <stdlib.h>
 
 namespace psfft {
 
@@ -72,53 +70,12 @@ static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *ou
     return cudaGetLastError();
 }
 
-template <typename T, int N, int DIR, int TC, int TPF, int NBUF>
-static cudaError_t cpass_pipe_v(const PassArgs &a, int axis, const void *in, void *out, int fields)
-{
-    using C = Cx<T>;
-    constexpr bool PAD = (TC * sizeof(C) < 128);
-    constexpr size_t smem = (size_t)NBUF * ColMap<N, TC, PAD>::size * sizeof(C);
-    auto kern = k_cpass_pipe<T, N, DIR, TC, TPF, NBUF>;
-    cudaError_t e = set_smem(kern, smem);
-    if (e != cudaSuccess) return e;
-    const long plane = (long)a.ldk * N;
-    long axis_stride, inner, outer_stride, outer;
-    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)N * fields; }
-    else { axis_stride = plane; inner = plane; outer_stride = plane * N; outer = fields; }
-    const long ntx = (inner + TC - 1) / TC, ntiles = ntx * outer;
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-    const int per_sm = (int)(227 * 1024 / (smem + 1024));
-    const long grid = ntiles < (long)sms * per_sm ? ntiles : (long)sms * per_sm;
-    kern<<<(unsigned)grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)a.twN, axis_stride, inner,
-                                                        outer_stride, (int)ntx, ntiles);
-    return cudaGetLastError();
-}
-
 template <typename T, int N, int DIR>
 static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
     using C = Cx<T>;
     constexpr int TC = cpass_cols(N, (int)sizeof(C));
     constexpr int TPF = cpass_tpf(N);
-#ifdef PSFFT_EXPERIMENT
-    if constexpr (N == 512 && sizeof(T) == 8) {
-        static const int v = getenv("PSFFT_CPASS_VARIANT") ? atoi(getenv("PSFFT_CPASS_VARIANT")) : 0;
-        const int vv = axis == 1 ? v % 10 : v / 10;   // units digit: y-pass, tens digit: z-pass
-        switch (vv) {
-            case 1: return cpass_v<T, N, DIR, 8, 64, 2>(a, axis, in, out, fields);
-            case 2: return cpass_v<T, N, DIR, 8, 32, 1>(a, axis, in, out, fields);
-            case 3: return cpass_v<T, N, DIR, 4, 32, 1>(a, axis, in, out, fields);
-            case 4: return cpass_v<T, N, DIR, 16, 32, 1>(a, axis, in, out, fields);
-            case 5: return cpass_v<T, N, DIR, 2, 64, 1>(a, axis, in, out, fields);
-            case 6: return cpass_v<T, N, DIR, 8, 64, 1>(a, axis, in, out, fields);
-            case 7: return cpass_pipe_v<T, N, DIR, 8, 64, 2>(a, axis, in, out, fields);
-            case 8: return cpass_pipe_v<T, N, DIR, 8, 64, 3>(a, axis, in, out, fields);
-            case 9: return cpass_pipe_v<T, N, DIR, 8, 32, 3>(a, axis, in, out, fields);
-            default: break;
-        }
-    }
-#endif
     return cpass_v<T, N, DIR, TC, TPF, 2>(a, axis, in, out, fields);
 }
 
@@ -147,16 +104,9 @@ __host__ __device__ constexpr int job_tpf(int N, int TC)
 }
 
 template <typename T, int N, int DIR, class Job>
-static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid, int id = 0)
+static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid)
 {
     constexpr int TC = cpass_cols(N, (int)sizeof(typename Job::Elem));
-#ifdef PSFFT_EXPERIMENT
-    if constexpr (N == 512 && sizeof(T) == 8) {
-        static const int v = getenv("PSFFT_JOB_VARIANT") ? atoi(getenv("PSFFT_JOB_VARIANT")) : 0;
-        if ((v >> id) & 1) return run_job_v<T, N, DIR, cpass_tpf(N), 2>(a, job, grid);
-    }
-#endif
-    (void)id;
     return run_job_v<T, N, DIR, job_tpf(N, TC), 2>(a, job, grid);
 }
 
@@ -173,7 +123,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_z_n(cons
     job.nf = job.plane * N;
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 0);
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N));
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_y_n(const PassArgs &a, const RhsArgs &r)
@@ -187,7 +137,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_y_n(cons
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.kxp = KXP;
-    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 1);
+    return run_job<T, N, +1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N));
 }
 
 template <typename T, int N, int NV, int NS, int MINB>
@@ -231,7 +181,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_y_n(cons
     job.wnf = job.wplane * N;
     job.kxp = KXP;
     job.nfields = 3 * NV + NS;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N), 2);
+    return run_job<T, N, -1>(a, job, dim3((unsigned)(KXP / (TC * EW)), (unsigned)N));
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
@@ -258,7 +208,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(cons
     job.wplane = (long)KXP * N;
     job.wnf = job.wplane * N;
     job.ldk = a.ldk;
-    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC * EW - 1) / (TC * EW))), 3);
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC * EW - 1) / (TC * EW))));
 }
 
 #define PSFFT_RHS_LAUNCHER(name)                                                                       \
