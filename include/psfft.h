@@ -71,6 +71,7 @@ typedef struct psfft_layout {
     size_t work_bytes_hd;        /* workspace for psfft_hd_rhs */
     size_t work_bytes_mhd;       /* workspace for psfft_mhd_rhs */
     size_t work_bytes_boussinesq; /* workspace for psfft_boussinesq_rhs */
+    int Ny, Nz;                  /* grid points along y, z (= N except for psfft_plan_create3 plans) */
 } psfft_layout;
 
 /* Sizes for a prospective plan.  Supported N: 2^a * 3^b with b <= 1 and 8 <= N <= 1024
@@ -84,6 +85,16 @@ int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out);
  * the plan. */
 int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tables,
                       size_t table_bytes, void *stream);
+
+/* Anisotropic grids ("we also update the formulation ... to accommodate anisotropic grids";
+ * its largest runs are 1024 x 1024 x 256 and 2048 x 2048 x 512): a plan for an Nx x Ny x Nz grid,
+ * each size from the supported list.  Real field [b][z][y][x] (Nx contiguous), half spectrum [b][kz][ky][kx]
+ * with ldk = Nx/2 + 1; psfft_fft3d_r2c / c2r work as above (inverse scaled by 1/(Nx Ny Nz)).  The right-hand-side
+ * and Runge-Kutta calls need a cubic plan and return PSFFT_E_SIZE otherwise (the work_bytes_* of the RHS are 0
+ * in the layout of a non-cubic plan).  layout.N is Nx. */
+int psfft_plan_query3(int Nx, int Ny, int Nz, int dtype, int batch, psfft_layout *out);
+int psfft_plan_create3(psfft_plan *plan, int Nx, int Ny, int Nz, int dtype, int batch, void *d_tables,
+                       size_t table_bytes, void *stream);
 
 /* Free host-side state (PAPER.md:187 clean-up).  Never touches caller memory. */
 int psfft_plan_destroy(psfft_plan plan);

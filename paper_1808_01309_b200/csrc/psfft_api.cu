@@ -31,20 +31,21 @@ int xsched_stages(int N, int *radix)
     return n;
 }
 
-size_t table_entries(int N, size_t *off_twN, size_t *off_twM, size_t *off_twX)
+TableOffsets table_entries(int Nx, int Ny, int Nz)
 {
     auto up = [](size_t n) { return (n + 15) / 16 * 16; };
-    const size_t a = up((size_t)N);
-    const size_t b = a + up((size_t)tw_size(N));
-    const size_t c = b + up((size_t)tw_size(N / 2));
-    if (off_twN) *off_twN = a;
-    if (off_twM) *off_twM = b;
-    if (off_twX) *off_twX = c;
+    TableOffsets o;
+    o.y = up((size_t)Nx);
+    o.m = o.y + up((size_t)tw_size(Ny));
+    o.x = o.m + up((size_t)tw_size(Nx / 2));
     int radix[8];
-    const int S = xsched_stages(N, radix);
+    const int S = xsched_stages(Nx, radix);
     size_t x = 0, Ns = radix[0];
     for (int s = 1; s < S; ++s) { x += (size_t)(radix[s] - 1) * Ns; Ns *= radix[s]; }
-    return c + up(x);
+    const size_t end_x = o.x + up(x);
+    o.z = Nz == Ny ? o.y : end_x;
+    o.total = Nz == Ny ? end_x : end_x + up((size_t)tw_size(Nz));
+    return o;
 }
 }  // namespace psfft
 
@@ -113,23 +114,26 @@ bool supported_n(int N)
     return false;
 }
 
-int fill_layout(int N, int dtype, int batch, psfft_layout *o)
+int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
 {
     if (!o) return PSFFT_E_NULL;
     if (dtype != PSFFT_F32 && dtype != PSFFT_F64) return PSFFT_E_DTYPE;
-    if (!supported_n(N) || batch < 1) return PSFFT_E_SIZE;
+    if (!supported_n(N) || !supported_n(Ny) || !supported_n(Nz) || batch < 1) return PSFFT_E_SIZE;
     const size_t s = dtype == PSFFT_F64 ? 8 : 4;
     memset(o, 0, sizeof(*o));
     o->N = N;
+    o->Ny = Ny;
+    o->Nz = Nz;
     o->dtype = dtype;
     o->batch = batch;
     o->ldk = N / 2 + 1;
-    o->real_elems = (size_t)N * N * N;
-    o->spec_elems = (size_t)o->ldk * N * N;
+    o->real_elems = (size_t)N * Ny * Nz;
+    o->spec_elems = (size_t)o->ldk * Ny * Nz;
     o->real_bytes = o->real_elems * s;
     o->spec_bytes = o->spec_elems * 2 * s;
-    o->table_bytes = table_entries(N, nullptr, nullptr, nullptr) * 2 * s;
+    o->table_bytes = table_entries(N, Ny, Nz).total * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
+    if (Ny != N || Nz != N) return PSFFT_OK;   // anisotropic plans: transforms only (no RHS workspace)
     // fused path: 5 + 6 compact fields [N][N][kx_pitch] per vector field; unfused path: 12 C per vector field
     const size_t wfield = (size_t)N * N * rhs_pitch(N, (int)(2 * s)) * 2 * s;
     o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
@@ -138,6 +142,7 @@ int fill_layout(int N, int dtype, int batch, psfft_layout *o)
     return PSFFT_OK;
 }
 
+inline bool cubic(const psfft_layout &l) { return l.Ny == l.N && l.Nz == l.N; }
 inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 Plan *get(psfft_plan p)
@@ -150,13 +155,15 @@ PassArgs args_of(const Plan *pl, void *stream)
 {
     PassArgs a;
     const size_t cs = pl->lay.dtype == PSFFT_F64 ? 16 : 8;
-    size_t oN, oM, oX;
-    table_entries(pl->lay.N, &oN, &oM, &oX);
+    const TableOffsets o = table_entries(pl->lay.N, pl->lay.Ny, pl->lay.Nz);
     a.tab = pl->d_tab;
-    a.twN = static_cast<const char *>(pl->d_tab) + oN * cs;
-    a.twM = static_cast<const char *>(pl->d_tab) + oM * cs;
-    a.twX = static_cast<const char *>(pl->d_tab) + oX * cs;
+    a.twN = a.twY = static_cast<const char *>(pl->d_tab) + o.y * cs;
+    a.twM = static_cast<const char *>(pl->d_tab) + o.m * cs;
+    a.twX = static_cast<const char *>(pl->d_tab) + o.x * cs;
+    a.twZ = static_cast<const char *>(pl->d_tab) + o.z * cs;
     a.N = pl->lay.N;
+    a.Ny = pl->lay.Ny;
+    a.Nz = pl->lay.Nz;
     a.ldk = pl->lay.ldk;
     a.stream = reinterpret_cast<cudaStream_t>(stream);
     return a;
@@ -174,7 +181,7 @@ inline const char *off(const void *p, size_t bytes) { return static_cast<const c
 // ---- transforms ----------------------------------------------------------------------------
 template <typename T> int r2c_fields(Plan *pl, const PassArgs &a, const void *d_real, void *d_spec, int fields)
 {
-    const long nrows = (long)fields * a.N * a.N;
+    const long nrows = (long)fields * a.Ny * a.Nz;
     const double C = (double)pl->lay.spec_bytes * fields, R = (double)pl->lay.real_bytes * fields;
     { ProfScope ps(pl, a.stream, K_XR2C, R + C); CU(launch_xpass_r2c<T>(a, d_real, d_spec, nrows, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass<T>(a, -1, 1, d_spec, d_spec, fields, &pl->launches)); }
@@ -186,8 +193,8 @@ template <typename T> int r2c_fields(Plan *pl, const PassArgs &a, const void *d_
 template <typename T> int c2r_fields_inplace(Plan *pl, const PassArgs &a, const void *d_spec_in, void *d_spec_work,
                                              void *d_real, int fields)
 {
-    const long nrows = (long)fields * a.N * a.N;
-    const double scale = 1.0 / ((double)a.N * a.N * a.N);
+    const long nrows = (long)fields * a.Ny * a.Nz;
+    const double scale = 1.0 / ((double)a.N * a.Ny * a.Nz);
     const double C = (double)pl->lay.spec_bytes * fields, R = (double)pl->lay.real_bytes * fields;
     { ProfScope ps(pl, a.stream, K_CPZ, 2 * C); CU(launch_cpass<T>(a, +1, 2, d_spec_in, d_spec_work, fields, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass<T>(a, +1, 1, d_spec_work, d_spec_work, fields, &pl->launches)); }
@@ -282,14 +289,25 @@ int mhd_rhs_t(Plan *pl, const PassArgs &a, const void *uhat, const void *bhat, v
 // ================================================================================================
 extern "C" {
 
-int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out) { return fill_layout(N, dtype, batch, out); }
+int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out) { return fill_layout(N, N, N, dtype, batch, out); }
+
+int psfft_plan_query3(int Nx, int Ny, int Nz, int dtype, int batch, psfft_layout *out)
+{
+    return fill_layout(Nx, Ny, Nz, dtype, batch, out);
+}
 
 int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tables, size_t table_bytes, void *stream)
+{
+    return psfft_plan_create3(plan, N, N, N, dtype, batch, d_tables, table_bytes, stream);
+}
+
+int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int batch, void *d_tables, size_t table_bytes,
+                       void *stream)
 {
     if (!plan) return PSFFT_E_NULL;
     *plan = nullptr;
     psfft_layout lay;
-    int rc = fill_layout(N, dtype, batch, &lay);
+    int rc = fill_layout(N, Ny, Nz, dtype, batch, &lay);
     if (rc) return rc;
     if (!d_tables) return PSFFT_E_NULL;
     if (misaligned(d_tables)) return PSFFT_E_ALIGN;
@@ -298,8 +316,8 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
     // Every entry is exp(-2 pi i m / n) from the reduced integer m, evaluated in long double and
     // rounded once to the plan dtype.  [base: n = N, m = 0..N-1][stage tables, L = N][L = N/2].
     std::vector<unsigned char> host(lay.table_bytes);
-    size_t off_twN, off_twM, off_twX;
-    table_entries(N, &off_twN, &off_twM, &off_twX);
+    const TableOffsets toff = table_entries(N, Ny, Nz);
+    const size_t off_twN = toff.y, off_twM = toff.m, off_twX = toff.x;
     auto put = [&](size_t idx, long m, long n) {
         m %= n;
         const long double two_pi = 6.283185307179586476925286766559005768L;
@@ -329,8 +347,9 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
             Ns *= R;
         }
     };
-    stage_tables(off_twN, N);
+    stage_tables(off_twN, Ny);
     stage_tables(off_twM, N / 2);
+    if (Nz != Ny) stage_tables(toff.z, Nz);
     {   // symmetric schedule of the mid_x transforms: stage s >= 1 with earlier radix product Ns, [r-1][k]
         int radix[8];
         const int S = xsched_stages(N, radix);
@@ -425,6 +444,7 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
+    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_uhat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     pl->launches = 0;
@@ -443,6 +463,7 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
+    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_uhat || !d_bhat || !d_rhs_u || !d_rhs_b || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_bhat) || misaligned(d_rhs_u) || misaligned(d_rhs_b) || misaligned(d_work))
         return PSFFT_E_ALIGN;
@@ -484,6 +505,7 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
+    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_uhat || !d_thhat || !d_rhs_u || !d_rhs_th || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_thhat) || misaligned(d_rhs_u) || misaligned(d_rhs_th) || misaligned(d_work))
         return PSFFT_E_ALIGN;
@@ -497,7 +519,7 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
 size_t psfft_rk_work_bytes(psfft_plan plan, int system)
 {
     Plan *pl = get(plan);
-    if (!pl || system < 0 || system > 2) return 0;
+    if (!pl || system < 0 || system > 2 || !cubic(pl->lay)) return 0;
     const size_t rhs = system == PSFFT_SYS_HD ? pl->lay.work_bytes_hd
                      : system == PSFFT_SYS_MHD ? pl->lay.work_bytes_mhd : pl->lay.work_bytes_boussinesq;
     const size_t nfields = system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : 4;
@@ -509,6 +531,7 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
+    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_y_in || !d_y_out || !d_work || !params) return PSFFT_E_NULL;
     if (system < 0 || system > 2 || ord < 1 || ord > 4 || d_y_in == d_y_out) return PSFFT_E_SIZE;
     if (misaligned(d_y_in) || misaligned(d_y_out) || misaligned(d_work)) return PSFFT_E_ALIGN;

@@ -20,7 +20,10 @@ struct PassArgs {
     const void *twN;   // per-stage twiddle tables of the length-N transforms (y, z passes)
     const void *twM;   // per-stage twiddle tables of the length-N/2 transforms (x passes)
     const void *twX;   // per-stage twiddle tables of the length-N transforms in the symmetric schedule (mid_x)
-    int N;
+    int N;             // grid points along x (and along y, z for the cubic plans every RHS call needs)
+    int Ny, Nz;        // grid points along y, z (psfft_plan_create3: anisotropic grids, transforms only)
+    const void *twY;   // per-stage tables of the length-Ny / length-Nz column transforms (= twN when cubic)
+    const void *twZ;
     int ldk;
     cudaStream_t stream;
 };
@@ -59,8 +62,10 @@ template <typename T> cudaError_t launch_rhs_mid_x(const PassArgs &a, const RhsA
 template <typename T> cudaError_t launch_rhs_fwd_y(const PassArgs &a, const RhsArgs &r, int *launches);
 template <typename T> cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches);
 
-// complex entries of the four tables (base, twN, twM, twX) for grid size N
-size_t table_entries(int N, size_t *off_twN, size_t *off_twM, size_t *off_twX);
+// complex entries of the tables of an (Nx, Ny, Nz) plan: [roots of unity, Nx][stage tables Ny][stage tables
+// Nx/2][symmetric-schedule stage tables Nx][stage tables Nz, only when Nz != Ny]
+struct TableOffsets { size_t y, m, x, z, total; };
+TableOffsets table_entries(int Nx, int Ny, int Nz);
 // symmetric radix schedule of the mid_x transforms (psfft_midxg.cuh): fills radix[], returns the stage count
 int xsched_stages(int N, int *radix);
 

@@ -60,13 +60,14 @@ static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *ou
     auto kern = k_cpass<T, N, DIR, TC, TPF, MINB>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    const long plane = (long)a.ldk * N;
+    // N is the length of the transformed axis: Ny for the y-pass, Nz for the z-pass
+    const long plane = (long)a.ldk * a.Ny;
     long axis_stride, inner, outer_stride, outer;
-    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)N * fields; }
-    else { axis_stride = plane; inner = plane; outer_stride = plane * N; outer = fields; }
+    if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)a.Nz * fields; }
+    else { axis_stride = plane; inner = plane; outer_stride = plane * a.Nz; outer = fields; }
     dim3 grid((unsigned)((inner + TC - 1) / TC), (unsigned)outer);
-    kern<<<grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)a.twN, axis_stride, inner,
-                                              outer_stride);
+    kern<<<grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)(axis == 1 ? a.twY : a.twZ),
+                                              axis_stride, inner, outer_stride);
     return cudaGetLastError();
 }
 
@@ -259,7 +260,7 @@ template <typename T>
 cudaError_t launch_cpass(const PassArgs &a, int dir, int axis, const void *in, void *out, int fields, int *launches)
 {
     ++*launches;
-    switch (a.N) {
+    switch (axis == 1 ? a.Ny : a.Nz) {
 #define X(n) case n: return dir < 0 ? cpass_n<T, n, -1>(a, axis, in, out, fields) : cpass_n<T, n, +1>(a, axis, in, out, fields);
         PSFFT_FOR_EACH_N(X)
 #undef X

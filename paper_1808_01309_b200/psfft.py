@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 
 EXPORTS = [
-    "psfft_plan_query", "psfft_plan_create", "psfft_plan_destroy", "psfft_plan_layout",
+    "psfft_plan_query", "psfft_plan_create", "psfft_plan_query3", "psfft_plan_create3", "psfft_plan_destroy",
+    "psfft_plan_layout",
     "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs",
     "psfft_rk_work_bytes", "psfft_rk_step",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
@@ -38,7 +39,7 @@ class Layout(ctypes.Structure):
                 ("real_bytes", ctypes.c_size_t), ("spec_bytes", ctypes.c_size_t),
                 ("table_bytes", ctypes.c_size_t), ("work_bytes_fft", ctypes.c_size_t),
                 ("work_bytes_hd", ctypes.c_size_t), ("work_bytes_mhd", ctypes.c_size_t),
-                ("work_bytes_boussinesq", ctypes.c_size_t)]
+                ("work_bytes_boussinesq", ctypes.c_size_t), ("Ny", ctypes.c_int), ("Nz", ctypes.c_int)]
 
 
 _lib = None
@@ -55,6 +56,8 @@ def lib() -> ctypes.CDLL:
         vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
         L.psfft_plan_query.argtypes = [ci, ci, ci, ctypes.POINTER(Layout)]
         L.psfft_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, vp, sz, vp]
+        L.psfft_plan_query3.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(Layout)]
+        L.psfft_plan_create3.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, vp, sz, vp]
         L.psfft_plan_destroy.argtypes = [vp]
         L.psfft_plan_layout.argtypes = [vp, ctypes.POINTER(Layout)]
         L.psfft_fft3d_r2c.argtypes = [vp, vp, vp, vp, vp]
@@ -124,6 +127,19 @@ def plan_create(N: int, dtype: int, batch: int, d_tables, table_bytes: int, stre
     h = ctypes.c_void_p()
     _check(lib().psfft_plan_create(ctypes.byref(h), N, dtype, batch, _ptr(d_tables), table_bytes, _stream(stream)),
            "psfft_plan_create")
+    return h.value
+
+
+def plan_query3(Nx: int, Ny: int, Nz: int, dtype: int, batch: int = 1) -> Layout:
+    lay = Layout()
+    _check(lib().psfft_plan_query3(Nx, Ny, Nz, dtype, batch, ctypes.byref(lay)), "psfft_plan_query3")
+    return lay
+
+
+def plan_create3(Nx: int, Ny: int, Nz: int, dtype: int, batch: int, d_tables, table_bytes: int, stream=None) -> int:
+    h = ctypes.c_void_p()
+    _check(lib().psfft_plan_create3(ctypes.byref(h), Nx, Ny, Nz, dtype, batch, _ptr(d_tables), table_bytes,
+                                    _stream(stream)), "psfft_plan_create3")
     return h.value
 
 
@@ -239,11 +255,13 @@ class Plan:
         self.rdtype = dtype
         self.cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
         code = F64 if dtype == torch.float64 else F32
-        self.layout = plan_query(N, code, batch)
-        self.N, self.batch, self.ldk = N, batch, self.layout.ldk
+        # N: one size (cubic grid) or (Nx, Ny, Nz) for an anisotropic grid (transforms only)
+        Nx, Ny, Nz = (N, N, N) if isinstance(N, int) else tuple(N)
+        self.layout = plan_query3(Nx, Ny, Nz, code, batch)
+        self.N, self.Ny, self.Nz, self.batch, self.ldk = Nx, Ny, Nz, batch, self.layout.ldk
         with torch.cuda.device(self.device):
             self.tables = torch.empty(self.layout.table_bytes, dtype=torch.uint8, device=self.device)
-            self.handle = plan_create(N, code, batch, self.tables, self.layout.table_bytes)
+            self.handle = plan_create3(Nx, Ny, Nz, code, batch, self.tables, self.layout.table_bytes)
         self._work = None
         self._work_kind = None
         self.ensure_work(work)
@@ -271,11 +289,11 @@ class Plan:
             pass
 
     def spec_shape(self, fields: int):
-        return (fields, self.N, self.N, self.ldk)
+        return (fields, self.Nz, self.Ny, self.ldk)
 
     def r2c(self, real: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         assert real.is_cuda and real.dtype == self.rdtype and real.is_contiguous()
-        assert real.numel() == self.batch * self.N ** 3
+        assert real.numel() == self.batch * self.layout.real_elems
         if out is None:
             out = torch.empty(self.spec_shape(self.batch), dtype=self.cdtype, device=self.device)
         fft3d_r2c(self.handle, real, out, self.ensure_work("fft"))
@@ -285,7 +303,7 @@ class Plan:
         assert spec.is_cuda and spec.dtype == self.cdtype and spec.is_contiguous()
         assert spec.numel() == self.batch * self.layout.spec_elems
         if out is None:
-            out = torch.empty((self.batch, self.N, self.N, self.N), dtype=self.rdtype, device=self.device)
+            out = torch.empty((self.batch, self.Nz, self.Ny, self.N), dtype=self.rdtype, device=self.device)
         fft3d_c2r(self.handle, spec, out, self.ensure_work("fft"))
         return out
 

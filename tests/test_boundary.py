@@ -80,3 +80,17 @@ def test_product_never_imports_the_oracle():
     osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "psfft_oracle.c")).read()
     assert not re.search(r"^\s*(import|from)\s+paper_1808_01309_b200", osrc, flags=re.M)
     assert "psfft.h" not in osrc and "csrc" not in osrc.replace("paper_1808_01309_b200/csrc/", "")
+
+
+def test_plan_query3_anisotropic_sizes(lib):
+    """Anisotropic plans (PAPER.md:370 runs 1024 x 1024 x 256): sizes per axis, no RHS workspace."""
+    lay = psfft.plan_query3(1024, 1024, 256, psfft.F32, 1)
+    assert (lay.N, lay.Ny, lay.Nz, lay.ldk) == (1024, 1024, 256, 513)
+    assert lay.real_elems == 1024 * 1024 * 256 and lay.spec_elems == 513 * 1024 * 256
+    assert lay.work_bytes_fft == lay.spec_bytes and lay.work_bytes_hd == 0 and lay.work_bytes_boussinesq == 0
+    cub = psfft.plan_query3(512, 512, 512, psfft.F64, 3)
+    ref = psfft.plan_query(512, psfft.F64, 3)
+    assert (cub.table_bytes, cub.work_bytes_hd, cub.Ny, cub.Nz) == (ref.table_bytes, ref.work_bytes_hd, 512, 512)
+    assert psfft.plan_query3(64, 64, 16, psfft.F64, 1).table_bytes > psfft.plan_query3(64, 64, 64, psfft.F64, 1).table_bytes - 16 * 64
+    bad = psfft.Layout()
+    assert lib.psfft_plan_query3(512, 500, 512, psfft.F64, 1, ctypes.byref(bad)) == -2

@@ -77,6 +77,37 @@ def test_config1_roundtrip_32(dtype):
     assert rel(back, x) < TOL[dtype]
 
 
+# ---- anisotropic grids (transforms) ---------------------------
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("shape", [(32, 16, 8), (8, 24, 48), (64, 64, 16), (48, 32, 32), (128, 96, 24), (16, 128, 64)])
+def test_anisotropic_r2c_c2r_match_oracle(shape, dtype):
+    """(Nx, Ny, Nz) all different, incl. radix-3 sizes and the paper's flat-box aspect ratio (4:4:1)."""
+    Nx, Ny, Nz = shape
+    x = synth.uniform01(77, np.arange(Nz * Ny * Nx, dtype=np.uint64)).reshape(1, Nz, Ny, Nx) * 2 - 1
+    x = x.astype(RDT[dtype])
+    p = psfft.Plan(shape, dtype, 1)
+    assert (p.layout.N, p.layout.Ny, p.layout.Nz, p.layout.ldk) == (Nx, Ny, Nz, Nx // 2 + 1)
+    X = p.r2c(dev(x))
+    assert tuple(X.shape) == (1, Nz, Ny, Nx // 2 + 1)
+    Xo = oracle.r2c3d(x[0].astype(np.float64))
+    assert rel(X.cpu().numpy()[0], Xo) < TOL[dtype]
+    back = p.c2r(X).cpu().numpy()
+    assert rel(back, x) < TOL[dtype]
+    rng = np.random.default_rng(5)
+    Y = (rng.standard_normal(Xo.shape) + 1j * rng.standard_normal(Xo.shape)).astype(CDT[dtype])   # non-Hermitian input
+    y = p.c2r(dev(Y[None])).cpu().numpy()[0]
+    assert rel(y, oracle.c2r3d(Y.astype(np.complex128), Nx)) < TOL[dtype]
+
+
+def test_anisotropic_plan_rejects_the_right_hand_sides():
+    p = psfft.Plan((32, 32, 16), torch.float64, 1)
+    assert p.layout.work_bytes_hd == 0 and psfft.rk_work_bytes(p.handle, psfft.SYS_HD) == 0
+    u = torch.zeros((3, 16, 32, 17), dtype=torch.complex128, device="cuda")
+    with pytest.raises(psfft.PsfftError):
+        psfft.hd_rhs(p.handle, u, torch.empty_like(u), 0.0, u)
+
+
 def test_degenerate_inputs():
     N = 16
     p = psfft.Plan(N, torch.float64, 1)
