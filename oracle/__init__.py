@@ -206,3 +206,14 @@ def rk_step(sys: int, y, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0, 
     _load().orc_rk_step(ctypes.c_int(N), ctypes.c_int(sys), ctypes.c_int(ord), ctypes.c_double(dt), par, _p(y),
                         _p(out))
     return out
+
+
+def gpe_rhs(psihat, alpha: float, beta: float) -> np.ndarray:
+    """O10: right-hand side of the Gross-Pitaevskii equation (Eq. 7) for psi = p + i q carried as
+    the two real fields (p, q): psihat, result = [2][kz][ky][kx]; alpha = hbar/(2m), beta = g/hbar."""
+    y = _c128(psihat)
+    N = y.shape[-2]
+    assert y.shape == (2, N, N, N // 2 + 1)
+    out = np.empty_like(y)
+    _load().orc_gpe_rhs(ctypes.c_int(N), _p(y), ctypes.c_double(alpha), ctypes.c_double(beta), _p(out))
+    return out

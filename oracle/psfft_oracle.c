@@ -606,3 +606,53 @@ void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cp
     free(ym);
     free(r);
 }
+
+/* ---------------------------------------------------------------------------------------
+ * O10 gpe_rhs: the Gross-Pitaevskii equation, Eq. 7,
+ *         i hbar d_t psi = -hbar^2/(2m) Lap psi + g |psi|^2 psi
+ *     <=> d_t psi = i alpha Lap psi - i beta |psi|^2 psi,   alpha = hbar/(2m), beta = g/hbar.
+ *     The paper counts GPE as "1 complex (or 2 real)" primitive fields: psi = p + i q with
+ *     p, q REAL fields carried as two half spectra, like every other field of the framework:
+ *         d_t p = -alpha Lap q + beta (p^2 + q^2) q,      d_t q = alpha Lap p - beta (p^2 + q^2) p.
+ *     Step by step (nonlinear term in physical space; 2/3-rule mask as for the other
+ *     solvers, reading G23):
+ *       1. pm = M p^, qm = M q^
+ *       2. p, q = c2r3d(pm), c2r3d(qm)                        (2 inverse transforms)
+ *       3. a = (p^2 + q^2) q,  b = (p^2 + q^2) p              (pointwise)
+ *       4. a^ = M r2c3d(a),  b^ = M r2c3d(b)                  (2 forward transforms)
+ *       5. R_p = beta a^ + alpha |k|^2 qm,   R_q = -beta b^ - alpha |k|^2 pm
+ *     psihat, rhs: [2][kz][ky][kx] = (p^, q^); values = N^3 x Fourier coefficient.
+ * ------------------------------------------------------------------------------------- */
+void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs)
+{
+    int H = N / 2 + 1;
+    long nf = (long)N * N * H, nr = (long)N * N * N;
+    cplx *pm = (cplx *)malloc(sizeof(cplx) * 2 * nf);
+    double *p = (double *)malloc(sizeof(double) * 2 * nr);
+    double *a = (double *)malloc(sizeof(double) * 2 * nr);
+    memcpy(pm, psihat, sizeof(cplx) * 2 * nf);
+    orc_apply_mask(N, 2, pm);                                            /* 1 */
+    for (int c = 0; c < 2; ++c) orc_c2r3d(N, N, N, pm + c * nf, p + c * nr);   /* 2 */
+#pragma omp parallel for schedule(static)                                /* 3 */
+    for (long i = 0; i < nr; ++i) {
+        double rho = p[i] * p[i] + p[nr + i] * p[nr + i];
+        a[i] = rho * p[nr + i];
+        a[nr + i] = rho * p[i];
+    }
+    free(p);
+    for (int c = 0; c < 2; ++c) orc_r2c3d(N, N, N, a + c * nr, rhs + c * nf); /* 4 */
+    free(a);
+    orc_apply_mask(N, 2, rhs);
+#pragma omp parallel for schedule(static)                                /* 5 */
+    for (int r = 0; r < N; ++r)
+        for (int q = 0; q < N; ++q)
+            for (int x = 0; x < H; ++x) {
+                long o = ((long)r * N + q) * H + x;
+                double kx = x, ky = wavenumber(q, N), kz = wavenumber(r, N);
+                double k2 = kx * kx + ky * ky + kz * kz;
+                cplx ra = rhs[o], rb = rhs[nf + o];
+                rhs[o] = beta * ra + alpha * k2 * pm[nf + o];
+                rhs[nf + o] = -beta * rb - alpha * k2 * pm[o];
+            }
+    free(pm);
+}
