@@ -72,6 +72,7 @@ typedef struct psfft_layout {
     size_t work_bytes_mhd;       /* workspace for psfft_mhd_rhs */
     size_t work_bytes_boussinesq; /* workspace for psfft_boussinesq_rhs */
     int Ny, Nz;                  /* grid points along y, z (= N except for psfft_plan_create3 plans) */
+    size_t work_bytes_gpe;       /* workspace for psfft_gpe_rhs */
 } psfft_layout;
 
 /* Sizes for a prospective plan.  Supported N: 2^a * 3^b with b <= 1 and 8 <= N <= 1024
@@ -153,6 +154,19 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
                          void *d_rhs_th, double nu, double kappa, double nbv, void *d_work,
                          void *stream);
 
+/* Right-hand side of the Gross-Pitaevskii equation (Eq. 7),
+ *     i hbar d_t psi = -hbar^2/(2m) Lap psi + g |psi|^2 psi   <=>   d_t psi = i alpha Lap psi - i beta |psi|^2 psi,
+ * alpha = hbar/(2m), beta = g/hbar, for psi = p + i q carried as the two REAL fields p, q ("1 complex (or 2 real)"
+ * primitive fields):
+ *     rhs_p = beta M F[(p^2 + q^2) q] + alpha |k|^2 M q^,     rhs_q = -beta M F[(p^2 + q^2) p] - alpha |k|^2 M p^
+ * with p, q = F^-1 of (M p^, M q^): 2 inverse + 2 forward transforms.  In the x pass the packed row P^ + i Q^
+ * inverse-transforms to psi itself, so one complex transform per row and direction does both fields.
+ *   d_psihat  in   2 spectral fields (p^, q^)      d_rhs  out  2 spectral fields
+ *   d_work         >= work_bytes_gpe
+ * psfft_rk_step takes PSFFT_SYS_GPE with params = { alpha, beta, - }. */
+int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alpha, double beta, void *d_work,
+                  void *stream);
+
 /* One explicit Runge-Kutta time step around a right-hand side above ("the system of ODEs
  * is solved using an explicit Runge-Kutta scheme (of 2nd-4th order)"; the paper does not print the
  * scheme -- DESIGN.md reading G21: the low-storage form with `ord` stages
@@ -169,6 +183,7 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
 #define PSFFT_SYS_HD 0
 #define PSFFT_SYS_MHD 1
 #define PSFFT_SYS_BOUSSINESQ 2
+#define PSFFT_SYS_GPE 3          /* y = (p^, q^): 2 fields; params = { alpha, beta, unused } */
 size_t psfft_rk_work_bytes(psfft_plan plan, int system);
 int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out, int ord, double dt,
                   const double *params, void *d_work, void *stream);

@@ -200,7 +200,7 @@ def rk_step(sys: int, y, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0, 
     fields; c2 = eta), 2 = Boussinesq (u^, theta^: 4 fields; c2 = kappa)."""
     y = _c128(y)
     N = y.shape[-2]
-    assert y.shape == ({0: 3, 1: 6, 2: 4}[sys], N, N, N // 2 + 1)
+    assert y.shape == ({0: 3, 1: 6, 2: 4, 3: 2}[sys], N, N, N // 2 + 1)   # sys 3 = GPE: nu = alpha, c2 = beta
     out = np.empty_like(y)
     par = (ctypes.c_double * 3)(nu, c2, nbv)
     _load().orc_rk_step(ctypes.c_int(N), ctypes.c_int(sys), ctypes.c_int(ord), ctypes.c_double(dt), par, _p(y),

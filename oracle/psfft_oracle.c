@@ -579,20 +579,22 @@ void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, d
  *         y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0)
  *     (R = O6 / O7 / O8, M = the 2/3 mask).  For a linear R = L y this is the degree-`ord` Taylor
  *     polynomial of exp(dt L), i.e. order `ord`; for the nonlinear terms it is second order.
- *     sys: 0 = HD (y = u^, 3 fields), 1 = MHD (y = u^, b^: 6 fields), 2 = Boussinesq (y = u^, theta^: 4).
- *     par = { nu, eta (MHD) or kappa (Boussinesq), N_bv }.
+ *     sys: 0 = HD (y = u^, 3 fields), 1 = MHD (y = u^, b^: 6 fields), 2 = Boussinesq (y = u^, theta^: 4),
+ *     3 = GPE (y = p^, q^: 2 fields).  par = { nu, eta (MHD) or kappa (Boussinesq), N_bv }; GPE: { alpha, beta }.
  * ------------------------------------------------------------------------------------- */
+void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs);   /* O10, below */
 static void rk_rhs(int N, int sys, const double *par, const cplx *y, cplx *r)
 {
     long nf = (long)N * N * (N / 2 + 1);
     if (sys == 0) orc_hd_rhs(N, y, par[0], r);
     else if (sys == 1) orc_mhd_rhs(N, y, y + 3 * nf, par[0], par[1], r, r + 3 * nf);
+    else if (sys == 3) orc_gpe_rhs(N, y, par[0], par[1], r);
     else orc_boussinesq_rhs(N, y, y + 3 * nf, par[0], par[1], par[2], r, r + 3 * nf);
 }
 
 void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cplx *y0, cplx *y1)
 {
-    int nfields = sys == 0 ? 3 : sys == 1 ? 6 : 4;
+    int nfields = sys == 0 ? 3 : sys == 1 ? 6 : sys == 3 ? 2 : 4;
     long nf = (long)N * N * (N / 2 + 1), n = nfields * nf;
     cplx *ym = (cplx *)malloc(sizeof(cplx) * n);   /* M y_n */
     cplx *r = (cplx *)malloc(sizeof(cplx) * n);

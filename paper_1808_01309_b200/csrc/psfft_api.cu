@@ -139,6 +139,7 @@ int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
     o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
     o->work_bytes_mhd = 2 * o->work_bytes_hd;
     o->work_bytes_boussinesq = 16 * wfield;   // 5 + 2 z-fields, 6 + 3 y-fields
+    o->work_bytes_gpe = 4 * wfield;           // 2 z/y-fields, 2 x-out fields
     return PSFFT_OK;
 }
 
@@ -245,6 +246,29 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     { ProfScope ps(pl, a.stream, K_MIDX, yf * rows + ff * rows); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_FWDY, ff * rows + ff * disc); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (double)C + (nepi + nbase) * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
+    return PSFFT_OK;
+}
+
+// ---- Gross-Pitaevskii right-hand side (five passes, psfft_rhs.cuh / psfft_midxg.cuh) -----------------
+template <typename T>
+int gpe_t(Plan *pl, const PassArgs &a, const void *psi, void *rhs, double alpha, double beta, const void *base,
+          double cstep, void *work)
+{
+    const size_t C = pl->lay.spec_bytes;
+    const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
+    const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
+    GpeArgs g;
+    g.psi = psi; g.dst = rhs; g.base = base;
+    g.alpha = alpha; g.beta = beta; g.cstep = cstep;
+    g.zbuf = work;
+    g.obuf = off(work, 2 * W);
+    const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
+    const double nepi = (alpha != 0.0 ? 2.0 : 0.0) + (base ? 2.0 : 0.0);
+    { ProfScope ps(pl, a.stream, K_INVZ, 2 * sph + 2 * disc); CU(launch_gpe_pass<T>(a, g, 0, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_INVY, 2 * disc + 2 * rows); CU(launch_gpe_pass<T>(a, g, 1, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_MIDX, 2 * rows + 2 * rows); CU(launch_gpe_pass<T>(a, g, 2, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDY, 2 * rows + 2 * disc); CU(launch_gpe_pass<T>(a, g, 3, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, 2 * disc + 2 * (double)C + nepi * sph); CU(launch_gpe_pass<T>(a, g, 4, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -516,14 +540,30 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
     return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
 }
 
+int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alpha, double beta, void *d_work,
+                  void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!cubic(pl->lay)) return PSFFT_E_SIZE;
+    if (!d_psihat || !d_rhs || !d_work) return PSFFT_E_NULL;
+    if (misaligned(d_psihat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? gpe_t<double>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, d_work)
+                                      : gpe_t<float>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, d_work);
+}
+
+static int sys_fields(int system) { return system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : system == PSFFT_SYS_GPE ? 2 : 4; }
+
 size_t psfft_rk_work_bytes(psfft_plan plan, int system)
 {
     Plan *pl = get(plan);
-    if (!pl || system < 0 || system > 2 || !cubic(pl->lay)) return 0;
+    if (!pl || system < 0 || system > 3 || !cubic(pl->lay)) return 0;
     const size_t rhs = system == PSFFT_SYS_HD ? pl->lay.work_bytes_hd
-                     : system == PSFFT_SYS_MHD ? pl->lay.work_bytes_mhd : pl->lay.work_bytes_boussinesq;
-    const size_t nfields = system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : 4;
-    return nfields * pl->lay.spec_bytes + rhs;
+                     : system == PSFFT_SYS_MHD ? pl->lay.work_bytes_mhd
+                     : system == PSFFT_SYS_GPE ? pl->lay.work_bytes_gpe : pl->lay.work_bytes_boussinesq;
+    return (size_t)sys_fields(system) * pl->lay.spec_bytes + rhs;
 }
 
 int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out, int ord, double dt,
@@ -533,18 +573,27 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
     if (!pl) return PSFFT_E_PLAN;
     if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_y_in || !d_y_out || !d_work || !params) return PSFFT_E_NULL;
-    if (system < 0 || system > 2 || ord < 1 || ord > 4 || d_y_in == d_y_out) return PSFFT_E_SIZE;
+    if (system < 0 || system > 3 || ord < 1 || ord > 4 || d_y_in == d_y_out) return PSFFT_E_SIZE;
     if (misaligned(d_y_in) || misaligned(d_y_out) || misaligned(d_work)) return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     const size_t C = pl->lay.spec_bytes;
-    const int nfields = system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : 4;
+    const int nfields = sys_fields(system);
     void *stage = d_work;                                  // one state-sized stage buffer
     void *rhswork = off(d_work, (size_t)nfields * C);
     const void *cur = d_y_in;
     for (int j = 1; j <= ord; ++j) {
         // stage outputs alternate between the stage buffer and d_y_out so that the last one lands in d_y_out
         void *out = ((ord - j) % 2 == 0) ? d_y_out : stage;
+        if (system == PSFFT_SYS_GPE) {   // params = { alpha, beta }
+            const double cstep = dt / (double)(ord - j + 1);
+            const int rc = pl->lay.dtype == PSFFT_F64
+                               ? gpe_t<double>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, rhswork)
+                               : gpe_t<float>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, rhswork);
+            if (rc) return rc;
+            cur = out;
+            continue;
+        }
         RhsSys y;
         y.nv = system == PSFFT_SYS_MHD ? 2 : 1;
         y.ns = system == PSFFT_SYS_BOUSSINESQ ? 1 : 0;

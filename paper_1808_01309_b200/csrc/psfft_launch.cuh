@@ -62,6 +62,18 @@ template <typename T> cudaError_t launch_rhs_mid_x(const PassArgs &a, const RhsA
 template <typename T> cudaError_t launch_rhs_fwd_y(const PassArgs &a, const RhsArgs &r, int *launches);
 template <typename T> cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches);
 
+// Gross-Pitaevskii right-hand side (psi = p + i q as two real fields): pass = 0 inv_z, 1 inv_y, 2 mid_x,
+// 3 fwd_y, 4 fwd_z
+struct GpeArgs {
+    const void *psi;      // p^, q^ (caller layout)
+    void *dst;            // R_p, R_q
+    const void *base;     // Runge-Kutta stage: y_n, or NULL
+    double alpha, beta, cstep;
+    void *zbuf;           // 2 compact fields: inv_z out, inv_y in place
+    void *obuf;           // 2 compact fields: mid_x out, fwd_y in place
+};
+template <typename T> cudaError_t launch_gpe_pass(const PassArgs &a, const GpeArgs &g, int pass, int *launches);
+
 // complex entries of the tables of an (Nx, Ny, Nz) plan: [roots of unity, Nx][stage tables Ny][stage tables
 // Nx/2][symmetric-schedule stage tables Nx][stage tables Nz, only when Nz != Ny]
 struct TableOffsets { size_t y, m, x, z, total; };

@@ -212,6 +212,62 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(cons
     return run_job<T, N, -1>(a, job, dim3((unsigned)((job.plane + TC * EW - 1) / (TC * EW))));
 }
 
+// ---- Gross-Pitaevskii right-hand side ------------------------------------------------------------
+template <typename T, int N> static cudaError_t gpe_pass_n(const PassArgs &a, const GpeArgs &g, int pass)
+{
+    using C = Cx<T>;
+    constexpr int TC = job_cols(N), EW = 16 / (int)sizeof(C);
+    constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
+    const long plane = (long)a.ldk * N, wplane = (long)KXP * N;
+    const dim3 ygrid((unsigned)(KXP / (TC * EW)), (unsigned)N);
+    if (pass == 0) {
+        JobPlainInvZ<T, N, TC, 2> job;
+        job.src = (const C *)g.psi; job.dst = (C *)g.zbuf;
+        job.plane = plane; job.nf = plane * N; job.wplane = wplane; job.wnf = wplane * N;
+        return run_job<T, N, +1>(a, job, ygrid);
+    }
+    if (pass == 1 || pass == 3) {
+        if (pass == 1) {
+            JobPlainInvY<T, N, TC> job;
+            job.buf = (C *)g.zbuf; job.wplane = wplane; job.wnf = wplane * N; job.kxp = KXP; job.nfields = 2;
+            return run_job<T, N, +1>(a, job, ygrid);
+        }
+        JobFwdY<T, N, TC> job;
+        job.buf = (C *)g.obuf; job.wplane = wplane; job.wnf = wplane * N; job.kxp = KXP; job.nfields = 2;
+        return run_job<T, N, -1>(a, job, ygrid);
+    }
+    if (pass == 2) {
+        using PX = XPad<N, (int)sizeof(C)>;
+        constexpr int ROWS = xg_rows<N>(), THREADS = ROWS * XSched<N>::TPR;
+        constexpr int M0 = (sizeof(T) == 8 ? 512 : 1024) / THREADS;
+        constexpr int MINB = M0 < 1 ? 1 : M0;
+        constexpr size_t smem = (size_t)ROWS * 2 * PX::BUF * sizeof(C);
+        auto kern = k_mid_x_gpe<T, N, MINB>;
+        cudaError_t e = set_smem(kern, smem);
+        if (e != cudaSuccess) return e;
+        kern<<<(unsigned)(N * N / ROWS), THREADS, smem, a.stream>>>((const C *)g.zbuf, (C *)g.obuf, (const C *)a.twX,
+                                                                     wplane * N, KXP, (T)(1.0 / ((double)N * N * N)));
+        return cudaGetLastError();
+    }
+    constexpr int TCZ = cpass_cols(N, (int)sizeof(C));
+    JobGpeFwdZ<T, N, TCZ> job;
+    job.src = (const C *)g.obuf; job.dst = (C *)g.dst; job.psi = (const C *)g.psi; job.base = (const C *)g.base;
+    job.alpha = (T)g.alpha; job.beta = (T)g.beta; job.cstep = (T)g.cstep;
+    job.plane = plane; job.nf = plane * N; job.wplane = wplane; job.wnf = wplane * N; job.ldk = a.ldk;
+    return run_job<T, N, -1>(a, job, dim3((unsigned)((plane + TCZ - 1) / TCZ)));
+}
+
+template <typename T> cudaError_t launch_gpe_pass(const PassArgs &a, const GpeArgs &g, int pass, int *launches)
+{
+    ++*launches;
+    switch (a.N) {
+#define X(n) case n: return gpe_pass_n<T, n>(a, g, pass);
+        PSFFT_FOR_EACH_N(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
 #define PSFFT_RHS_LAUNCHER(name)                                                                       \
     template <typename T> cudaError_t launch_rhs_##name(const PassArgs &a, const RhsArgs &r, int *launches) \
     {                                                                                                  \
@@ -322,6 +378,7 @@ cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void
     template cudaError_t launch_rhs_inv_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
     template cudaError_t launch_rhs_mid_x<T>(const PassArgs &, const RhsArgs &, int *);                               \
     template cudaError_t launch_rhs_fwd_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
+    template cudaError_t launch_gpe_pass<T>(const PassArgs &, const GpeArgs &, int, int *);                            \
     template cudaError_t launch_rhs_fwd_z<T>(const PassArgs &, const RhsArgs &, int *);
 
 }  // namespace psfft

@@ -390,4 +390,106 @@ __global__ void __launch_bounds__(xg_rows<N>() * XSched<N>::TPR, MINB)
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// mid_x of the Gross-Pitaevskii equation (Eq. 7): psi = p + i q.  The packed row
+// Z = P^ + i Q^ inverse-transforms to psi itself (ONE complex length-N transform per row), the cubic term
+// rho = |psi|^2, F = rho q + i rho p is formed in registers, and one forward transform + split gives
+// a^ = F[rho q], b^ = F[rho p] for kx < N/3.   in: 2 compact fields (P, Q rows);  out: 2 compact fields.
+// ------------------------------------------------------------------------------------------
+template <typename T, int N, int MINB>
+__global__ void __launch_bounds__(xg_rows<N>() * XSched<N>::TPR, MINB)
+    k_mid_x_gpe(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ twx, long nfw, int kxp,
+                T scale1)
+{
+    using C = Cx<T>;
+    using X = XSched<N>;
+    using P = XPad<N, (int)sizeof(C)>;
+    constexpr int RM = X::RM, TPR = X::TPR, S = X::S, BUF = P::BUF, KX = kx_count(N);
+    constexpr int ND = (KX + TPR - 1) / TPR;
+    extern __shared__ __align__(16) unsigned char smraw[];
+
+    const int g = threadIdx.x / TPR, b = threadIdx.x % TPR;
+    C *sm = reinterpret_cast<C *>(smraw) + g * (2 * BUF);   // buffer 0: the transform, buffer 1: split exchange
+    const long rowoff = ((long)blockIdx.x * xg_rows<N>() + g) * kxp;
+    const C zero = mk<T>(0, 0);
+
+    // ---- inverse, first stage (same classes of r as k_mid_xg) ----
+    C z[RM];
+    {
+        const C *f = in + rowoff;
+#pragma unroll
+        for (int r = 0; r < RM; ++r) {
+            const int e = b + TPR * r;
+            const bool dc = TPR * r < KX, mc = TPR * r + TPR - 1 > N - KX;
+            const int k = dc ? e : N - e;
+            C pa = zero, qa = zero;
+            if ((dc || mc) && k < KX) { pa = ld_stream(f + k); qa = ld_stream(f + nfw + k); }
+            if (dc) {
+                if (r == 0 && b == 0) { pa.y = (T)0; qa.y = (T)0; }
+                z[r] = mk<T>(pa.x - qa.y, pa.y + qa.x);        // P + i Q
+            } else if (mc) {
+                z[r] = mk<T>(pa.x + qa.y, qa.x - pa.y);        // conj P + i conj Q
+            } else {
+                z[r] = zero;
+            }
+        }
+        bfly<RM, +1, T>(z);
+#pragma unroll
+        for (int r = 0; r < RM; ++r) sm[P::pad(RM * b + r)] = z[r];
+    }
+    __syncthreads();
+    xg_middle_stages<T, N, 1, +1, 1>(sm, twx, b);
+    {
+        const C *ts = twx + X::tw_off(S - 1) + b;
+#pragma unroll
+        for (int r = 0; r < RM; ++r) z[r] = sm[P::pad(b + TPR * r)];
+        twiddle_r<RM, +1, T>(z, ts, TPR);
+        bfly<RM, +1, T>(z);
+    }
+    // ---- cubic term at x = b + TPR r: psi = scale1 z;  F = |psi|^2 (q + i p) ----
+    C F[RM];
+#pragma unroll
+    for (int r = 0; r < RM; ++r) {
+        const T pr = z[r].x * scale1, qr = z[r].y * scale1;
+        const T rho = pr * pr + qr * qr;
+        F[r] = mk<T>(rho * qr, rho * pr);
+    }
+    bfly<RM, -1, T>(F);
+#pragma unroll
+    for (int r = 0; r < RM; ++r) sm[P::pad(b + TPR * r)] = F[r];
+    __syncthreads();
+    xg_middle_stages<T, N, 1, -1, 1>(sm, twx, b);
+    {
+        const C *ts = twx + X::tw_off(S - 1) + b;
+#pragma unroll
+        for (int r = 0; r < RM; ++r) {
+            const int e = b + TPR * r;
+            F[r] = sm[P::pad(S == 2 ? e / RM + TPR * (e % RM) : e)];
+        }
+        twiddle_r<RM, -1, T>(F, ts, TPR);
+        bfly<RM, -1, T>(F);
+    }
+    // ---- split: a^[k] = (F[k] + conj F[N-k])/2, b^[k] = -i (F[k] - conj F[N-k])/2 ----
+    C *ex = sm + BUF;
+#pragma unroll
+    for (int e = 0; e < ND; ++e) ex[e * TPR + b] = F[RM - ND + e];
+    __syncthreads();
+    const int bp = (TPR - b) % TPR;
+    C *o = out + rowoff;
+#pragma unroll
+    for (int r = 0; r < ND; ++r) {
+        const int k = b + TPR * r;
+        if (k < KX) {
+            const int e = (b == 0) ? (r == 0 ? 0 : ND - r) : ND - 1 - r;
+            C c = ex[e * TPR + bp];
+            if (b == 0 && r == 0) c = F[0];
+            const C a = F[r];
+            const C sa = mk<T>((T)0.5 * (a.x + c.x), (T)0.5 * (a.y - c.y));
+            const C d = mk<T>((T)0.5 * (a.x - c.x), (T)0.5 * (a.y + c.y));
+            st_stream(o + k, sa);
+            st_stream(o + nfw + k, mk<T>(d.y, -d.x));
+        }
+    }
+}
+
 }  // namespace psfft

@@ -512,4 +512,133 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     }
 };
 
+// ------------------------------------------------------------------------------------------
+// Gross-Pitaevskii equation (Eq. 7), psi = p + i q as two real fields: plain masked
+// inverse z / y passes of NF fields, and the fwd_z epilogue R_p = beta a^ + alpha |k|^2 q^,
+// R_q = -beta b^ - alpha |k|^2 p^ (a = |psi|^2 q, b = |psi|^2 p from mid_x).
+// ------------------------------------------------------------------------------------------
+template <typename T, int N, int TC, int NF> struct JobPlainInvZ : JobElems<JobPlainInvZ<T, N, TC, NF>, Cx<T>, Ex<T>> {
+    using C = Cx<T>;
+    const C *src;       // NF spectral fields, caller layout
+    C *dst;             // NF compact fields
+    long plane, nf, wplane, wnf;
+    struct State { long col, wcol; int kxy2; bool active; };
+    __device__ __forceinline__ int rounds() const { return NF; }
+    __device__ __forceinline__ bool begin(State &s, long colidx) const
+    {
+        const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, N);
+        s.kxy2 = kx * kx + ky * ky;
+        s.active = 9 * s.kxy2 < N * N;
+        s.col = (long)blockIdx.y * (plane / N) + kx;
+        s.wcol = (long)blockIdx.y * (wplane / N) + kx;
+        return s.active;
+    }
+    __device__ __forceinline__ void idle(const State &, int, int) const {}
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        const int kz = wavenumber(i, N);
+        C x = mk<T>(0, 0);
+        if (s.active && 9 * (s.kxy2 + kz * kz) < N * N) x = ldg_c(src + r * nf + i * plane + s.col);
+        return x;
+    }
+    __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (s.active) st_stream(dst + r * wnf + i * wplane + s.wcol, v);
+    }
+    __device__ __forceinline__ void store_e(const State *s, int r, int i, float2x2 v) const
+    {
+        st_stream2(dst + r * wnf + i * wplane + s[0].wcol, v, s[0].active, s[1].active);
+    }
+    __device__ __forceinline__ void store_e(const State *s, int r, int i, double2 v) const { store(s[0], r, i, v); }
+};
+
+// in place on NF compact fields; reads only the retained (ky, kx), writes every ky of the retained kx
+template <typename T, int N, int TC> struct JobPlainInvY : JobElems<JobPlainInvY<T, N, TC>, Cx<T>, Ex<T>> {
+    using C = Cx<T>;
+    C *buf;
+    long wplane, wnf;
+    int kxp, nfields;
+    struct State { long base; int kx; bool active; };
+    __device__ __forceinline__ int rounds() const { return nfields; }
+    __device__ __forceinline__ bool begin(State &s, long colidx) const
+    {
+        s.kx = (int)colidx;
+        s.active = s.kx < kx_count(N);
+        s.base = (long)blockIdx.y * wplane + s.kx;
+        return true;
+    }
+    __device__ __forceinline__ void idle(const State &, int, int) const {}
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        const int ky = wavenumber(i, N);
+        C x = mk<T>(0, 0);
+        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) x = ld_stream(buf + r * wnf + s.base + (long)i * kxp);
+        return x;
+    }
+    __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (s.active) st_stream(buf + r * wnf + s.base + (long)i * kxp, v);
+    }
+};
+
+template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, N, TC>, Cx<T>, Cx<T>> {
+    using C = Cx<T>;
+    const C *src;        // 2 compact fields (after fwd_y): a^, b^
+    C *dst;              // 2 fields, caller layout: R_p, R_q
+    const C *psi;        // p^, q^ (caller layout) for the dispersion term
+    const C *base;       // Runge-Kutta stage: y_n (NULL: plain right-hand side)
+    T alpha, beta, cstep;
+    long plane, nf, wplane, wnf;
+    int ldk;
+    struct State { long col, wcol; int kxy2; bool active, valid; };
+    __device__ __forceinline__ int rounds() const { return 2; }
+    __device__ __forceinline__ bool begin(State &s, long colidx) const
+    {
+        s.col = colidx;
+        s.valid = s.col < plane;
+        s.active = false;
+        s.kxy2 = 0;
+        s.wcol = 0;
+        if (s.valid) {
+            const int kx = (int)(s.col % ldk), q = (int)(s.col / ldk), ky = wavenumber(q, N);
+            s.kxy2 = kx * kx + ky * ky;
+            s.active = 9 * s.kxy2 < N * N;
+            s.wcol = (long)q * (wplane / N) + kx;
+        }
+        return s.active;
+    }
+    __device__ __forceinline__ void idle(const State &s, int t, int nt) const
+    {
+        if (!s.valid) return;
+        for (int r = 0; r < 2; ++r)
+            for (int i = t; i < N; i += nt) st_stream(dst + r * nf + i * plane + s.col, mk<T>(0, 0));
+    }
+    __device__ __forceinline__ C load(const State &s, int r, int i) const
+    {
+        C x = mk<T>(0, 0);
+        if (s.active) x = ld_stream(src + r * wnf + i * wplane + s.wcol);
+        return x;
+    }
+    __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
+    __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
+    {
+        if (!s.valid) return;
+        const int kz = wavenumber(i, N);
+        C *o = dst + r * nf + i * plane + s.col;
+        if (!(s.active && 9 * (s.kxy2 + kz * kz) < N * N)) { *o = mk<T>(0, 0); return; }
+        // r = 0: R_p = beta a^ + alpha |k|^2 q^;   r = 1: R_q = -beta b^ - alpha |k|^2 p^
+        const T sg = r == 0 ? (T)1 : (T)-1;
+        const C other = ldg_c(psi + (1 - r) * nf + i * plane + s.col);
+        const T d = sg * alpha * (T)(s.kxy2 + kz * kz), b = sg * beta;
+        C res = mk<T>(b * v.x + d * other.x, b * v.y + d * other.y);
+        if (base != nullptr) {
+            const C y0 = ldg_c(base + r * nf + i * plane + s.col);
+            res.x = y0.x + cstep * res.x; res.y = y0.y + cstep * res.y;
+        }
+        *o = res;
+    }
+};
+
 }  // namespace psfft

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_query3", "psfft_plan_create3", "psfft_plan_destroy",
     "psfft_plan_layout",
-    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs",
+    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs", "psfft_gpe_rhs",
     "psfft_rk_work_bytes", "psfft_rk_step",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
@@ -39,7 +39,8 @@ class Layout(ctypes.Structure):
                 ("real_bytes", ctypes.c_size_t), ("spec_bytes", ctypes.c_size_t),
                 ("table_bytes", ctypes.c_size_t), ("work_bytes_fft", ctypes.c_size_t),
                 ("work_bytes_hd", ctypes.c_size_t), ("work_bytes_mhd", ctypes.c_size_t),
-                ("work_bytes_boussinesq", ctypes.c_size_t), ("Ny", ctypes.c_int), ("Nz", ctypes.c_int)]
+                ("work_bytes_boussinesq", ctypes.c_size_t), ("Ny", ctypes.c_int), ("Nz", ctypes.c_int),
+                ("work_bytes_gpe", ctypes.c_size_t)]
 
 
 _lib = None
@@ -65,6 +66,7 @@ def lib() -> ctypes.CDLL:
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_boussinesq_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, cd, vp, vp]
+        L.psfft_gpe_rhs.argtypes = [vp, vp, vp, cd, cd, vp, vp]
         L.psfft_rk_work_bytes.argtypes = [vp, ci]
         L.psfft_rk_work_bytes.restype = sz
         L.psfft_rk_step.argtypes = [vp, ci, vp, vp, ci, cd, ctypes.POINTER(cd), vp, vp]
@@ -171,7 +173,12 @@ def boussinesq_rhs(plan: int, d_uhat, d_thhat, d_rhs_u, d_rhs_th, nu: float, kap
                                       float(kappa), float(nbv), _ptr(d_work), _stream(stream)), "psfft_boussinesq_rhs")
 
 
-SYS_HD, SYS_MHD, SYS_BOUSSINESQ = 0, 1, 2
+SYS_HD, SYS_MHD, SYS_BOUSSINESQ, SYS_GPE = 0, 1, 2, 3
+
+
+def gpe_rhs(plan: int, d_psihat, d_rhs, alpha: float, beta: float, d_work, stream=None) -> None:
+    _check(lib().psfft_gpe_rhs(plan, _ptr(d_psihat), _ptr(d_rhs), float(alpha), float(beta), _ptr(d_work),
+                               _stream(stream)), "psfft_gpe_rhs")
 
 
 def rk_work_bytes(plan: int, system: int) -> int:
@@ -271,7 +278,8 @@ class Plan:
                 "mhd": self.layout.work_bytes_mhd, "boussinesq": self.layout.work_bytes_boussinesq,
                 "rk_hd": 3 * self.layout.spec_bytes + self.layout.work_bytes_hd,
                 "rk_mhd": 6 * self.layout.spec_bytes + self.layout.work_bytes_mhd,
-                "rk_boussinesq": 4 * self.layout.spec_bytes + self.layout.work_bytes_boussinesq}[kind]
+                "rk_boussinesq": 4 * self.layout.spec_bytes + self.layout.work_bytes_boussinesq,
+                "gpe": self.layout.work_bytes_gpe, "rk_gpe": 2 * self.layout.spec_bytes + self.layout.work_bytes_gpe}[kind]
         if self._work is None or self._work.numel() < need:
             self._work = None
             self._work = torch.empty(need, dtype=torch.uint8, device=self.device)
@@ -334,11 +342,20 @@ class Plan:
     def rk_step(self, system: int, y: torch.Tensor, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0,
                 nbv: float = 0.0, out: torch.Tensor | None = None) -> torch.Tensor:
         """One Runge-Kutta step; y: [3 | 6 | 4, N, N, N/2+1] complex (HD | MHD u,b | Boussinesq u,theta)."""
-        nf = {SYS_HD: 3, SYS_MHD: 6, SYS_BOUSSINESQ: 4}[system]
+        nf = {SYS_HD: 3, SYS_MHD: 6, SYS_BOUSSINESQ: 4, SYS_GPE: 2}[system]
         assert y.is_cuda and y.dtype == self.cdtype and y.is_contiguous() and tuple(y.shape) == self.spec_shape(nf)
         if out is None:
             out = torch.empty_like(y)
-        work = self.ensure_work({SYS_HD: "rk_hd", SYS_MHD: "rk_mhd", SYS_BOUSSINESQ: "rk_boussinesq"}[system])
+        work = self.ensure_work({SYS_HD: "rk_hd", SYS_MHD: "rk_mhd", SYS_BOUSSINESQ: "rk_boussinesq",
+                                 SYS_GPE: "rk_gpe"}[system])
         assert rk_work_bytes(self.handle, system) <= work.numel()
         rk_step(self.handle, system, y, out, ord, dt, (nu, c2, nbv), work)
+        return out
+
+    def gpe_rhs(self, psihat: torch.Tensor, alpha: float, beta: float) -> torch.Tensor:
+        """psihat: [2, N, N, N/2+1] = (p^, q^) of psi = p + i q."""
+        assert psihat.is_cuda and psihat.dtype == self.cdtype and psihat.is_contiguous()
+        assert tuple(psihat.shape) == self.spec_shape(2)
+        out = torch.empty_like(psihat)
+        gpe_rhs(self.handle, psihat, out, alpha, beta, self.ensure_work("gpe"))
         return out

@@ -305,6 +305,48 @@ def test_rk_step_beltrami_closed_form_and_argument_checks():
         psfft.rk_step(p.handle, psfft.SYS_HD, yd, torch.empty_like(yd), 5, dt, (nu, 0, 0), work)   # ord > 4
 
 
+# ---- Gross-Pitaevskii (Eq. 7; the paper's fourth solver) ----------------------------------------
+
+def gpe_state(N, kcut, dtype):
+    y = np.stack([synth.scalar_spectrum(N, 3.0, kcut, 1234, tag=11), synth.scalar_spectrum(N, 3.0, kcut, 1234, tag=12)])
+    y[0, 0, 0, 0] = float(N) ** 3                                   # condensate: psi = 1 + fluctuations
+    return np.ascontiguousarray(y.astype(CDT[dtype]))
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [16, 24, 32, 48, 64, 96, 128])
+def test_gpe_rhs_matches_oracle(N, dtype):
+    y = gpe_state(N, N // 2 - 1, dtype)                             # kcut above N/3: the input mask acts
+    p = psfft.Plan(N, dtype, 1, work="gpe")
+    yd = dev(y)
+    got = p.gpe_rhs(yd, 0.37, 1.3).cpu().numpy()
+    assert np.array_equal(yd.cpu().numpy(), y)
+    want = oracle.gpe_rhs(y.astype(np.complex128), 0.37, 1.3)
+    assert rel(got, want) < TOL[dtype]
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+
+
+def test_gpe_plane_wave_closed_form():
+    """psi = A exp(i k.x) is an exact solution: rhs = -i (alpha |k|^2 + beta A^2) psi."""
+    N, A, alpha, beta = 32, 0.7, 0.3, 1.1
+    x, y, z = synth.grid_axes(N)
+    psi = A * np.exp(1j * (2 * x + y - 3 * z + 0 * x * y * z))
+    pk = lambda f: np.stack([oracle.r2c3d(np.ascontiguousarray(f.real)), oracle.r2c3d(np.ascontiguousarray(f.imag))])
+    p = psfft.Plan(N, torch.float64, 1, work="gpe")
+    got = p.gpe_rhs(dev(pk(psi)), alpha, beta).cpu().numpy()
+    assert rel(got, pk(-1j * (alpha * 14 + beta * A * A) * psi)) < 1e-13
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,ord", [(16, 1), (32, 2), (48, 3), (64, 4)])
+def test_gpe_rk_step_matches_oracle(N, ord, dtype):
+    y = gpe_state(N, N // 2 - 1, dtype)
+    p = psfft.Plan(N, dtype, 1)
+    got = p.rk_step(psfft.SYS_GPE, dev(y), ord, 0.01, 0.37, 1.3).cpu().numpy()
+    want = oracle.rk_step(3, y.astype(np.complex128), ord, 0.01, 0.37, 1.3)
+    assert rel(got, want) < TOL[dtype]
+
+
 # ---- host-buffer (end-to-end) entry points -----------------------------------------------------------
 
 def test_host_entry_points():

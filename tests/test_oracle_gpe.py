@@ -93,3 +93,15 @@ def test_numpy_restatement_and_mask():
     got = oracle.gpe_rhs(y0, alpha, beta)
     assert rel(got, want) < 1e-13
     assert np.all(got[:, ~M] == 0)
+
+
+def test_rk_step_on_a_plane_wave_is_the_truncated_exponential():
+    """O9 with sys = 3: |psi| stays A along the exact solution, so the RK polynomial of -i omega dt multiplies psi
+    only to first order in the nonlinearity; for beta = 0 (linear) it is exact: psi_1 = P_ord(-i alpha k^2 dt) psi_0."""
+    N, alpha, dt, ord = 16, 0.3, 0.05, 4
+    x, y, z = synth.grid_axes(N)
+    psi = 0.7 * np.exp(1j * (2 * x + y - z + 0 * x * y * z))
+    w = -1j * alpha * 6 * dt
+    poly = 1 + w + w ** 2 / 2 + w ** 3 / 6 + w ** 4 / 24
+    got = oracle.rk_step(3, pack(psi), ord, dt, alpha, 0.0)
+    assert rel(got, pack(poly * psi)) < 1e-14
