@@ -344,16 +344,20 @@ def run_ours(args) -> int:
         bwork = plan.ensure_work("rk_boussinesq")
         f_b = lambda: psfft.boussinesq_rhs(h, uh, th, rhs, rt, 1e-3, 1e-3, 1.0, bwork)
         f_rk = lambda: psfft.rk_step(h, psfft.SYS_HD, uh, rhs, 2, 1e-3, (1e-3, 0.0, 0.0), bwork)
-        for f in (f_b, f_rk):
+        f_g = lambda: psfft.gpe_rhs(h, uh, rhs, 0.3, 1.0, bwork)     # the first two fields as (p^, q^)
+        for f in (f_b, f_rk, f_g):
             for _ in range(3):
                 f()
         torch.cuda.synchronize()
         t_b = time_loop(f_b, K, stream)
         t_rk = time_loop(f_rk, K, stream)
+        t_g = time_loop(f_g, K, stream)
         next_rows = {"boussinesq_rhs": {"ms": t_b, "evals_per_s": 1e3 / t_b,
                                         "workload": f"{N}^3 fp64, u as above + random-phase theta, nu = kappa = 1e-3, N_bv = 1"},
                      "hd_rk2_step": {"ms": t_rk, "steps_per_s": 1e3 / t_rk,
-                                     "workload": f"{N}^3 fp64, two fused RHS stages, nu = 1e-3, dt = 1e-3"}}
+                                     "workload": f"{N}^3 fp64, two fused RHS stages, nu = 1e-3, dt = 1e-3"},
+                     "gpe_rhs": {"ms": t_g, "evals_per_s": 1e3 / t_g,
+                                 "workload": f"{N}^3 fp64, psi = p + i q as two real fields, alpha = 0.3, beta = 1"}}
         del th, rt
 
     if rank != 0:

@@ -206,3 +206,24 @@ def test_rk2_step_512_fp64():
     assert rel(got, uh) > 1e-2                                           # the step moved the state
     # the second stage produced modes beyond 2 kcut = 64 (they exist on this grid, not on the 256^3 one)
     assert np.abs(got[:, :8, :8, 70:120]).max() > 0.0
+
+
+def test_gpe_rhs_512_fp64():
+    """The fourth solver at the bench size: an exact solution (plane wave on a condensate is NOT exact, a single
+    plane wave is) element by element, and a random state against the 256^3 oracle (P12; the cubic term of a
+    field with |k| <= 24 reaches 72 < 85, inside both truncation spheres)."""
+    N, alpha, beta, A = 512, 0.3, 1.1, 0.7
+    p = psfft.Plan(N, torch.float64, 1, work="gpe")
+    y = np.zeros((2, N, N, N // 2 + 1), np.complex128)       # psi = A exp(i (5x - 3y + 2z)):  p^ + i q^ has one mode
+    y[0, 2, N - 3, 5] = 0.5 * A * N**3                        # p = A cos(phase)
+    y[1, 2, N - 3, 5] = -0.5j * A * N**3                      # q = A sin(phase)
+    got = p.gpe_rhs(torch.from_numpy(y).cuda(), alpha, beta).cpu().numpy()
+    om = alpha * 38 + beta * A * A                            # d_t psi = -i om psi:  d_t p = om q, d_t q = -om p
+    want = np.stack([om * y[1], -om * y[0]])
+    assert rel(got, want) < 1e-12
+    assert np.count_nonzero(np.abs(got) > 1e-9 * N**3) == 2
+    y = np.stack([synth.scalar_spectrum(N, 3.0, 24, 1234, tag=11), synth.scalar_spectrum(N, 3.0, 24, 1234, tag=12)])
+    g = np.stack([synth.scalar_spectrum(256, 3.0, 24, 1234, tag=11), synth.scalar_spectrum(256, 3.0, 24, 1234, tag=12)])
+    got = p.gpe_rhs(torch.from_numpy(y).cuda(), alpha, beta).cpu().numpy()
+    assert box_compare(got, N, oracle.gpe_rhs(g, alpha, beta), 256, 72) < 1e-12
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
