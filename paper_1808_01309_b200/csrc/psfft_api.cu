@@ -216,6 +216,7 @@ struct RhsSys {
     // Runge-Kutta stage: outputs are base + cstep * rhs (base_u == NULL: plain right-hand side)
     const void *base_u, *base_b, *base_t;
     double cstep;
+    bool sparse_out;   // intermediate Runge-Kutta stage: zeros outside the sphere are not written
 };
 
 template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys &y, void *work)
@@ -231,6 +232,7 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     r.ssrc = y.thhat; r.sdst = y.rt;
     r.sdiff = y.kappa; r.nbv = y.nbv;
     r.base[0] = y.base_u; r.base[1] = y.base_b; r.sbase = y.base_t; r.cstep = y.cstep;
+    r.sparse_out = y.sparse_out;
     const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
     r.zbuf = work;                                         // 5 nv + 2 ns compact fields (later 3 nv + ns: mid_x out, fwd_y in place)
     r.ybuf = off(work, (size_t)(5 * nv + 2 * ns) * W);     // 6 nv + 3 ns compact fields
@@ -245,21 +247,21 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     { ProfScope ps(pl, a.stream, K_INVY, zf * disc + yf * rows); CU(launch_rhs_inv_y<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_MIDX, yf * rows + ff * rows); CU(launch_rhs_mid_x<T>(a, r, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_FWDY, ff * rows + ff * disc); CU(launch_rhs_fwd_y<T>(a, r, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (double)C + (nepi + nbase) * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, ff * disc + ff * (y.sparse_out ? sph : (double)C) + (nepi + nbase) * sph); CU(launch_rhs_fwd_z<T>(a, r, &pl->launches)); }
     return PSFFT_OK;
 }
 
 // ---- Gross-Pitaevskii right-hand side (five passes, psfft_rhs.cuh / psfft_midxg.cuh) -----------------
 template <typename T>
 int gpe_t(Plan *pl, const PassArgs &a, const void *psi, void *rhs, double alpha, double beta, const void *base,
-          double cstep, void *work)
+          double cstep, bool sparse_out, void *work)
 {
     const size_t C = pl->lay.spec_bytes;
     const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
     const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
     GpeArgs g;
     g.psi = psi; g.dst = rhs; g.base = base;
-    g.alpha = alpha; g.beta = beta; g.cstep = cstep;
+    g.alpha = alpha; g.beta = beta; g.cstep = cstep; g.sparse_out = sparse_out;
     g.zbuf = work;
     g.obuf = off(work, 2 * W);
     const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
@@ -268,7 +270,7 @@ int gpe_t(Plan *pl, const PassArgs &a, const void *psi, void *rhs, double alpha,
     { ProfScope ps(pl, a.stream, K_INVY, 2 * disc + 2 * rows); CU(launch_gpe_pass<T>(a, g, 1, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_MIDX, 2 * rows + 2 * rows); CU(launch_gpe_pass<T>(a, g, 2, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_FWDY, 2 * rows + 2 * disc); CU(launch_gpe_pass<T>(a, g, 3, &pl->launches)); }
-    { ProfScope ps(pl, a.stream, K_FWDZ, 2 * disc + 2 * (double)C + nepi * sph); CU(launch_gpe_pass<T>(a, g, 4, &pl->launches)); }
+    { ProfScope ps(pl, a.stream, K_FWDZ, 2 * disc + 2 * (sparse_out ? sph : (double)C) + nepi * sph); CU(launch_gpe_pass<T>(a, g, 4, &pl->launches)); }
     return PSFFT_OK;
 }
 
@@ -475,7 +477,7 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
     PassArgs a = args_of(pl, stream);
     if (fused) {
         const RhsSys y = {1, 0, d_uhat, nullptr, nullptr, d_rhs, nullptr, nullptr, nu, 0.0, 0.0, 0.0,
-                          nullptr, nullptr, nullptr, 0.0};
+                          nullptr, nullptr, nullptr, 0.0, false};
         return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
     }
     return pl->lay.dtype == PSFFT_F64 ? hd_rhs_t<double>(pl, a, d_uhat, d_rhs, nu, d_work)
@@ -495,7 +497,7 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
     PassArgs a = args_of(pl, stream);
     if (fused) {
         const RhsSys y = {2, 0, d_uhat, d_bhat, nullptr, d_rhs_u, d_rhs_b, nullptr, nu, eta, 0.0, 0.0,
-                          nullptr, nullptr, nullptr, 0.0};
+                          nullptr, nullptr, nullptr, 0.0, false};
         return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
     }
     return pl->lay.dtype == PSFFT_F64 ? mhd_rhs_t<double>(pl, a, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu, eta, d_work)
@@ -536,7 +538,7 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     const RhsSys y = {1, 1, d_uhat, nullptr, d_thhat, d_rhs_u, nullptr, d_rhs_th, nu, 0.0, kappa, nbv,
-                      nullptr, nullptr, nullptr, 0.0};
+                      nullptr, nullptr, nullptr, 0.0, false};
     return pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, d_work) : rhs_fused_t<float>(pl, a, y, d_work);
 }
 
@@ -550,8 +552,8 @@ int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alp
     if (misaligned(d_psihat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
-    return pl->lay.dtype == PSFFT_F64 ? gpe_t<double>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, d_work)
-                                      : gpe_t<float>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, d_work);
+    return pl->lay.dtype == PSFFT_F64 ? gpe_t<double>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, false, d_work)
+                                      : gpe_t<float>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, false, d_work);
 }
 
 static int sys_fields(int system) { return system == PSFFT_SYS_HD ? 3 : system == PSFFT_SYS_MHD ? 6 : system == PSFFT_SYS_GPE ? 2 : 4; }
@@ -588,8 +590,8 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
         if (system == PSFFT_SYS_GPE) {   // params = { alpha, beta }
             const double cstep = dt / (double)(ord - j + 1);
             const int rc = pl->lay.dtype == PSFFT_F64
-                               ? gpe_t<double>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, rhswork)
-                               : gpe_t<float>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, rhswork);
+                               ? gpe_t<double>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, j < ord, rhswork)
+                               : gpe_t<float>(pl, a, cur, out, params[0], params[1], d_y_in, cstep, j < ord, rhswork);
             if (rc) return rc;
             cur = out;
             continue;
@@ -609,6 +611,7 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
         y.kappa = system == PSFFT_SYS_BOUSSINESQ ? params[1] : 0.0;
         y.nbv = system == PSFFT_SYS_BOUSSINESQ ? params[2] : 0.0;
         y.cstep = dt / (double)(ord - j + 1);
+        y.sparse_out = j < ord;   // only the last stage has to define the zeros of d_y_out
         const int rc = pl->lay.dtype == PSFFT_F64 ? rhs_fused_t<double>(pl, a, y, rhswork)
                                                   : rhs_fused_t<float>(pl, a, y, rhswork);
         if (rc) return rc;

@@ -53,6 +53,7 @@ struct RhsArgs {
     const void *base[2];
     const void *sbase;
     double cstep;
+    bool sparse_out;      // intermediate stage: skip the zero fill outside the truncation sphere
     void *zbuf;           // 5 nv + 2 ns compact fields (inv_z out; later mid_x out / fwd_y in place, 3 nv + ns fields)
     void *ybuf;           // 6 nv + 3 ns compact fields (inv_y out)
 };
@@ -69,6 +70,7 @@ struct GpeArgs {
     void *dst;            // R_p, R_q
     const void *base;     // Runge-Kutta stage: y_n, or NULL
     double alpha, beta, cstep;
+    bool sparse_out;
     void *zbuf;           // 2 compact fields: inv_z out, inv_y in place
     void *obuf;           // 2 compact fields: mid_x out, fwd_y in place
 };

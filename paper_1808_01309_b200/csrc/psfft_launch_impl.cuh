@@ -198,6 +198,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(cons
     for (int v = 0; v < NV; ++v) job.base[v] = (const C *)r.base[v];
     job.sbase = (const C *)r.sbase;
     job.cstep = (T)r.cstep;
+    job.sparse = r.sparse_out;
     job.src = (const C *)r.zbuf;
     for (int v = 0; v < NV; ++v) {
         job.dst[v] = (C *)r.dst[v];
@@ -252,7 +253,7 @@ template <typename T, int N> static cudaError_t gpe_pass_n(const PassArgs &a, co
     constexpr int TCZ = cpass_cols(N, (int)sizeof(C));
     JobGpeFwdZ<T, N, TCZ> job;
     job.src = (const C *)g.obuf; job.dst = (C *)g.dst; job.psi = (const C *)g.psi; job.base = (const C *)g.base;
-    job.alpha = (T)g.alpha; job.beta = (T)g.beta; job.cstep = (T)g.cstep;
+    job.alpha = (T)g.alpha; job.beta = (T)g.beta; job.cstep = (T)g.cstep; job.sparse = g.sparse_out;
     job.plane = plane; job.nf = plane * N; job.wplane = wplane; job.wnf = wplane * N; job.ldk = a.ldk;
     return run_job<T, N, -1>(a, job, dim3((unsigned)((plane + TCZ - 1) / TCZ)));
 }

@@ -388,6 +388,8 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     const C *base[NV];   // Runge-Kutta stage: y_n (NULL: plain right-hand side); out = base + cstep * rhs
     const C *sbase;
     T cstep;
+    bool sparse;         // intermediate Runge-Kutta stage: the zeros outside the truncation sphere are not written
+                         // (the next stage masks on load and never reads them)
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
     int ldk;
@@ -417,7 +419,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     // nothing retained in this tile: the output is all zeros (thread t of nt writes rows t, t + nt, ...)
     __device__ __forceinline__ void idle(const State &s, int t, int nt) const
     {
-        if (!s.valid) return;
+        if (!s.valid || sparse) return;
         const C z = mk<T>(0, 0);
         for (int g = 0; g < NV; ++g)
             for (int comp = 0; comp < 3; ++comp)
@@ -442,7 +444,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
         const bool keep = s.active && 9 * (kxy2 + kz * kz) < N * N;
         if (NS > 0 && r == 3 * NV) {   // Eq. 2: R_theta = -s^ + N_bv u^_z - kappa |k|^2 theta^
             C *os = sdst + i * plane + s.col;
-            if (!keep) { *os = mk<T>(0, 0); return; }
+            if (!keep) { if (!sparse) *os = mk<T>(0, 0); return; }
             C rt = mk<T>(-v.x, -v.y);
             if (nbv != (T)0) {
                 const C uz = ldg_c(aux[0] + 2 * nf + i * plane + s.col);
@@ -461,7 +463,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
             return;
         }
         C *o = (g == 0 ? dst[0] : dst[NV - 1]) + i * plane + s.col;
-        if (!keep) { o[comp * nf] = mk<T>(0, 0); return; }
+        if (!keep) { if (!sparse) o[comp * nf] = mk<T>(0, 0); return; }
         if (comp < 2) { o[comp * nf] = v; return; }   // raw; read back here by this same thread (same address: ordered)
         finish(s, g, i, o, __ldcg(o), __ldcg(o + nf), v);
     }
@@ -590,6 +592,7 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
     const C *psi;        // p^, q^ (caller layout) for the dispersion term
     const C *base;       // Runge-Kutta stage: y_n (NULL: plain right-hand side)
     T alpha, beta, cstep;
+    bool sparse;         // as in JobFwdZ
     long plane, nf, wplane, wnf;
     int ldk;
     struct State { long col, wcol; int kxy2; bool active, valid; };
@@ -611,7 +614,7 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
     }
     __device__ __forceinline__ void idle(const State &s, int t, int nt) const
     {
-        if (!s.valid) return;
+        if (!s.valid || sparse) return;
         for (int r = 0; r < 2; ++r)
             for (int i = t; i < N; i += nt) st_stream(dst + r * nf + i * plane + s.col, mk<T>(0, 0));
     }
@@ -627,7 +630,7 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
         if (!s.valid) return;
         const int kz = wavenumber(i, N);
         C *o = dst + r * nf + i * plane + s.col;
-        if (!(s.active && 9 * (s.kxy2 + kz * kz) < N * N)) { *o = mk<T>(0, 0); return; }
+        if (!(s.active && 9 * (s.kxy2 + kz * kz) < N * N)) { if (!sparse) *o = mk<T>(0, 0); return; }
         // r = 0: R_p = beta a^ + alpha |k|^2 q^;   r = 1: R_q = -beta b^ - alpha |k|^2 p^
         const T sg = r == 0 ? (T)1 : (T)-1;
         const C other = ldg_c(psi + (1 - r) * nf + i * plane + s.col);

@@ -289,6 +289,22 @@ def test_rk_step_matches_oracle(N, ord, system, dtype):
     assert rel(got, y) > 1e-3                                        # the step did something
 
 
+@pytest.mark.parametrize("system", [0, 3])
+def test_rk_intermediate_stages_never_read_outside_the_sphere(system):
+    """Intermediate stages skip the zero fill outside the truncation sphere (the next stage masks on load): poison
+    the workspace and the output with NaN bit patterns first; the result must still match the oracle and be fully
+    defined."""
+    N, ord = 32, 4
+    y = rk_state(system, N, 3.0, N // 2 - 1, torch.float64) if system == 0 else gpe_state(N, N // 2 - 1, torch.float64)
+    p = psfft.Plan(N, torch.float64, 1)
+    p.ensure_work("rk_hd" if system == 0 else "rk_gpe").fill_(0xFF)
+    out = torch.full(y.shape, float("nan"), dtype=torch.complex128, device="cuda")
+    got = p.rk_step(system, dev(y), ord, 0.02, 0.013, 0.5, out=out).cpu().numpy()
+    want = oracle.rk_step(system, y, ord, 0.02, 0.013, 0.5)
+    assert np.isfinite(got).all() and rel(got, want) < 1e-12
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+
+
 def test_rk_step_beltrami_closed_form_and_argument_checks():
     """ABC flow under viscosity: one RK4 step multiplies u^ by 1 + x + x^2/2 + x^3/6 + x^4/24, x = -nu dt."""
     N, nu, dt = 32, 0.7, 0.05
