@@ -109,27 +109,57 @@ __global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
 // z-pass: axis_stride = ldk*N, inner = ldk*N, outer = fields,     outer_stride = ldk*N*N
 // In place (in == out) is allowed: a CTA reads all of its columns before it writes any.
 // ------------------------------------------------------------------------------------------
+// The tile is [N rows] x [TC elements Ex<T>]: one fp64 column or two adjacent fp32 columns per element
+// (packed fp32x2 butterflies, psfft_core.cuh).  vec: every pair of columns is 16-byte aligned (z-pass: the
+// strides are even) so that an fp32 element moves with one 16-byte access; otherwise (y-pass: odd pitch ldk)
+// with two 8-byte ones.
 template <typename T, int N, int DIR, int TC, int TPF, int MINB>
 __global__ void __launch_bounds__(TC *TPF, MINB)
     k_cpass(const Cx<T> *in, Cx<T> *out, const Cx<T> *__restrict__ tw, long axis_stride, long inner,
-            long outer_stride)
+            long outer_stride, bool vec)
 {
     using C = Cx<T>;
-    constexpr bool PAD = (TC * sizeof(C) < 128);
+    using E = Ex<T>;
+    constexpr int EW = ElemWidth<E>::value;
+    constexpr bool PAD = (TC * sizeof(E) < 128);
     using Map = ColMap<N, TC, PAD>;
     extern __shared__ __align__(16) unsigned char smraw[];
-    C *sm = reinterpret_cast<C *>(smraw);
+    E *sm = reinterpret_cast<E *>(smraw);
 
     const int c = threadIdx.x % TC, t = threadIdx.x / TC;
-    const long col = (long)blockIdx.x * TC + c;
-    const bool valid = col < inner;
+    const long col = ((long)blockIdx.x * TC + c) * EW;
+    const bool valid = col < inner, valid1 = col + 1 < inner;   // valid1: second column of an fp32 pair
     const long base = (long)blockIdx.y * outer_stride + (valid ? col : 0);
     const C *src = in + base;
     C *dst = out + base;
 
-    auto ld = [&](int i) -> C { return valid ? ld_stream(src + i * axis_stride) : mk<T>(0, 0); };
-    auto st = [&](int i, C v) {
-        if (valid) st_stream(dst + i * axis_stride, v);
+    auto ld = [&](int i) -> E {
+        if constexpr (EW == 1) {
+            return valid ? ld_stream(src + i * axis_stride) : mk<T>(0, 0);
+        } else {
+            E x = ezero<E>();
+            if (vec && valid1) {
+                const float4 q = __ldcs(reinterpret_cast<const float4 *>(src + i * axis_stride));
+                x.re = make_float2(q.x, q.z);
+                x.im = make_float2(q.y, q.w);
+            } else {
+                if (valid) ecol_set(x, 0, ld_stream(src + i * axis_stride));
+                if (valid1) ecol_set(x, 1, ld_stream(src + i * axis_stride + 1));
+            }
+            return x;
+        }
+    };
+    auto st = [&](int i, E v) {
+        if constexpr (EW == 1) {
+            if (valid) st_stream(dst + i * axis_stride, v);
+        } else {
+            if (vec && valid1) {
+                __stcs(reinterpret_cast<float4 *>(dst + i * axis_stride), make_float4(v.re.x, v.im.x, v.re.y, v.im.y));
+            } else {
+                if (valid) st_stream(dst + i * axis_stride, ecol(v, 0));
+                if (valid1) st_stream(dst + i * axis_stride + 1, ecol(v, 1));
+            }
+        }
     };
     fft_stages<T, N, 1, DIR, TPF, false, false, false, Map>(sm, tw, c, t, ld, st);
 }

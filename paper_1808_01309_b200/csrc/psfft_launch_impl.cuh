@@ -55,8 +55,10 @@ template <typename T, int N, int DIR, int TC, int TPF, int MINB>
 static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
     using C = Cx<T>;
-    constexpr bool PAD = (TC * sizeof(C) < 128);
-    constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(C);
+    using E = Ex<T>;
+    constexpr int EW = ElemWidth<E>::value;
+    constexpr bool PAD = (TC * sizeof(E) < 128);
+    constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(E);
     auto kern = k_cpass<T, N, DIR, TC, TPF, MINB>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
@@ -65,18 +67,27 @@ static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *ou
     long axis_stride, inner, outer_stride, outer;
     if (axis == 1) { axis_stride = a.ldk; inner = a.ldk; outer_stride = plane; outer = (long)a.Nz * fields; }
     else { axis_stride = plane; inner = plane; outer_stride = plane * a.Nz; outer = fields; }
-    dim3 grid((unsigned)((inner + TC - 1) / TC), (unsigned)outer);
+    dim3 grid((unsigned)((inner + TC * EW - 1) / (TC * EW)), (unsigned)outer);
+    // fp32 pairs: 16-byte access when every pair of columns is aligned (even strides; the bases are 16-byte aligned)
+    const bool vec = axis_stride % 2 == 0 && outer_stride % 2 == 0 && inner % 2 == 0;
     kern<<<grid, TC * TPF, smem, a.stream>>>((const C *)in, (C *)out, (const C *)(axis == 1 ? a.twY : a.twZ),
-                                              axis_stride, inner, outer_stride);
+                                              axis_stride, inner, outer_stride, vec);
     return cudaGetLastError();
+}
+
+// Column passes: 8 elements per thread (one radix-8 butterfly per stage) while the CTA stays within
+// 512 threads -- twice the warps of the 16-element shape for the same two tiles per SM (measured, 512^3
+// fp64: inv_y 1.67 -> 1.50 ms, fwd_y 0.85 -> 0.60 ms; profiles/r1b_summary.md)
+__host__ __device__ constexpr int job_tpf(int N, int TC)
+{
+    return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= 512) ? N / 8 : cpass_tpf(N);
 }
 
 template <typename T, int N, int DIR>
 static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
-    using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C));
-    constexpr int TPF = cpass_tpf(N);
+    constexpr int TC = cpass_cols(N, (int)sizeof(Ex<T>));   // 16-byte elements in both precisions
+    constexpr int TPF = job_tpf(N, TC);
     return cpass_v<T, N, DIR, TC, TPF, 2>(a, axis, in, out, fields);
 }
 
@@ -94,14 +105,6 @@ static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
     if (e != cudaSuccess) return e;
     kern<<<grid, TC * TPF, smem, a.stream>>>(job, (const C *)a.twN);
     return cudaGetLastError();
-}
-
-// RHS column passes: 8 elements per thread (one radix-8 butterfly per stage) while the CTA stays within
-// 512 threads -- twice the warps of the 16-element shape for the same two tiles per SM (measured, 512^3
-// fp64: inv_y 1.67 -> 1.50 ms, fwd_y 0.85 -> 0.60 ms; profiles/r1b_summary.md)
-__host__ __device__ constexpr int job_tpf(int N, int TC)
-{
-    return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= 512) ? N / 8 : cpass_tpf(N);
 }
 
 template <typename T, int N, int DIR, class Job>
