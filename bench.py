@@ -327,13 +327,25 @@ def run_ours(args) -> int:
         t_f = dist_max(time_loop(f_fwd, K, stream), dev)
         t_b = dist_max(time_loop(f_bwd, K, stream), dev)
         rt_err = float((y - x).abs().max())
+        # side reference only (north_star: cuFFT "may be timed only as a side reference"; never on the product path)
+        cufft = None
+        try:
+            c_f = lambda: torch.fft.rfftn(x, dim=(1, 2, 3))
+            c_b = lambda: torch.fft.irfftn(X, s=(N, N, N), dim=(1, 2, 3))
+            for _ in range(2):
+                c_f(); c_b()
+            torch.cuda.synchronize()
+            cufft = {"ms_r2c": time_loop(c_f, min(K, 10), stream), "ms_c2r": time_loop(c_b, min(K, 10), stream),
+                     "what": "torch.fft.rfftn / irfftn (cuFFT) on the same tensors, allocation of the result included"}
+        except Exception as exc:     # out of memory on a busy device: the side reference is optional
+            cufft = {"unavailable": str(exc)[:80]}
         fbytes = 3.0 * (plan.layout.real_bytes + 5.0 * spec_bytes)
         fft3d = {"workload": f"{N}^3 fp64 batch 3, uniform [-1,1) seed 1234 (BASELINE.json configs[2])",
                  "ms_r2c": t_f, "ms_c2r": t_b, "ms_r2c_plus_c2r": t_f + t_b, "ms_per_transform_per_field": (t_f + t_b) / 6.0,
                  "algorithmic_bytes_per_direction": fbytes, "GBps_r2c": fbytes / (t_f * 1e-3) / 1e9,
                  "GBps_c2r": fbytes / (t_b * 1e-3) / 1e9, "hbm_frac": 2 * fbytes / ((t_f + t_b) * 1e-3) / 1e9 / peak,
                  "hbm_frac_of_nominal_8TBps": 2 * fbytes / ((t_f + t_b) * 1e-3) / 1e9 / 8000.0,
-                 "roundtrip_max_abs_err": rt_err}
+                 "roundtrip_max_abs_err": rt_err, "side_reference_cufft": cufft}
         del x, X, y
 
     # ---- the rows SURVEY.md §8(f) marks "next", same size, same protocol (device-resident) --------------
