@@ -402,3 +402,64 @@ def test_unfused_rhs_matches_oracle(N, dtype):
     psfft.mhd_rhs_unfused(p.handle, du, db, ru, rb, 0.01, 0.02, p._work)
     wu, wb = oracle.mhd_rhs(uh.astype(np.complex128), bh.astype(np.complex128), 0.01, 0.02)
     assert rel(ru.cpu().numpy(), wu) < TOL[dtype] and rel(rb.cpu().numpy(), wb) < TOL[dtype]
+
+
+# ---- guard bands: no call writes outside the buffers it was given ------------------------------------------
+
+class Arena:
+    """One device allocation carved into 256-byte aligned blocks separated by guard bands of a known pattern."""
+    GUARD = 4096
+
+    def __init__(self, nbytes):
+        self.buf = torch.full((nbytes,), 0xA5, dtype=torch.uint8, device="cuda")
+        self.off = self.GUARD
+        self.blocks = []
+
+    def take(self, nbytes):
+        start = (self.off + 255) // 256 * 256
+        self.off = start + nbytes + self.GUARD
+        assert self.off <= self.buf.numel()
+        self.blocks.append((start, nbytes))
+        return self.buf[start:start + nbytes]
+
+    def guards_intact(self):
+        mask = torch.ones(self.buf.numel(), dtype=torch.bool, device="cuda")
+        for start, n in self.blocks:
+            mask[start:start + n] = False
+        return bool((self.buf[mask] == 0xA5).all())
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [12, 32, 48, 64])
+def test_no_call_writes_outside_its_buffers(N, dtype):
+    code = psfft.F64 if dtype == torch.float64 else psfft.F32
+    lay = psfft.plan_query(N, code, 2)
+    C = lay.spec_bytes
+    work_bytes = max(lay.work_bytes_fft, 6 * C + lay.work_bytes_mhd, 4 * C + lay.work_bytes_boussinesq,
+                     2 * C + lay.work_bytes_gpe)
+    ar = Arena(lay.table_bytes + 2 * lay.real_bytes * 2 + 14 * C + work_bytes + 64 * Arena.GUARD)
+    tables = ar.take(lay.table_bytes)
+    h = psfft.plan_create(N, code, 2, tables, lay.table_bytes)
+    real, real2 = ar.take(2 * lay.real_bytes), ar.take(2 * lay.real_bytes)
+    yin, yout, work = ar.take(6 * C), ar.take(6 * C), ar.take(work_bytes)
+    real.view(dtype).uniform_(-1, 1)
+    kc = N // 2 - 1
+    y = np.concatenate([synth.solenoidal_spectrum(N, 2.0, kc, 3, tag=0), synth.solenoidal_spectrum(N, 2.0, kc, 3, tag=1)])
+    yin.view(torch.complex128 if dtype == torch.float64 else torch.complex64).copy_(
+        torch.from_numpy(y.astype(CDT[dtype])).reshape(-1))
+    u, b = yin[:3 * C], yin[3 * C:]
+    try:
+        psfft.fft3d_r2c(h, real, yout[:2 * C], work)
+        psfft.fft3d_c2r(h, yout[:2 * C], real2, work)
+        psfft.hd_rhs(h, u, yout[:3 * C], 0.1, work)
+        psfft.mhd_rhs(h, u, b, yout[:3 * C], yout[3 * C:], 0.1, 0.1, work)
+        psfft.boussinesq_rhs(h, u, b[:C], yout[:3 * C], yout[3 * C:4 * C], 0.1, 0.1, 1.0, work)
+        psfft.gpe_rhs(h, u[:2 * C], yout[:2 * C], 0.1, 1.0, work)
+        for system, nf in ((0, 3), (1, 6), (2, 4), (3, 2)):
+            psfft.rk_step(h, system, yin[:nf * C], yout[:nf * C], 3, 0.01, (0.1, 0.1, 1.0), work)
+        torch.cuda.synchronize()
+        assert ar.guards_intact()
+        assert np.array_equal(yin.view(torch.complex128 if dtype == torch.float64 else torch.complex64).cpu().numpy(),
+                              y.astype(CDT[dtype]).reshape(-1))                      # inputs untouched by every call
+    finally:
+        psfft.plan_destroy(h)
