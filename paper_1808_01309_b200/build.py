@@ -27,8 +27,19 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _flags() -> str:
+    return " ".join(NVCC_FLAGS[:6] + os.environ.get("PSFFT_NVCC_EXTRA", "").split())
+
+
+def _stamp() -> str:
+    return os.path.join(HERE, "build", "flags.txt")
+
+
 def _stale() -> bool:
     if not os.path.exists(LIB):
+        return True
+    # a library built with other flags (e.g. a size-restricted experimental build) is stale
+    if not os.path.exists(_stamp()) or open(_stamp()).read() != _flags():
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "psfft.h")]
@@ -58,6 +69,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    with open(_stamp(), "w") as f:
+        f.write(_flags())
     return LIB
 
 
