@@ -131,6 +131,9 @@ def test_config4_hd_rhs_768_fp32():
 
 def test_config5_mhd_rhs_1024_fp32():
     N = 1024
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()          # the earlier full-size tests leave their buffers in torch's cache
     free, _ = torch.cuda.mem_get_info()
     lay = psfft.plan_query(N, psfft.F32, 1)
     need = lay.work_bytes_mhd + 12 * lay.spec_bytes
