@@ -36,8 +36,7 @@ TableOffsets table_entries(int Nx, int Ny, int Nz)
     auto up = [](size_t n) { return (n + 15) / 16 * 16; };
     TableOffsets o;
     o.y = up((size_t)Nx);
-    o.m = o.y + up((size_t)tw_size(Ny));
-    o.x = o.m + up((size_t)tw_size(Nx / 2));
+    o.x = o.y + up((size_t)tw_size(Ny));
     int radix[8];
     const int S = xsched_stages(Nx, radix);
     size_t x = 0, Ns = radix[0];
@@ -159,7 +158,6 @@ PassArgs args_of(const Plan *pl, void *stream)
     const TableOffsets o = table_entries(pl->lay.N, pl->lay.Ny, pl->lay.Nz);
     a.tab = pl->d_tab;
     a.twN = a.twY = static_cast<const char *>(pl->d_tab) + o.y * cs;
-    a.twM = static_cast<const char *>(pl->d_tab) + o.m * cs;
     a.twX = static_cast<const char *>(pl->d_tab) + o.x * cs;
     a.twZ = static_cast<const char *>(pl->d_tab) + o.z * cs;
     a.N = pl->lay.N;
@@ -340,10 +338,10 @@ int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int b
     if (table_bytes < lay.table_bytes) return PSFFT_E_TABLE;
 
     // Every entry is exp(-2 pi i m / n) from the reduced integer m, evaluated in long double and
-    // rounded once to the plan dtype.  [base: n = N, m = 0..N-1][stage tables, L = N][L = N/2].
+    // rounded once to the plan dtype.  Layout: table_entries() above.
     std::vector<unsigned char> host(lay.table_bytes);
     const TableOffsets toff = table_entries(N, Ny, Nz);
-    const size_t off_twN = toff.y, off_twM = toff.m, off_twX = toff.x;
+    const size_t off_twN = toff.y, off_twX = toff.x;
     auto put = [&](size_t idx, long m, long n) {
         m %= n;
         const long double two_pi = 6.283185307179586476925286766559005768L;
@@ -374,7 +372,6 @@ int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int b
         }
     };
     stage_tables(off_twN, Ny);
-    stage_tables(off_twM, N / 2);
     if (Nz != Ny) stage_tables(toff.z, Nz);
     {   // symmetric schedule of the mid_x transforms: stage s >= 1 with earlier radix product Ns, [r-1][k]
         int radix[8];

@@ -295,17 +295,11 @@ template <int DIR, typename C> __device__ __forceinline__ C root_of(const C *__r
 //   ColMap : tile [row][TC columns]; thread column c, rows along the FFT axis.
 //            One padding row of TC elements after every 8 rows when a row is 64 B, so that
 //            the two rows of a 128 B wavefront never share banks in the stride-8 writes.
-//   RowMap : one contiguous transform per group, [c][i]; index i padded by i/8 so that
-//            stride-R writes of 16 B (fp64) / 8 B (fp32) elements are conflict-free.
 // ------------------------------------------------------------------------------------------
 template <int L, int TC, bool PAD> struct ColMap {
     static constexpr int rows = PAD ? L + (L >> 3) : L;
     static constexpr int size = rows * TC;
     __device__ __forceinline__ static int at(int i, int c) { return (PAD ? i + (i >> 3) : i) * TC + c; }
-};
-template <int L> struct RowMap {
-    static constexpr int ld = L + (L >> 3) + 1;
-    __device__ __forceinline__ static int at(int i, int c) { return c * ld + i + (i >> 3); }
 };
 
 // ------------------------------------------------------------------------------------------

@@ -2,8 +2,8 @@
 //
 // Pass structure: a 3D transform is three passes, each reading and
 // writing the field exactly once (the minimal-pass count for an out-of-cache 3D FFT):
-//   x-pass  contiguous rows; real <-> half-complex through a half-length complex FFT plus
-//           the split/merge step (PAPER.md:70 step 1, first half)
+//   x-pass  contiguous rows; real <-> half-complex, two rows per complex transform (psfft_xpass2.cuh;
+//           PAPER.md:70 step 1, first half)
 //   y-pass  columns with element stride ldk (PAPER.md:70 step 1, second half)
 //   z-pass  columns with element stride ldk*N (PAPER.md:77 step 3)
 // The paper's transpose (PAPER.md:76 step 2) is not a pass: the y/z kernels read tiles of
@@ -12,94 +12,6 @@
 #include "psfft_core.cuh"
 
 namespace psfft {
-
-// ------------------------------------------------------------------------------------------
-// forward x-pass: N reals -> N/2+1 complex per row  (a1 in SURVEY.md §8)
-//   z[n] = x[2n] + i x[2n+1]  (the row reinterpreted as complex),  Z = FFT_{N/2}(z),
-//   X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) w_N^k (Z[k] - conj Z[M-k]),  k = 0..M,  M = N/2.
-// ------------------------------------------------------------------------------------------
-template <typename T, int N, int ROWS>
-__global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
-    k_xpass_r2c(const T *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ tab,
-                const Cx<T> *__restrict__ tw, long nrows, int ldk)
-{
-    using C = Cx<T>;
-    constexpr int M = N / 2;
-    constexpr int TPF = threads_per_fft(M);
-    constexpr bool WARP = (TPF <= 32) && (32 % TPF == 0);
-    using Map = RowMap<M>;
-    extern __shared__ __align__(16) unsigned char smraw[];
-    C *sm = reinterpret_cast<C *>(smraw);
-
-    const int c = threadIdx.x / TPF, t = threadIdx.x % TPF;
-    long row = (long)blockIdx.x * ROWS + c;
-    const bool valid = row < nrows;
-    if (!valid) row = nrows - 1;  // keep the group in lock step; results discarded
-    const C *src = reinterpret_cast<const C *>(in + row * N);
-    C *dst = out + row * (long)ldk;
-
-    auto ld = [&](int i) -> C { return ld_stream(src + i); };
-    auto st = [&](int, C) {};
-    fft_stages<T, M, 1, -1, TPF, false, true, WARP, Map>(sm, tw, c, t, ld, st);
-
-    if (!valid) return;
-#pragma unroll 2
-    for (int k = t; k <= M / 2; k += TPF) {
-        const C zk = sm[Map::at(k, c)];
-        const C zm = cconj(sm[Map::at((M - k) % M, c)]);
-        const C w = root_of<-1>(tab, k);
-        const C e = cscale(cadd(zk, zm), (T)0.5);
-        const C d = cscale(csub(zk, zm), (T)0.5);
-        const C o = mul_diri<-1>(cmul(w, d));  // -(i/2) w (Z[k] - conj Z[M-k])
-        st_stream(dst + k, cadd(e, o));
-        if (2 * k != M) st_stream(dst + (M - k), cconj(csub(e, o)));
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// inverse x-pass: N/2+1 complex -> N reals per row, times `scale`  (a6)
-//   A = Y[k], B = conj Y[M-k] (imaginary parts of Y[0], Y[M] dropped),
-//   Z'[k] = (A + B) + i w_N^{-k} (A - B),  z = IFFT_{N/2}(Z'),  x[2n] = Re z[n], x[2n+1] = Im z[n].
-// ------------------------------------------------------------------------------------------
-template <typename T, int N, int ROWS>
-__global__ void __launch_bounds__(ROWS *threads_per_fft(N / 2))
-    k_xpass_c2r(const Cx<T> *__restrict__ in, T *__restrict__ out, const Cx<T> *__restrict__ tab,
-                const Cx<T> *__restrict__ tw, long nrows, int ldk, T scale)
-{
-    using C = Cx<T>;
-    constexpr int M = N / 2;
-    constexpr int TPF = threads_per_fft(M);
-    constexpr bool WARP = (TPF <= 32) && (32 % TPF == 0);
-    using Map = RowMap<M>;
-    extern __shared__ __align__(16) unsigned char smraw[];
-    C *sm = reinterpret_cast<C *>(smraw);
-
-    const int c = threadIdx.x / TPF, t = threadIdx.x % TPF;
-    long row = (long)blockIdx.x * ROWS + c;
-    const bool valid = row < nrows;
-    if (!valid) row = nrows - 1;
-    const C *src = in + row * (long)ldk;
-    C *dst = reinterpret_cast<C *>(out + row * N);
-
-#pragma unroll 2
-    for (int k = t; k <= M / 2; k += TPF) {
-        C a = ld_stream(src + k);
-        C b = cconj(ld_stream(src + (M - k)));
-        if (k == 0) { a.y = (T)0; b.y = (T)0; }
-        const C w = root_of<+1>(tab, k);  // exp(+2 pi i k / N)
-        const C e = cadd(a, b);
-        const C o = mul_diri<+1>(cmul(w, csub(a, b)));
-        sm[Map::at(k, c)] = cadd(e, o);
-        if (k != 0 && 2 * k != M) sm[Map::at(M - k, c)] = cconj(csub(e, o));
-    }
-    group_sync<WARP>();
-
-    auto ld = [&](int) -> C { return mk<T>(0, 0); };
-    auto st = [&](int i, C v) {
-        if (valid) st_stream(dst + i, cscale(v, scale));
-    };
-    fft_stages<T, M, 1, +1, TPF, true, false, WARP, Map>(sm, tw, c, t, ld, st);
-}
 
 // ------------------------------------------------------------------------------------------
 // strided column pass (y or z): complex FFT of length N along an axis with element stride

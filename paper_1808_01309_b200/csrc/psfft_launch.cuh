@@ -18,8 +18,7 @@ namespace psfft {
 struct PassArgs {
     const void *tab;   // roots of unity exp(-2 pi i m/N), N complex of the plan dtype
     const void *twN;   // per-stage twiddle tables of the length-N transforms (y, z passes)
-    const void *twM;   // per-stage twiddle tables of the length-N/2 transforms (x passes)
-    const void *twX;   // per-stage twiddle tables of the length-N transforms in the symmetric schedule (mid_x)
+    const void *twX;   // per-stage twiddle tables of the length-N transforms in the symmetric schedule (x passes, mid_x)
     int N;             // grid points along x (and along y, z for the cubic plans every RHS call needs)
     int Ny, Nz;        // grid points along y, z (psfft_plan_create3: anisotropic grids, transforms only)
     const void *twY;   // per-stage tables of the length-Ny / length-Nz column transforms (= twN when cubic)
@@ -76,9 +75,9 @@ struct GpeArgs {
 };
 template <typename T> cudaError_t launch_gpe_pass(const PassArgs &a, const GpeArgs &g, int pass, int *launches);
 
-// complex entries of the tables of an (Nx, Ny, Nz) plan: [roots of unity, Nx][stage tables Ny][stage tables
-// Nx/2][symmetric-schedule stage tables Nx][stage tables Nz, only when Nz != Ny]
-struct TableOffsets { size_t y, m, x, z, total; };
+// complex entries of the tables of an (Nx, Ny, Nz) plan: [roots of unity, Nx][stage tables Ny]
+// [symmetric-schedule stage tables Nx (x passes, mid_x)][stage tables Nz, only when Nz != Ny]
+struct TableOffsets { size_t y, x, z, total; };
 TableOffsets table_entries(int Nx, int Ny, int Nz);
 // symmetric radix schedule of the mid_x transforms (psfft_midxg.cuh): fills radix[], returns the stage count
 int xsched_stages(int N, int *radix);

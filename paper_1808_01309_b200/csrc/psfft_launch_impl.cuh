@@ -4,50 +4,54 @@
 #include "psfft_kernels.cuh"
 #include "psfft_rhs.cuh"
 #include "psfft_midxg.cuh"
+#include "psfft_xpass2.cuh"
 #include "psfft_launch.cuh"
 
 namespace psfft {
 
 // tile shapes ------------------------------------------------------------------------------
-// x-pass: transforms per CTA so that a CTA has about 256 threads
-__host__ __device__ constexpr int xpass_rows(int N)
-{
-    int tpf = threads_per_fft(N / 2);
-    return tpf >= 256 ? 1 : 256 / tpf;
-}
 template <typename K> static cudaError_t set_smem(K kernel, size_t bytes)
 {
     if (bytes <= 48 * 1024) return cudaSuccess;
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// x-passes: two adjacent rows per complex length-N transform (psfft_xpass2.cuh); nrows is even for every
+// supported size
+template <typename T, int N> constexpr int xpass2_minb()
+{
+    constexpr int threads = xg_rows<N>() * XSched<N>::TPR;
+    constexpr int m = 512 / threads;
+    return m < 1 ? 1 : m;
+}
+
 template <typename T, int N>
 static cudaError_t xpass_r2c_n(const PassArgs &a, const void *in, void *out, long nrows)
 {
-    constexpr int ROWS = xpass_rows(N);
-    constexpr int TPF = threads_per_fft(N / 2);
-    constexpr size_t smem = (size_t)ROWS * RowMap<N / 2>::ld * sizeof(Cx<T>);
-    auto kern = k_xpass_r2c<T, N, ROWS>;
+    using C = Cx<T>;
+    constexpr int ROWS = xg_rows<N>(), THREADS = ROWS * XSched<N>::TPR;
+    constexpr size_t smem = (size_t)ROWS * 2 * XPad<N, (int)sizeof(C)>::BUF * sizeof(C);
+    auto kern = k_xpass2_r2c<T, N, xpass2_minb<T, N>()>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    const unsigned grid = (unsigned)((nrows + ROWS - 1) / ROWS);
-    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const T *)in, (Cx<T> *)out, (const Cx<T> *)a.tab,
-                                                (const Cx<T> *)a.twM, nrows, a.ldk);
+    const long npairs = nrows / 2;
+    kern<<<(unsigned)((npairs + ROWS - 1) / ROWS), THREADS, smem, a.stream>>>((const T *)in, (C *)out, (const C *)a.twX,
+                                                                              npairs, a.ldk);
     return cudaGetLastError();
 }
 
 template <typename T, int N>
 static cudaError_t xpass_c2r_n(const PassArgs &a, const void *in, void *out, long nrows, double scale)
 {
-    constexpr int ROWS = xpass_rows(N);
-    constexpr int TPF = threads_per_fft(N / 2);
-    constexpr size_t smem = (size_t)ROWS * RowMap<N / 2>::ld * sizeof(Cx<T>);
-    auto kern = k_xpass_c2r<T, N, ROWS>;
+    using C = Cx<T>;
+    constexpr int ROWS = xg_rows<N>(), THREADS = ROWS * XSched<N>::TPR;
+    constexpr size_t smem = (size_t)ROWS * XPad<N, (int)sizeof(C)>::BUF * sizeof(C);
+    auto kern = k_xpass2_c2r<T, N, xpass2_minb<T, N>()>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
-    const unsigned grid = (unsigned)((nrows + ROWS - 1) / ROWS);
-    kern<<<grid, ROWS * TPF, smem, a.stream>>>((const Cx<T> *)in, (T *)out, (const Cx<T> *)a.tab,
-                                                (const Cx<T> *)a.twM, nrows, a.ldk, (T)scale);
+    const long npairs = nrows / 2;
+    kern<<<(unsigned)((npairs + ROWS - 1) / ROWS), THREADS, smem, a.stream>>>((const C *)in, (T *)out, (const C *)a.twX,
+                                                                              npairs, a.ldk, (T)scale);
     return cudaGetLastError();
 }
 
