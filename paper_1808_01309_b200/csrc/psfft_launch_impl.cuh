@@ -107,6 +107,9 @@ static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
     auto kern = k_cpass_job<T, N, DIR, TC, TPF, MINB, Job>;
     cudaError_t e = set_smem(kern, smem);
     if (e != cudaSuccess) return e;
+    // small grids (N <= 256): one CTA per (tile position, round) instead of looping over the rounds, so that
+    // the pass fills the machine
+    if (Job::split_rounds && (long)grid.x * grid.y < 2048) grid.z = (unsigned)job.rounds();
     kern<<<grid, TC * TPF, smem, a.stream>>>(job, (const C *)a.twN);
     return cudaGetLastError();
 }

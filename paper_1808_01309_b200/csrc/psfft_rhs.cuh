@@ -83,6 +83,7 @@ template <class Derived, typename C, typename E> struct JobElems {
     static constexpr int EW = ElemWidth<E>::value;
     using Elem = E;
     static constexpr bool prefetch_next = false;
+    static constexpr bool split_rounds = true;   // rounds are independent: may run in different CTAs
     template <class State> __device__ __forceinline__ const void *next_addr(const State &, int, int) const { return nullptr; }
     template <class State> __device__ __forceinline__ E load_e(const State *s, int r, int i) const
     {
@@ -129,16 +130,17 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
         for (int j = 0; j < EW; ++j) job.idle(s[j], t, blockDim.x / TC);
         return;
     }
+    // gridDim.z > 1 (small grids, see run_job_v): the rounds of a tile position are spread over blockIdx.z
 #pragma unroll 1
-    for (int r = 0; r < job.rounds(); ++r) {
+    for (int r = blockIdx.z; r < job.rounds(); r += gridDim.z) {
         // Jobs that ask for it: pull the next round's tile into L2 while this round computes -- one prefetch
         // per 128-byte tile row, issued by the threads of the tile's first column (whose retained range is the
         // widest).  Measured at 512^3: fp32 inv_y 1.05 -> 0.94 ms, fwd_y 0.41 -> 0.35 ms; no gain in fp64 and
         // for the z passes, which leave it off.
         if constexpr (Job::prefetch_next) {
-            if (c == 0 && r + 1 < job.rounds()) {
+            if (c == 0 && r + (int)gridDim.z < job.rounds()) {
                 for (int i = t; i < N; i += TPF) {
-                    const void *p = job.next_addr(s[0], r + 1, i);
+                    const void *p = job.next_addr(s[0], r + (int)gridDim.z, i);
                     if (p) asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
                 }
             }
@@ -163,7 +165,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvZ : JobElems<J
     long wplane, wnf;   // workspace layout: kxp N, kxp N N
     struct State { long col, wcol; int kxy2, ky; bool active; };
 
-    __device__ __forceinline__ int rounds() const { return 5 * NV + 2 * NS; }
+    __host__ __device__ __forceinline__ int rounds() const { return 5 * NV + 2 * NS; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, N);
@@ -229,7 +231,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
     struct State { long base; int kx; bool active; };
     static constexpr bool prefetch_next = sizeof(T) == 4;
 
-    __device__ __forceinline__ int rounds() const { return 6 * NV + 3 * NS; }
+    __host__ __device__ __forceinline__ int rounds() const { return 6 * NV + 3 * NS; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
@@ -319,7 +321,7 @@ template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>
     struct State { long base; int kx; bool active; };
     static constexpr bool prefetch_next = sizeof(T) == 4;
 
-    __device__ __forceinline__ int rounds() const { return nfields; }
+    __host__ __device__ __forceinline__ int rounds() const { return nfields; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
@@ -390,12 +392,13 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     T cstep;
     bool sparse;         // intermediate Runge-Kutta stage: the zeros outside the truncation sphere are not written
                          // (the next stage masks on load and never reads them)
+    static constexpr bool split_rounds = false;   // the third component's epilogue reads the first two back
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
     int ldk;
     struct State { long col, wcol; int kx, ky, kxy2; bool active, valid; };
 
-    __device__ __forceinline__ int rounds() const { return 3 * NV + NS; }
+    __host__ __device__ __forceinline__ int rounds() const { return 3 * NV + NS; }
     // grid (ceil(ldk N / TC)): tile = TC consecutive columns of the caller's (ky, kx) plane, whose
     // 128-byte rows are line-aligned (the plane size ldk N is a multiple of TC); the workspace side
     // is read at the compact address of the same (ky, kx)
@@ -525,7 +528,7 @@ template <typename T, int N, int TC, int NF> struct JobPlainInvZ : JobElems<JobP
     C *dst;             // NF compact fields
     long plane, nf, wplane, wnf;
     struct State { long col, wcol; int kxy2; bool active; };
-    __device__ __forceinline__ int rounds() const { return NF; }
+    __host__ __device__ __forceinline__ int rounds() const { return NF; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, N);
@@ -562,7 +565,7 @@ template <typename T, int N, int TC> struct JobPlainInvY : JobElems<JobPlainInvY
     long wplane, wnf;
     int kxp, nfields;
     struct State { long base; int kx; bool active; };
-    __device__ __forceinline__ int rounds() const { return nfields; }
+    __host__ __device__ __forceinline__ int rounds() const { return nfields; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
@@ -593,10 +596,11 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
     const C *base;       // Runge-Kutta stage: y_n (NULL: plain right-hand side)
     T alpha, beta, cstep;
     bool sparse;         // as in JobFwdZ
+    static constexpr bool split_rounds = false;   // the idle path fills both fields
     long plane, nf, wplane, wnf;
     int ldk;
     struct State { long col, wcol; int kxy2; bool active, valid; };
-    __device__ __forceinline__ int rounds() const { return 2; }
+    __host__ __device__ __forceinline__ int rounds() const { return 2; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.col = colidx;
