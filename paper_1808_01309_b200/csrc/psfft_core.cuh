@@ -182,13 +182,19 @@ __host__ __device__ constexpr bool supported_len(int L)
 // small N until a CTA has at least 128 threads.  (Measured on B200, 512^3 fp64: 64-byte rows run
 // the z-pass at 3.5 TB/s, 128-byte rows at 5.4 TB/s; profiles/r1a_summary.md.)
 __host__ __device__ constexpr int cpass_tpf(int N) { return N >= 128 ? N / 16 : threads_per_fft(N); }
-__host__ __device__ constexpr int cpass_cols(int N, int csize)
+// `cap`: largest tile in bytes.  64 KB (two tiles per SM) is the rule; at N = 1024 a 64 KB tile would have
+// 64-byte rows, and one 128 KB tile per SM with 128-byte rows is faster (measured, 1024^3 fp32 MHD: fwd_z
+// 15.1 -> 10.8 ms, fwd_y 7.7 -> 7.0 ms, inv_y unchanged); at N = 768 only the z-pass with the epilogue gains.
+__host__ __device__ constexpr int cpass_cols_cap(int N, int csize, long cap)
 {
     int tc = 128 / csize;
-    while (tc > 1 && (long)N * tc * csize > 65536) tc /= 2;
+    while (tc > 1 && (long)N * tc * csize > cap) tc /= 2;
     while (tc * cpass_tpf(N) < 128 && (long)N * tc * 2 * csize <= 65536) tc *= 2;
     return tc;
 }
+__host__ __device__ constexpr int cpass_cols(int N, int csize) { return cpass_cols_cap(N, csize, N >= 1024 ? 131072 : 65536); }
+// fwd_z (the pass that also writes the dense output) takes the big tile from N = 768 on
+__host__ __device__ constexpr int fwdz_cols(int N, int csize) { return cpass_cols_cap(N, csize, N >= 768 ? 131072 : 65536); }
 
 // number of kx with 9 kx^2 < N^2 (2/3-rule), and the compact row pitch of the RHS workspace fields:
 // kx_count rounded up to whole tiles of TC columns

@@ -82,17 +82,22 @@ static cudaError_t cpass_v(const PassArgs &a, int axis, const void *in, void *ou
 // Column passes: 8 elements per thread (one radix-8 butterfly per stage) while the CTA stays within
 // 512 threads -- twice the warps of the 16-element shape for the same two tiles per SM (measured, 512^3
 // fp64: inv_y 1.67 -> 1.50 ms, fwd_y 0.85 -> 0.60 ms; profiles/r1b_summary.md)
-__host__ __device__ constexpr int job_tpf(int N, int TC)
+// (A tile above 64 KB is alone on its SM and may take 1024 threads.)
+__host__ __device__ constexpr int job_tpf(int N, int TC, int esize)
 {
-    return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= 512) ? N / 8 : cpass_tpf(N);
+    const int cap = (long)N * TC * esize > 65536 ? 1024 : 512;
+    return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= cap) ? N / 8 : cpass_tpf(N);
 }
 
 template <typename T, int N, int DIR>
 static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
-    constexpr int TC = cpass_cols(N, (int)sizeof(Ex<T>));   // 16-byte elements in both precisions
-    constexpr int TPF = job_tpf(N, TC);
-    return cpass_v<T, N, DIR, TC, TPF, 2>(a, axis, in, out, fields);
+    // 16-byte elements in both precisions; the plain passes keep 64 KB tiles at every N (measured: 1024 x 1024 x 256
+    // r2c + c2r 5.77 ms with 64 KB tiles, 5.96 ms with 128 KB ones)
+    constexpr int TC = cpass_cols_cap(N, (int)sizeof(Ex<T>), 65536);
+    constexpr int TPF = job_tpf(N, TC, 16);
+    constexpr int MINB = ((long)N * TC * 16 * 2 <= 220 * 1024 && 2 * TC * TPF <= 1024) ? 2 : 1;
+    return cpass_v<T, N, DIR, TC, TPF, MINB>(a, axis, in, out, fields);
 }
 
 // ---- fused right-hand side -------------------------------------------------------------------
@@ -101,7 +106,7 @@ static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
 {
     using C = Cx<T>;
     using E = typename Job::Elem;
-    constexpr int TC = cpass_cols(N, (int)sizeof(E));   // elements per tile row
+    constexpr int TC = Job::is_fwdz ? fwdz_cols(N, (int)sizeof(E)) : cpass_cols(N, (int)sizeof(E));   // elements per tile row
     constexpr bool PAD = (TC * sizeof(E) < 128);
     constexpr size_t smem = (size_t)ColMap<N, TC, PAD>::size * sizeof(E);
     auto kern = k_cpass_job<T, N, DIR, TC, TPF, MINB, Job>;
@@ -117,8 +122,12 @@ static cudaError_t run_job_v(const PassArgs &a, const Job &job, dim3 grid)
 template <typename T, int N, int DIR, class Job>
 static cudaError_t run_job(const PassArgs &a, const Job &job, dim3 grid)
 {
-    constexpr int TC = cpass_cols(N, (int)sizeof(typename Job::Elem));
-    return run_job_v<T, N, DIR, job_tpf(N, TC), 2>(a, job, grid);
+    using E = typename Job::Elem;
+    constexpr int TC = Job::is_fwdz ? fwdz_cols(N, (int)sizeof(E)) : cpass_cols(N, (int)sizeof(E));
+    // two CTAs per SM when two tiles fit in shared memory and two CTAs' threads in the register file at 64 each
+    constexpr int TPF = job_tpf(N, TC, (int)sizeof(E));
+    constexpr int MINB = ((long)N * TC * sizeof(E) * 2 <= 220 * 1024 && 2 * TC * TPF <= 1024) ? 2 : 1;
+    return run_job_v<T, N, DIR, TPF, MINB>(a, job, grid);
 }
 
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_inv_z_n(const PassArgs &a, const RhsArgs &r)
@@ -198,7 +207,7 @@ template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_y_n(cons
 template <typename T, int N, int NV, int NS> static cudaError_t rhs_fwd_z_n(const PassArgs &a, const RhsArgs &r)
 {
     using C = Cx<T>;
-    constexpr int TC = cpass_cols(N, (int)sizeof(C)), EW = 1;   // single columns in both precisions
+    constexpr int TC = fwdz_cols(N, (int)sizeof(C)), EW = 1;   // single columns in both precisions
     constexpr int KXP = rhs_pitch(N, (int)sizeof(C));
     JobFwdZ<T, N, TC, NV, NS> job;
     job.sdst = (C *)r.sdst;
@@ -260,7 +269,7 @@ template <typename T, int N> static cudaError_t gpe_pass_n(const PassArgs &a, co
                                                                      wplane * N, KXP, (T)(1.0 / ((double)N * N * N)));
         return cudaGetLastError();
     }
-    constexpr int TCZ = cpass_cols(N, (int)sizeof(C));
+    constexpr int TCZ = fwdz_cols(N, (int)sizeof(C));
     JobGpeFwdZ<T, N, TCZ> job;
     job.src = (const C *)g.obuf; job.dst = (C *)g.dst; job.psi = (const C *)g.psi; job.base = (const C *)g.base;
     job.alpha = (T)g.alpha; job.beta = (T)g.beta; job.cstep = (T)g.cstep; job.sparse = g.sparse_out;

@@ -84,6 +84,7 @@ template <class Derived, typename C, typename E> struct JobElems {
     using Elem = E;
     static constexpr bool prefetch_next = false;
     static constexpr bool split_rounds = true;   // rounds are independent: may run in different CTAs
+    static constexpr bool is_fwdz = false;       // tile width rule: cpass_cols (fwdz_cols for the last pass)
     template <class State> __device__ __forceinline__ const void *next_addr(const State &, int, int) const { return nullptr; }
     template <class State> __device__ __forceinline__ E load_e(const State *s, int r, int i) const
     {
@@ -393,6 +394,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     bool sparse;         // intermediate Runge-Kutta stage: the zeros outside the truncation sphere are not written
                          // (the next stage masks on load and never reads them)
     static constexpr bool split_rounds = false;   // the third component's epilogue reads the first two back
+    static constexpr bool is_fwdz = true;
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
     int ldk;
@@ -597,6 +599,7 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
     T alpha, beta, cstep;
     bool sparse;         // as in JobFwdZ
     static constexpr bool split_rounds = false;   // the idle path fills both fields
+    static constexpr bool is_fwdz = true;
     long plane, nf, wplane, wnf;
     int ldk;
     struct State { long col, wcol; int kxy2; bool active, valid; };
