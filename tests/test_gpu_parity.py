@@ -64,6 +64,17 @@ def test_c2r_matches_oracle_on_non_hermitian_input(N, dtype):
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [192, 256, 384])
+def test_r2c_c2r_at_the_remaining_sizes(N, dtype):
+    x = synth.uniform_field(N, 1, 99, RDT[dtype])
+    p = psfft.Plan(N, dtype, 1)
+    X = p.r2c(dev(x))
+    Xo = oracle.r2c3d(x[0].astype(np.float64))
+    assert rel(X.cpu().numpy()[0], Xo) < TOL[dtype]
+    assert rel(p.c2r(X).cpu().numpy(), x) < TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 def test_config1_roundtrip_32(dtype):
     """BASELINE.json config 1: 32^3, uniform [-1,1) from seed, r2c then c2r; spectrum and round trip vs oracle."""
     N = 32
@@ -199,6 +210,19 @@ def test_config2_hd_rhs_128(dtype):
     assert rel(got, want) < TOL[dtype]
     M = oracle.dealias_mask(128)
     assert np.all(got[:, ~M] == 0)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [192, 256, 384])
+def test_rhs_at_the_remaining_sizes(N, dtype):
+    """Every supported size runs its own radix schedules (mid_x: 8 3 8, 8 4 8, 8 2 3 8): HD and Boussinesq against
+    the oracle on the grid itself."""
+    got, want = hd_case(N, 4.0, 32, dtype, nu=0.01)
+    assert rel(got, want) < TOL[dtype]
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+    if N != 384:
+        ru, rt, wu, wt = boussinesq_case(N, 4.0, 32, dtype, 0.01, 0.02, 1.5)
+        assert rel(ru, wu) < TOL[dtype] and rel(rt, wt) < TOL[dtype]
 
 
 def test_hd_rhs_viscous_term():
