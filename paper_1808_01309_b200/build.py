@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpsfft.so")
-SOURCES = ["psfft_api.cu", "psfft_f64.cu", "psfft_f32.cu"]
+SOURCES = ["psfft_api.cu"] + [f"psfft_{dt}_{grp}.cu" for dt in ("f64", "f32") for grp in ("midx", "col", "fft")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
@@ -47,7 +47,7 @@ def _stale() -> bool:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile the three translation units in parallel and link libpsfft.so.  Returns its path."""
+    """Compile the translation units in parallel and link libpsfft.so.  Returns its path."""
     if not force and not _stale():
         return LIB
     nvcc = _nvcc()

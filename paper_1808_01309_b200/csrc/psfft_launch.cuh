@@ -1,5 +1,5 @@
 // psfft_launch.cuh -- host-side launchers: pick the kernel instantiation for (dtype, N) and
-// enqueue it.  Declared here, defined (per dtype) in psfft_f32.cu / psfft_f64.cu.
+// enqueue it.  Declared here, defined in psfft_launch_impl.cuh and instantiated per dtype in psfft_f{32,64}_*.cu.
 #pragma once
 #include <cuda_runtime.h>
 #include <stddef.h>

@@ -1,5 +1,5 @@
-// psfft_launch_impl.cuh -- definitions of the launchers; included by psfft_f32.cu / psfft_f64.cu,
-// which instantiate them for one dtype each (two translation units compile in parallel).
+// psfft_launch_impl.cuh -- definitions of the launchers; included by psfft_f{32,64}_{fft,col,midx}.cu,
+// which instantiate one group of them for one dtype each (six translation units compile in parallel).
 #pragma once
 #include "psfft_kernels.cuh"
 #include "psfft_rhs.cuh"
@@ -385,7 +385,9 @@ cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void
     return cudaGetLastError();
 }
 
-#define PSFFT_INSTANTIATE(T)                                                                                          \
+// Explicit instantiations, in three groups per dtype so that six translation units compile in parallel
+// (psfft_f{32,64}_{fft,col,midx}.cu).
+#define PSFFT_INSTANTIATE_FFT(T)                                                                                      \
     template cudaError_t launch_xpass_r2c<T>(const PassArgs &, const void *, void *, long, int *);                    \
     template cudaError_t launch_xpass_c2r<T>(const PassArgs &, const void *, void *, long, double, int *);            \
     template cudaError_t launch_cpass<T>(const PassArgs &, int, int, const void *, void *, int, int *);               \
@@ -393,12 +395,14 @@ cudaError_t launch_finish(const PassArgs &a, int mode, const void *f, const void
     template cudaError_t launch_cross<T>(const PassArgs &, const void *, const void *, void *, int *);                \
     template cudaError_t launch_cross_mhd<T>(const PassArgs &, const void *, const void *, const void *, const void *, \
                                              void *, void *, int *);                                                  \
-    template cudaError_t launch_finish<T>(const PassArgs &, int, const void *, const void *, void *, double, int *); \
+    template cudaError_t launch_finish<T>(const PassArgs &, int, const void *, const void *, void *, double, int *);
+#define PSFFT_INSTANTIATE_COL(T)                                                                                      \
     template cudaError_t launch_rhs_inv_z<T>(const PassArgs &, const RhsArgs &, int *);                               \
     template cudaError_t launch_rhs_inv_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
-    template cudaError_t launch_rhs_mid_x<T>(const PassArgs &, const RhsArgs &, int *);                               \
     template cudaError_t launch_rhs_fwd_y<T>(const PassArgs &, const RhsArgs &, int *);                               \
     template cudaError_t launch_gpe_pass<T>(const PassArgs &, const GpeArgs &, int, int *);                            \
     template cudaError_t launch_rhs_fwd_z<T>(const PassArgs &, const RhsArgs &, int *);
+#define PSFFT_INSTANTIATE_MIDX(T)                                                                                     \
+    template cudaError_t launch_rhs_mid_x<T>(const PassArgs &, const RhsArgs &, int *);
 
 }  // namespace psfft
