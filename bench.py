@@ -130,20 +130,37 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(kernel: str):
-    """dram bytes (read + write) per launch of `kernel` from the committed ncu --set full capture
-    (profiles/traffic.csv: kernel,dram_bytes_per_launch,source), or None."""
+def kernel_revision() -> str:
+    """sha1 (first 12 hex digits) over the kernel sources: the revision an ncu capture belongs to."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1808_01309_b200", "csrc")
+    h = hashlib.sha1()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:12]
+
+
+def ncu_traffic(kernel: str, workload: str = "512^3 fp64"):
+    """(dram bytes (read + write) per launch of `kernel`, source) from the committed ncu --set full captures
+    (profiles/traffic.csv: workload,kernel,dram_bytes_per_launch,source,kernel_revision), or (None, why) when
+    there is no row or the row was captured on another revision of the kernel sources."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
-        return None
+        return None, "profiles/traffic.csv missing"
+    rev = kernel_revision()
+    stale = None
     try:
         for line in open(p).read().splitlines()[1:]:
-            cols = line.split(",")
-            if cols and cols[0] == kernel:
-                return float(cols[1])
-    except Exception:
-        return None
-    return None
+            cols = [c.strip() for c in line.split(",")]
+            if len(cols) >= 5 and cols[0] == workload and cols[1] == kernel:
+                if cols[4] == rev:
+                    return float(cols[2]), cols[3]
+                stale = f"capture {cols[3]} is of kernel revision {cols[4]}, the tree is {rev}"
+    except Exception as exc:
+        return None, str(exc)[:80]
+    return None, stale or "no capture for this kernel / workload"
 
 
 # ---- the oracle as CPU baseline (bench.py is one of the three places allowed to run oracle/) -------------
@@ -157,49 +174,92 @@ def work_ratio(N: int, n: int) -> float:
     return (N ** 3 * 3 * math.log2(N)) / (n ** 3 * 3 * math.log2(n))
 
 
-def oracle_sample(N: int, n: int, seed: int = 1234):
-    """One oracle hd_rhs at n^3 on all host cores; returns (seconds, cores)."""
+def cpu_model() -> str:
+    try:
+        for l in open("/proc/cpuinfo"):
+            if l.startswith("model name"):
+                return l.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_hd_rhs_seconds(n: int, threads: int, seed: int = 1234, uh=None):
+    """One oracle hd_rhs at n^3 (the metric's field recipe) on `threads` threads; returns (seconds, threads in effect)."""
     import numpy as np
     import oracle
     from paper_1808_01309_b200 import synth
-    cores = oracle.set_threads(os.cpu_count() or 1)
-    uh = synth.solenoidal_spectrum(n, 4.0, 32, seed)
+    cores = oracle.set_threads(threads)
+    if uh is None:
+        uh = synth.solenoidal_spectrum(n, 4.0, min(32, n // 2 - 1), seed)
     t0 = time.perf_counter()
     out = oracle.hd_rhs(uh, 0.0)
     dt = time.perf_counter() - t0
-    assert np.isfinite(out).all()
+    assert np.isfinite(out[:, :2, :2, :2]).all()
     return dt, cores
 
 
 def cpu_baseline(N: int) -> dict:
-    dt, cores = oracle_sample(N, SAMPLE_N)
-    return {"value": 1.0 / (dt * work_ratio(N, SAMPLE_N)), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"one oracle hd_rhs at {SAMPLE_N}^3 (same field recipe) in {dt:.2f} s on {cores} threads, scaled "
-                      f"to {N}^3 by the N^3 log2 N^3 work ratio {work_ratio(N, SAMPLE_N):.2f}"}
+    """The oracle as it stands on the box's host cores (SURVEY.md §8(d) "CPU baseline"): ONE real evaluation of
+    the metric's workload (hd_rhs at N^3, O6) on all cores, one r2c3d + c2r3d of one N^3 field (O3 + O4, the
+    transform half of the metric), and the single-thread figure measured at 256^3 (a single-thread N = 512
+    evaluation takes minutes; the 256^3 time is reported as measured, the scaled figure is labelled as such)."""
+    import numpy as np
+    import oracle
+    from paper_1808_01309_b200 import synth
+    ncpu = os.cpu_count() or 1
+    dt, cores = oracle_hd_rhs_seconds(N, ncpu)
+    x = synth.uniform_field(N, 1, 1234)[0]
+    t0 = time.perf_counter()
+    X = oracle.r2c3d(x)
+    t_f = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    y = oracle.c2r3d(X)
+    t_b = time.perf_counter() - t0
+    rt = float(np.abs(y - x).max())
+    del X, y, x
+    n1 = min(N, SAMPLE_N)
+    dt1, c1 = oracle_hd_rhs_seconds(n1, 1)
+    oracle.set_threads(ncpu)
+    return {"value": 1.0 / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model(),
+            "sample": f"one full oracle hd_rhs (O6) at {N}^3, the metric's own workload and field, {dt:.2f} s on {cores} "
+                      f"OpenMP threads; no extrapolation",
+            "seconds_per_eval": dt,
+            "fft3d": {"what": f"oracle r2c3d + c2r3d (O3 + O4) of one {N}^3 fp64 field on {cores} threads",
+                      "s_r2c": t_f, "s_c2r": t_b, "ms_r2c_plus_c2r_per_field": (t_f + t_b) * 1e3,
+                      "roundtrip_max_abs_err": rt},
+            "single_thread": {"N": n1, "cores": c1, "seconds_per_eval": dt1, "evals_per_s_at_that_N": 1.0 / dt1,
+                              "scaled_to_metric_N": {"extrapolated": n1 != N, "evals_per_s": 1.0 / (dt1 * work_ratio(N, n1)),
+                                                     "how": f"x {work_ratio(N, n1):.2f} (N^3 log2 N^3 work ratio)"}}}
 
 
 def run_reference(args) -> int:
-    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    """--impl reference: the oracle, as it stands, on the host cores.  Every step is ONE REAL evaluation of the
+    metric's workload (oracle hd_rhs at N^3 on all cores, about 15-20 s at 512^3); the number of steps actually run
+    is capped so that the arm ends within a few minutes, and `steps` / `ms_per_step` report what was run."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
+    from paper_1808_01309_b200 import synth
     N = args.N
-    n = SAMPLE_N
-    t_first, cores = oracle_sample(N, n)
-    if t_first * (args.steps + args.warmup) > 240.0:
-        n = 128
-    for _ in range(max(0, args.warmup - 1)):
-        oracle_sample(N, n)
-    times = [oracle_sample(N, n)[0] for _ in range(args.steps)]
+    ncpu = os.cpu_count() or 1
+    uh = synth.solenoidal_spectrum(N, 4.0, min(32, N // 2 - 1), 1234)
+    t_start = time.perf_counter()
+    t_warm, cores = oracle_hd_rhs_seconds(N, ncpu, uh=uh)            # one warm-up evaluation (page faults, thread pool)
+    budget = float(args.reference_budget_s)
+    steps = max(1, min(args.steps, int((budget - t_warm) / max(t_warm, 1e-3))))
+    times = [oracle_hd_rhs_seconds(N, ncpu, uh=uh)[0] for _ in range(steps)]
     dt = sum(times) / len(times)
-    value = 1.0 / (dt * work_ratio(N, n))
-    sample = (f"each step = one oracle hd_rhs at {n}^3 on {cores} threads ({dt:.2f} s), scaled to {N}^3 by the "
-              f"N^3 log2 N^3 work ratio {work_ratio(N, n):.2f}")
+    value = 1.0 / dt
+    sample = (f"each step = one full oracle hd_rhs (O6) at {N}^3 on {cores} threads ({dt:.2f} s); {steps} of the requested "
+              f"{args.steps} steps run after 1 warm-up (cap: {budget:.0f} s of oracle time); no extrapolation")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * work_ratio(N, n) * 1e3,
+            "steps": steps, "warmup": 1, "steps_requested": args.steps, "warmup_requested": args.warmup,
+            "ms_per_step": dt * 1e3, "wall_s": time.perf_counter() - t_start,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": workload_config(N, world),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -228,6 +288,129 @@ def time_loop(fn, steps: int, stream) -> float:
     return e0.elapsed_time(e1) / steps
 
 
+def roofline_of(recs, K: int, ms_step: float, dense_bytes: float, dense_model: str, peak: float, workload: str) -> dict:
+    """Roofline object from the per-launch records (kernel name, ms, algorithmic bytes) of K steps.
+    Three different questions, kept apart:
+      frac                         dominant kernel: its algorithmic bytes (compulsory reads + writes GIVEN the zero
+                                   structure of the dealiased spectra) / its launch time / peak
+      step_bytes_moved.frac        whole step: sum of all kernels' algorithmic bytes / step time / peak
+      step_dense_model.equivalent_frac
+                                   whole step against SURVEY.md §8(a)'s DENSE count (42 C HD, 84 C MHD): may exceed 1
+                                   because the pruned passes move about half of those bytes -- an equivalent-work
+                                   figure, not a bandwidth."""
+    tot = {}
+    for name, t, b in recs:
+        a = tot.setdefault(name, [0.0, 0.0, 0])
+        a[0] += t; a[1] += b; a[2] += 1
+    dom = max(tot, key=lambda k: tot[k][0])
+    achieved = tot[dom][1] / (tot[dom][0] * 1e-3) / 1e9
+    moved = sum(v[1] for v in tot.values()) / K
+    traffic, traffic_src = ncu_traffic(dom, workload)
+    return {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+            "launches_timed": tot[dom][2], "avg_launch_ms": tot[dom][0] / tot[dom][2],
+            "algorithmic_bytes_per_launch": tot[dom][1] / tot[dom][2],
+            "kernel_share_of_step": tot[dom][0] / sum(v[0] for v in tot.values()),
+            "per_kernel": {k: {"ms_per_step": v[0] / K, "GBps": v[1] / (v[0] * 1e-3) / 1e9, "frac": v[1] / (v[0] * 1e-3) / 1e9 / peak,
+                               "launches_per_step": v[2] / K} for k, v in tot.items()},
+            "step_bytes_moved": {"algorithmic_bytes": moved, "GBps": moved / (ms_step * 1e-3) / 1e9,
+                                 "frac": moved / (ms_step * 1e-3) / 1e9 / peak},
+            "step_dense_model": {"algorithmic_bytes": dense_bytes, "model": dense_model,
+                                 "GBps_equivalent": dense_bytes / (ms_step * 1e-3) / 1e9,
+                                 "equivalent_frac": dense_bytes / (ms_step * 1e-3) / 1e9 / peak}}
+
+
+def device_spectrum(torch, synth, N, k0, kcut, seed, tag, cdtype, dev):
+    """synth.solenoidal_spectrum built directly on the device: zeros + a scatter of the few thousand modes."""
+    iz, iy, ix, v = synth.solenoidal_modes(N, k0, kcut, seed, tag)
+    u = torch.zeros((3, N, N, N // 2 + 1), dtype=cdtype, device=dev)
+    t = lambda a: torch.from_numpy(a.astype("int64")).to(dev)
+    u[:, t(iz), t(iy), t(ix)] = torch.from_numpy(v).to(dev).to(cdtype)
+    return u
+
+
+def other_configs(torch, psfft, synth, dev, stream, peak, K: int) -> dict:
+    """BASELINE.json configs 1, 2, 4, 5 (the metric's config 3 / 3b is the headline), same protocol: plan outside
+    the timed region, 3 warm-up calls, K timed calls between CUDA events, device-resident inputs; then K more
+    calls with the per-launch events on for the bytes actually moved.  Inputs of 768^3 / 1024^3 are far larger
+    than L2; 32^3 and 128^3 are (partly) L2-resident and latency-bound -- reported in microseconds, no fraction
+    for 32^3 (SURVEY.md §8(d) table "Synthetic inputs")."""
+    import gc
+    out = {}
+
+    def timed(fn, n):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        return time_loop(fn, n, stream)
+
+    # configs[0]: 32^3 fp64 r2c + c2r, one field
+    N = 32
+    p = psfft.Plan(N, torch.float64, 1, device=dev)
+    x = torch.from_numpy(synth.uniform_field(N, 1, 1234)).to(dev)
+    X = torch.empty(p.spec_shape(1), dtype=torch.complex128, device=dev)
+    y = torch.empty_like(x)
+    w = p.ensure_work("fft")
+    t_f = timed(lambda: psfft.fft3d_r2c(p.handle, x, X, w), 200)
+    t_b = timed(lambda: psfft.fft3d_c2r(p.handle, X, y, w), 200)
+    out["configs[0]"] = {"workload": "32^3 fp64 r2c then c2r, one field, uniform [-1,1) seed 1234", "us_r2c": t_f * 1e3,
+                         "us_c2r": t_b * 1e3, "launches": 6, "roundtrip_max_abs_err": float((y - x).abs().max()),
+                         "note": "latency-bound (3 launches per direction, 0.5 MB working set in L2): no roofline fraction"}
+    p.close()
+    del p, x, X, y, w
+
+    def rhs_config(key, N, rdtype, system, k0, kcut, workload, dense_units, note):
+        gc.collect()
+        torch.cuda.empty_cache()
+        cdt = torch.complex128 if rdtype == torch.float64 else torch.complex64
+        code = psfft.F64 if rdtype == torch.float64 else psfft.F32
+        lay = psfft.plan_query(N, code, 1)
+        nvec = 2 if system == "mhd" else 1
+        need = (lay.work_bytes_mhd if system == "mhd" else lay.work_bytes_hd) + 6 * nvec * lay.spec_bytes
+        free = torch.cuda.mem_get_info(dev)[0]
+        if free < need + (1 << 30):
+            out[key] = {"workload": workload, "skipped": f"needs {need / 2**30:.0f} GiB, {free / 2**30:.0f} GiB free"}
+            return
+        p = psfft.Plan(N, rdtype, 1, device=dev, work=system)
+        u = device_spectrum(torch, synth, N, k0, kcut, 1234, 0, cdt, dev)
+        ru = torch.empty_like(u)
+        wk = p.ensure_work(system)
+        if system == "mhd":
+            b = device_spectrum(torch, synth, N, k0, kcut, 1234, 1, cdt, dev)
+            rb = torch.empty_like(b)
+            fn = lambda: psfft.mhd_rhs(p.handle, u, b, ru, rb, 0.0, 0.0, wk)
+        else:
+            fn = lambda: psfft.hd_rhs(p.handle, u, ru, 0.0, wk)
+        n = max(3, min(K, 10))
+        ms = timed(fn, n)
+        psfft.profile_reset(p.handle)
+        psfft.profile_enable(p.handle, True)
+        time_loop(fn, n, stream)
+        torch.cuda.synchronize()
+        psfft.profile_enable(p.handle, False)
+        dt = "fp64" if rdtype == torch.float64 else "fp32"
+        rl = roofline_of(psfft.profile_records(p.handle), n, ms, dense_units * lay.spec_bytes,
+                         f"fused 3-pass dense count = {dense_units} C (SURVEY.md §8(a))", peak, f"{N}^3 {dt}")
+        out[key] = {"workload": workload, "ms": ms, "evals_per_s": 1e3 / ms, "steps": n,
+                    "frac_bytes_moved": rl["step_bytes_moved"]["frac"],
+                    "dense_model_equivalent_frac": rl["step_dense_model"]["equivalent_frac"],
+                    "dominant_kernel": rl["kernel"], "dominant_kernel_frac": rl["frac"],
+                    "per_kernel": rl["per_kernel"], "launches_per_eval": psfft.last_launch_count(p.handle), "note": note}
+        p.close()
+
+    rhs_config("configs[1]", 128, torch.float64, "hd", 4.0, 32,
+               "128^3 fp64 HD RHS, E(k) ~ k^4 exp(-2(k/4)^2), unit energy, seed 1234", 42,
+               "working set ~ 0.2 GB against 126 MB of L2: partly L2-resident, fractions may exceed the HBM figure")
+    rhs_config("configs[3]", 768, torch.float32, "hd", 4.0, 32,
+               "768^3 fp32 HD RHS (radix-3 schedules), same field recipe, k0 = 4", 42, "inputs far larger than L2")
+    rhs_config("configs[4]", 1024, torch.float32, "mhd", 3.0, 24,
+               "1024^3 fp32 MHD RHS, u and b each E(k) ~ k^4 exp(-2(k/3)^2), 12 inverse + 6 forward transforms", 84,
+               "155 GB resident; inputs far larger than L2")
+    gc.collect()
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args) -> int:
     import numpy as np
     import torch
@@ -243,7 +426,29 @@ def run_ours(args) -> int:
     N, K, W = args.N, args.steps, max(3, args.warmup)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream()
+    peak, peak_src = hbm_peak()
+    m = metric_parts(torch, psfft, synth, N, K, W, rank, local, world, dev, stream, peak, peak_src)   # its buffers die here
 
+    # ---- the other BASELINE.json configs, after the metric (they need the memory the 512^3 buffers held) ----
+    configs = None
+    if world == 1 and not args.no_configs:
+        configs = other_configs(torch, psfft, synth, dev, stream, peak, K)
+
+    if rank != 0:
+        return 0
+    line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": m["ms_max"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(N, world), "clocks": m["clk"], "e2e": m["e2e"],
+            "gpu_launches": m["launches_per_step"] * K, "launches_per_step": m["launches_per_step"],
+            "roofline": m["roofline"], "fft3d": m["fft3d"], "next_rows": m["next_rows"], "configs": configs}
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(N)
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def metric_parts(torch, psfft, synth, N, K, W, rank, local, world, dev, stream, peak, peak_src) -> dict:
+    """The metric's two halves at N^3 fp64 (HD RHS evals/s; batch-3 r2c + c2r) plus e2e and the NEXT rows."""
     # synthetic input (host, pinned) -> device
     kcut = min(32, N // 2 - 1)
     uh_host = torch.from_numpy(synth.solenoidal_spectrum(N, 4.0, kcut, 1234 + rank)).pin_memory()
@@ -262,39 +467,30 @@ def run_ours(args) -> int:
     torch.cuda.synchronize()
     launches_per_step = psfft.last_launch_count(h)
 
-    # ---- timed region: K steps, device-resident input, per-launch events recorded live ----------------
-    psfft.profile_reset(h)
-    psfft.profile_enable(h, True)
+    # ---- timed region: K steps, device-resident input, measurement hooks OFF -> `value` --------------------
+    psfft.profile_enable(h, False)
     clocks = ClockSampler(local)
     dist_barrier()
     torch.cuda.synchronize()
     ms = time_loop(step, K, stream)
     torch.cuda.synchronize()
     dist_barrier()
-    psfft.profile_enable(h, False)
-    recs = psfft.profile_records(h)
     ms_max = dist_max(ms, dev)
     value = aggregate(ms_max, 1.0, world)
 
-    # ---- roofline of the dominant kernel, from the events of the timed region -------------------------
-    tot = {}
-    for name, t, b in recs:
-        a = tot.setdefault(name, [0.0, 0.0, 0])
-        a[0] += t; a[1] += b; a[2] += 1
-    dom = max(tot, key=lambda k: tot[k][0])
-    peak, peak_src = hbm_peak()
-    achieved = tot[dom][1] / (tot[dom][0] * 1e-3) / 1e9
+    # ---- the same K steps again with the per-launch CUDA events of the library ON -> roofline ------------
+    psfft.profile_reset(h)
+    psfft.profile_enable(h, True)
+    torch.cuda.synchronize()
+    ms_prof = time_loop(step, K, stream)
+    torch.cuda.synchronize()
+    psfft.profile_enable(h, False)
+    recs = psfft.profile_records(h)
     spec_bytes = plan.layout.spec_bytes
-    step_bytes = 42.0 * spec_bytes
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
-                "launches_timed": tot[dom][2], "avg_launch_ms": tot[dom][0] / tot[dom][2],
-                "algorithmic_bytes_per_launch": tot[dom][1] / tot[dom][2],
-                "kernel_share_of_step": tot[dom][0] / sum(v[0] for v in tot.values()),
-                "per_kernel": {k: {"ms_per_step": v[0] / K, "GBps": v[1] / (v[0] * 1e-3) / 1e9, "launches_per_step": v[2] / K}
-                               for k, v in tot.items()},
-                "step_model": {"algorithmic_bytes": step_bytes, "model": "fused 3-pass HD RHS = 42 C (SURVEY.md §8(a))",
-                               "GBps": step_bytes / (ms_max * 1e-3) / 1e9, "frac": step_bytes / (ms_max * 1e-3) / 1e9 / peak}}
+    roofline = roofline_of(recs, K, ms_max, 42.0 * spec_bytes, "fused 3-pass HD RHS = 42 C (SURVEY.md §8(a))", peak,
+                           f"{N}^3 fp64")
+    roofline["peak_source"] = peak_src
+    roofline["ms_per_step_with_event_hooks"] = ms_prof
 
     # ---- end to end through the C ABI with HOST buffers (H2D + kernels + D2H per step) ----------------
     d_in, d_out = torch.empty_like(uh), torch.empty_like(uh)
@@ -372,17 +568,8 @@ def run_ours(args) -> int:
                                  "workload": f"{N}^3 fp64, psi = p + i q as two real fields, alpha = 0.3, beta = 1"}}
         del th, rt
 
-    if rank != 0:
-        return 0
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": workload_config(N, world), "clocks": clk, "e2e": e2e,
-            "gpu_launches": launches_per_step * K, "launches_per_step": launches_per_step,
+    return {"value": value, "ms_max": ms_max, "clk": clk, "e2e": e2e, "launches_per_step": launches_per_step,
             "roofline": roofline, "fft3d": fft3d, "next_rows": next_rows}
-    if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = cpu_baseline(N)
-    print(json.dumps(line), flush=True)
-    return 0
 
 
 def main() -> int:
@@ -393,6 +580,9 @@ def main() -> int:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--N", type=int, default=512, help="grid size (the metric is quoted at 512)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configs (768^3, 1024^3 ...)")
+    ap.add_argument("--reference-budget-s", type=float, default=150.0,
+                    help="--impl reference: cap on the oracle time of the whole arm (full-size evaluations)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -24,8 +24,12 @@
  *   Memory   "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  The caller owns
  *            every buffer (inputs, outputs, workspace, tables); the library never allocates or
  *            frees device memory.  Device pointers must be 16-byte aligned (256 recommended).
+ *            (16 bytes is what the widest vector access of the kernels needs and what the fields inside a
+ *            multi-field array are aligned to: ldk*N*N*2s is in general not a multiple of 256.)
  *            Inputs are never modified.  Input and output of one call must not overlap; the
- *            workspace must overlap neither.
+ *            workspace must overlap neither: every execute call checks the byte ranges it will touch
+ *            (sizes from the plan's layout) and returns PSFFT_E_OVERLAP before enqueuing anything.
+ *            Inputs may alias one another.  The workspace SIZE cannot be checked (the ABI passes no size).
  *   Streams  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Execute
  *            calls only enqueue work and return without synchronising; they are CUDA-graph
  *            capturable.  A plan may be used on one stream at a time.
@@ -52,7 +56,8 @@ extern "C" {
 #define PSFFT_E_ALIGN (-4)       /* a device pointer is not 16-byte aligned */
 #define PSFFT_E_TABLE (-5)       /* table buffer smaller than layout.table_bytes */
 #define PSFFT_E_PLAN (-6)        /* invalid or destroyed plan handle */
-#define PSFFT_E_BATCH (-7)       /* call needs more fields than the plan's batch provides workspace for */
+#define PSFFT_E_BATCH (-7)       /* batch * Nz exceeds 65535 (grid limit of the y-pass) */
+#define PSFFT_E_OVERLAP (-8)     /* an output or workspace range of the call overlaps another range of the call */
 
 typedef struct psfft_plan_s *psfft_plan;
 
@@ -179,7 +184,7 @@ int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alp
  *   ord       1..4 stages
  *   params    HOST pointer to 3 doubles: { nu, eta (MHD) or kappa (Boussinesq), N_bv }
  *   d_work         >= psfft_rk_work_bytes(plan, system) = one state-sized stage buffer + the RHS workspace
- * Returns PSFFT_E_SIZE for a bad system / ord or d_y_in == d_y_out. */
+ * Returns PSFFT_E_SIZE for a bad system / ord, PSFFT_E_OVERLAP when d_y_in, d_y_out, d_work overlap. */
 #define PSFFT_SYS_HD 0
 #define PSFFT_SYS_MHD 1
 #define PSFFT_SYS_BOUSSINESQ 2

@@ -27,8 +27,8 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def _flags() -> str:
-    return " ".join(NVCC_FLAGS[:6] + os.environ.get("PSFFT_NVCC_EXTRA", "").split())
+def _flags(extra=()) -> str:
+    return " ".join(NVCC_FLAGS[:6] + list(extra))
 
 
 def _stamp() -> str:
@@ -46,15 +46,17 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile the translation units in parallel and link libpsfft.so.  Returns its path."""
+def build_library(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
+    """Compile the translation units in parallel and link libpsfft.so.  Returns its path.
+    extra_flags: additional nvcc flags of a development build (recorded in the stamp, so the next plain call
+    rebuilds the product library); the product is always built with NVCC_FLAGS alone."""
     if not force and not _stale():
         return LIB
     nvcc = _nvcc()
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("PSFFT_NVCC_EXTRA", "").split()
+    extra += list(extra_flags)
 
     def compile_one(src: str) -> str:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
@@ -70,7 +72,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         objs = list(ex.map(compile_one, SOURCES))
     subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
     with open(_stamp(), "w") as f:
-        f.write(_flags())
+        f.write(_flags(extra_flags))
     return LIB
 
 

@@ -5,7 +5,10 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <initializer_list>
+#include <mutex>
 #include <new>
+#include <unordered_set>
 #include <vector>
 
 #include "../../include/psfft.h"
@@ -118,6 +121,8 @@ int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
     if (!o) return PSFFT_E_NULL;
     if (dtype != PSFFT_F32 && dtype != PSFFT_F64) return PSFFT_E_DTYPE;
     if (!supported_n(N) || !supported_n(Ny) || !supported_n(Nz) || batch < 1) return PSFFT_E_SIZE;
+    // the y-pass puts (z plane, field) on gridDim.y (<= 65535)
+    if ((long)batch * Nz > 65535) return PSFFT_E_BATCH;
     const size_t s = dtype == PSFFT_F64 ? 8 : 4;
     memset(o, 0, sizeof(*o));
     o->N = N;
@@ -145,10 +150,39 @@ int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
 inline bool cubic(const psfft_layout &l) { return l.Ny == l.N && l.Nz == l.N; }
 inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
+// Live plans.  A handle is looked up here before it is dereferenced, so a destroyed or made-up handle is
+// answered with PSFFT_E_PLAN instead of a read through a dangling pointer.
+std::mutex g_plans_mu;
+std::unordered_set<const Plan *> g_plans;
+
 Plan *get(psfft_plan p)
 {
     Plan *pl = reinterpret_cast<Plan *>(p);
-    return (pl && pl->magic == PLAN_MAGIC) ? pl : nullptr;
+    if (!pl) return nullptr;
+    std::lock_guard<std::mutex> lock(g_plans_mu);
+    return g_plans.count(pl) ? pl : nullptr;
+}
+
+// "Input and output of one call must not overlap; the workspace must overlap neither" (psfft.h): byte ranges
+// of the call, checked on the host before anything is enqueued.  Inputs may alias one another (they are only
+// read); every written range (outputs, workspace) must be disjoint from every other range.
+struct Span {
+    const void *p;
+    size_t n;
+    bool written;
+};
+bool spans_overlap(std::initializer_list<Span> spans)
+{
+    for (const Span *a = spans.begin(); a != spans.end(); ++a) {
+        if (!a->p || !a->n) continue;
+        const uintptr_t a0 = reinterpret_cast<uintptr_t>(a->p), a1 = a0 + a->n;
+        for (const Span *b = a + 1; b != spans.end(); ++b) {
+            if (!b->p || !b->n || !(a->written || b->written)) continue;
+            const uintptr_t b0 = reinterpret_cast<uintptr_t>(b->p), b1 = b0 + b->n;
+            if (a0 < b1 && b0 < a1) return true;
+        }
+    }
+    return false;
 }
 
 PassArgs args_of(const Plan *pl, void *stream)
@@ -414,6 +448,10 @@ int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int b
         pl->n_disc = nd;
         pl->n_sphere = ns;
     }
+    {
+        std::lock_guard<std::mutex> lock(g_plans_mu);
+        g_plans.insert(pl);
+    }
     *plan = reinterpret_cast<psfft_plan>(pl);
     return PSFFT_OK;
 }
@@ -422,6 +460,10 @@ int psfft_plan_destroy(psfft_plan plan)
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
+    {
+        std::lock_guard<std::mutex> lock(g_plans_mu);
+        g_plans.erase(pl);
+    }
     pl->magic = 0;
     for (ProfRec &r : pl->recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
     for (cudaEvent_t e : pl->pool) cudaEventDestroy(e);
@@ -445,6 +487,8 @@ int psfft_fft3d_r2c(psfft_plan plan, const void *d_real, void *d_spec, void *d_w
     if (!pl) return PSFFT_E_PLAN;
     if (!d_real || !d_spec) return PSFFT_E_NULL;
     if (misaligned(d_real) || misaligned(d_spec)) return PSFFT_E_ALIGN;
+    if (spans_overlap({{d_real, pl->lay.batch * pl->lay.real_bytes, false}, {d_spec, pl->lay.batch * pl->lay.spec_bytes, true}}))
+        return PSFFT_E_OVERLAP;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     return pl->lay.dtype == PSFFT_F64 ? r2c_fields<double>(pl, a, d_real, d_spec, pl->lay.batch)
@@ -457,6 +501,9 @@ int psfft_fft3d_c2r(psfft_plan plan, const void *d_spec, void *d_real, void *d_w
     if (!pl) return PSFFT_E_PLAN;
     if (!d_real || !d_spec || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_real) || misaligned(d_spec) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    if (spans_overlap({{d_spec, pl->lay.batch * pl->lay.spec_bytes, false}, {d_real, pl->lay.batch * pl->lay.real_bytes, true},
+                       {d_work, pl->lay.work_bytes_fft, true}}))
+        return PSFFT_E_OVERLAP;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     return pl->lay.dtype == PSFFT_F64 ? c2r_fields_inplace<double>(pl, a, d_spec, d_work, d_real, pl->lay.batch)
@@ -470,6 +517,11 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
     if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_uhat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    {
+        const size_t C = pl->lay.spec_bytes;
+        if (spans_overlap({{d_uhat, 3 * C, false}, {d_rhs, 3 * C, true}, {d_work, pl->lay.work_bytes_hd, true}}))
+            return PSFFT_E_OVERLAP;
+    }
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     if (fused) {
@@ -490,6 +542,12 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
     if (!d_uhat || !d_bhat || !d_rhs_u || !d_rhs_b || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_bhat) || misaligned(d_rhs_u) || misaligned(d_rhs_b) || misaligned(d_work))
         return PSFFT_E_ALIGN;
+    {
+        const size_t C = pl->lay.spec_bytes;
+        if (spans_overlap({{d_uhat, 3 * C, false}, {d_bhat, 3 * C, false}, {d_rhs_u, 3 * C, true}, {d_rhs_b, 3 * C, true},
+                           {d_work, pl->lay.work_bytes_mhd, true}}))
+            return PSFFT_E_OVERLAP;
+    }
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     if (fused) {
@@ -532,6 +590,12 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
     if (!d_uhat || !d_thhat || !d_rhs_u || !d_rhs_th || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_thhat) || misaligned(d_rhs_u) || misaligned(d_rhs_th) || misaligned(d_work))
         return PSFFT_E_ALIGN;
+    {
+        const size_t C = pl->lay.spec_bytes;
+        if (spans_overlap({{d_uhat, 3 * C, false}, {d_thhat, C, false}, {d_rhs_u, 3 * C, true}, {d_rhs_th, C, true},
+                           {d_work, pl->lay.work_bytes_boussinesq, true}}))
+            return PSFFT_E_OVERLAP;
+    }
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     const RhsSys y = {1, 1, d_uhat, nullptr, d_thhat, d_rhs_u, nullptr, d_rhs_th, nu, 0.0, kappa, nbv,
@@ -547,6 +611,9 @@ int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alp
     if (!cubic(pl->lay)) return PSFFT_E_SIZE;
     if (!d_psihat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_psihat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
+    if (spans_overlap({{d_psihat, 2 * pl->lay.spec_bytes, false}, {d_rhs, 2 * pl->lay.spec_bytes, true},
+                       {d_work, pl->lay.work_bytes_gpe, true}}))
+        return PSFFT_E_OVERLAP;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     return pl->lay.dtype == PSFFT_F64 ? gpe_t<double>(pl, a, d_psihat, d_rhs, alpha, beta, nullptr, 0.0, false, d_work)
@@ -572,12 +639,15 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
     if (!pl) return PSFFT_E_PLAN;
     if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_y_in || !d_y_out || !d_work || !params) return PSFFT_E_NULL;
-    if (system < 0 || system > 3 || ord < 1 || ord > 4 || d_y_in == d_y_out) return PSFFT_E_SIZE;
+    if (system < 0 || system > 3 || ord < 1 || ord > 4) return PSFFT_E_SIZE;
     if (misaligned(d_y_in) || misaligned(d_y_out) || misaligned(d_work)) return PSFFT_E_ALIGN;
-    pl->launches = 0;
-    PassArgs a = args_of(pl, stream);
     const size_t C = pl->lay.spec_bytes;
     const int nfields = sys_fields(system);
+    if (spans_overlap({{d_y_in, nfields * C, false}, {d_y_out, nfields * C, true},
+                       {d_work, psfft_rk_work_bytes(plan, system), true}}))
+        return PSFFT_E_OVERLAP;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
     void *stage = d_work;                                  // one state-sized stage buffer
     void *rhswork = off(d_work, (size_t)nfields * C);
     const void *cur = d_y_in;
@@ -721,7 +791,8 @@ const char *psfft_strerror(int code)
         case PSFFT_E_ALIGN: return "psfft: device pointer not 16-byte aligned";
         case PSFFT_E_TABLE: return "psfft: table buffer too small";
         case PSFFT_E_PLAN: return "psfft: invalid plan handle";
-        case PSFFT_E_BATCH: return "psfft: plan batch too small for this call";
+        case PSFFT_E_BATCH: return "psfft: batch too large (batch * Nz must not exceed 65535)";
+        case PSFFT_E_OVERLAP: return "psfft: input, output and workspace ranges of a call must not overlap";
     }
     if (code > 0) return cudaGetErrorString((cudaError_t)code);
     return "psfft: unknown error code";

@@ -246,6 +246,21 @@ def version() -> str:
 
 # ---- convenience: a plan that owns its torch-allocated tables and workspace -----------------------
 
+def _on_plan_device(method):
+    """Plan methods run with the plan's device current (so that the stream resolved for the launch and every
+    buffer the method allocates belong to it) and refuse tensors that live elsewhere."""
+    import functools
+
+    @functools.wraps(method)
+    def wrapper(self, *args, **kwargs):
+        for t in list(args) + list(kwargs.values()):
+            if isinstance(t, torch.Tensor) and t.device != self.device:
+                raise PsfftError(f"tensor on {t.device}, plan on {self.device}")
+        with torch.cuda.device(self.device):
+            return method(self, *args, **kwargs)
+    return wrapper
+
+
 class Plan:
     """Plan + its caller-owned device buffers (allocated with torch; the library allocates nothing).
 
@@ -259,6 +274,8 @@ class Plan:
         if not torch.cuda.is_available():
             raise PsfftError("no CUDA device: libpsfft has no CPU fallback")
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self.rdtype = dtype
         self.cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
         code = F64 if dtype == torch.float64 else F32
@@ -273,6 +290,7 @@ class Plan:
         self._work_kind = None
         self.ensure_work(work)
 
+    @_on_plan_device
     def ensure_work(self, kind: str):
         need = {"fft": self.layout.work_bytes_fft, "hd": self.layout.work_bytes_hd,
                 "mhd": self.layout.work_bytes_mhd, "boussinesq": self.layout.work_bytes_boussinesq,
@@ -299,6 +317,7 @@ class Plan:
     def spec_shape(self, fields: int):
         return (fields, self.Nz, self.Ny, self.ldk)
 
+    @_on_plan_device
     def r2c(self, real: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         assert real.is_cuda and real.dtype == self.rdtype and real.is_contiguous()
         assert real.numel() == self.batch * self.layout.real_elems
@@ -307,6 +326,7 @@ class Plan:
         fft3d_r2c(self.handle, real, out, self.ensure_work("fft"))
         return out
 
+    @_on_plan_device
     def c2r(self, spec: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         assert spec.is_cuda and spec.dtype == self.cdtype and spec.is_contiguous()
         assert spec.numel() == self.batch * self.layout.spec_elems
@@ -315,6 +335,7 @@ class Plan:
         fft3d_c2r(self.handle, spec, out, self.ensure_work("fft"))
         return out
 
+    @_on_plan_device
     def hd_rhs(self, uhat: torch.Tensor, nu: float = 0.0, out: torch.Tensor | None = None) -> torch.Tensor:
         assert uhat.is_cuda and uhat.dtype == self.cdtype and uhat.is_contiguous()
         assert tuple(uhat.shape) == self.spec_shape(3)
@@ -323,6 +344,7 @@ class Plan:
         hd_rhs(self.handle, uhat, out, nu, self.ensure_work("hd"))
         return out
 
+    @_on_plan_device
     def mhd_rhs(self, uhat: torch.Tensor, bhat: torch.Tensor, nu: float = 0.0, eta: float = 0.0):
         for t in (uhat, bhat):
             assert t.is_cuda and t.dtype == self.cdtype and t.is_contiguous() and tuple(t.shape) == self.spec_shape(3)
@@ -330,6 +352,7 @@ class Plan:
         mhd_rhs(self.handle, uhat, bhat, ru, rb, nu, eta, self.ensure_work("mhd"))
         return ru, rb
 
+    @_on_plan_device
     def boussinesq_rhs(self, uhat: torch.Tensor, thhat: torch.Tensor, nu: float = 0.0, kappa: float = 0.0,
                        nbv: float = 0.0):
         assert uhat.is_cuda and uhat.dtype == self.cdtype and uhat.is_contiguous()
@@ -339,6 +362,7 @@ class Plan:
         boussinesq_rhs(self.handle, uhat, thhat, ru, rt, nu, kappa, nbv, self.ensure_work("boussinesq"))
         return ru, rt
 
+    @_on_plan_device
     def rk_step(self, system: int, y: torch.Tensor, ord: int, dt: float, nu: float = 0.0, c2: float = 0.0,
                 nbv: float = 0.0, out: torch.Tensor | None = None) -> torch.Tensor:
         """One Runge-Kutta step; y: [3 | 6 | 4, N, N, N/2+1] complex (HD | MHD u,b | Boussinesq u,theta)."""
@@ -352,6 +376,7 @@ class Plan:
         rk_step(self.handle, system, y, out, ord, dt, (nu, c2, nbv), work)
         return out
 
+    @_on_plan_device
     def gpe_rhs(self, psihat: torch.Tensor, alpha: float, beta: float) -> torch.Tensor:
         """psihat: [2, N, N, N/2+1] = (p^, q^) of psi = p + i q."""
         assert psihat.is_cuda and psihat.dtype == self.cdtype and psihat.is_contiguous()

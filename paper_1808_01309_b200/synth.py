@@ -12,6 +12,9 @@ define the synthetic stand-ins generated here:
                               (BASELINE.json configs 1 and 3).
 * ``solenoidal_spectrum``  -- 3-component divergence-free random-phase field with
                               E(k) ~ k^4 exp(-2 (k/k0)^2), unit energy (configs 2, 4, 5).
+* ``broadband_spectrum`` / ``broadband_scalar`` -- the same construction with a power-law shell
+                              spectrum filled to the Nyquist planes (developed-turbulence stand-in; the
+                              full-size parity inputs).
 * ``taylor_green`` / ``abc_flow`` / ``single_mode`` -- closed-form physical-space fields
                               used by the oracle's pins.
 
@@ -128,13 +131,29 @@ def solenoidal_spectrum(N: int, k0: float = 4.0, kcut: int | None = None, seed: 
         kcut = int(8 * k0)
     if kcut >= N // 2:
         raise ValueError("kcut must be below the Nyquist wavenumber")
-    kx, ky, kz, a = solenoidal_coefficients(k0, kcut, seed, tag)
+    iz, iy, ix, v = solenoidal_modes(N, k0, kcut, seed, tag)
     u = np.zeros((3, N, N, N // 2 + 1), dtype=np.complex128)
-    scale = float(N) ** 3
-    u[:, kz % N, ky % N, kx] = a * scale
-    on0 = kx == 0
-    u[:, (-kz[on0]) % N, (-ky[on0]) % N, 0] = np.conj(a[:, on0]) * scale
+    u[:, iz, iy, ix] = v
     return u.astype(dtype)
+
+
+def solenoidal_modes(N: int, k0: float = 4.0, kcut: int | None = None, seed: int = 1234, tag: int = 0):
+    """The non-zero entries of ``solenoidal_spectrum`` as a list: indices ``(iz, iy, ix)`` into
+    ``[kz][ky][kx]`` and values ``v[3, n]`` (= N^3 a_k, conjugate partners of the kx = 0 plane included).
+    For callers that scatter the few thousand modes into a zero-initialised DEVICE array instead of building
+    the dense host array (bench.py at 1024^3)."""
+    if kcut is None:
+        kcut = int(8 * k0)
+    if kcut >= N // 2:
+        raise ValueError("kcut must be below the Nyquist wavenumber")
+    kx, ky, kz, a = solenoidal_coefficients(k0, kcut, seed, tag)
+    scale = float(N) ** 3
+    on0 = kx == 0
+    iz = np.concatenate([kz % N, (-kz[on0]) % N])
+    iy = np.concatenate([ky % N, (-ky[on0]) % N])
+    ix = np.concatenate([kx, np.zeros(int(on0.sum()), dtype=kx.dtype)])
+    v = np.concatenate([a * scale, np.conj(a[:, on0]) * scale], axis=1)
+    return iz, iy, ix, v
 
 
 def scalar_coefficients(k0: float, kcut: int, seed: int = 1234, tag: int = 7):
@@ -171,6 +190,100 @@ def scalar_spectrum(N: int, k0: float = 4.0, kcut: int | None = None, seed: int 
     return t.astype(dtype)
 
 
+def _shell_amplitude(k2: np.ndarray, slope: float) -> np.ndarray:
+    """Per-mode amplitude of a power-law shell spectrum E(k) ~ k^slope: sqrt(E(k) / (4 pi k^2))."""
+    return np.sqrt(k2 ** (0.5 * slope) / (4.0 * np.pi * k2))
+
+
+def _canonical_plane(kx: int, kcut: int):
+    """Canonical wavevectors (kx, ky, kz) of one kx plane with 1 <= |k| <= kcut (see solenoidal_coefficients)."""
+    r = np.arange(-kcut, kcut + 1)
+    ky, kz = np.meshgrid(r, r, indexing="ij")
+    ky, kz = ky.ravel(), kz.ravel()
+    k2 = kx * kx + ky * ky + kz * kz
+    canon = (kx > 0) | ((ky > 0) | ((ky == 0) & (kz > 0)))
+    sel = canon & (k2 >= 1) & (k2 <= kcut * kcut)
+    return np.full(int(sel.sum()), kx), ky[sel], kz[sel], k2[sel].astype(np.float64)
+
+
+def _map_planes(fn, n: int) -> list:
+    """fn(0..n-1) on a small thread pool (numpy releases the GIL; the planes write disjoint slices).  The
+    results come back in plane order, so sums over them do not depend on the scheduling."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    workers = max(1, min(16, os.cpu_count() or 1))
+    if workers == 1 or n < 8:
+        return [fn(i) for i in range(n)]
+    with ThreadPoolExecutor(workers) as ex:
+        return list(ex.map(fn, range(n)))
+
+
+def broadband_spectrum(N: int, slope: float = -5.0 / 3.0, kcut: int | None = None, seed: int = 1234, tag: int = 0,
+                       dtype=np.complex128) -> np.ndarray:
+    """Half spectrum ``uhat[3][kz][ky][kx]`` of a random-phase solenoidal field whose shell spectrum is the
+    power law E(k) ~ k^slope on 1 <= |k| <= kcut (default: N/2 - 1, every shell below the Nyquist planes), unit
+    energy.  The stand-in for a developed turbulent state (the paper's production runs):
+    every mode of the 2/3-rule sphere carries an O(1) share of its shell, and modes OUTSIDE the sphere are
+    populated too, so the input mask, the pruned column ranges and the outermost retained shell all see data.
+    Same per-wavevector keys and polarisation construction as ``solenoidal_spectrum`` (grid independent);
+    generated one kx plane at a time so that 1024^3 stays within a few GB of host memory."""
+    if kcut is None:
+        kcut = N // 2 - 1
+    if kcut >= N // 2:
+        raise ValueError("kcut must be below the Nyquist wavenumber")
+    u = np.zeros((3, N, N, N // 2 + 1), dtype=dtype)
+
+    def plane(kx0: int) -> float:
+        kx, ky, kz, k2 = _canonical_plane(kx0, kcut)
+        if kx.size == 0:
+            return 0.0
+        kk = np.sqrt(k2)
+        key = _key(seed, tag, kx, ky, kz)
+        th1 = 2.0 * np.pi * _variate(key, 0)
+        th2 = 2.0 * np.pi * _variate(key, 1)
+        phi = 2.0 * np.pi * _variate(key, 2)
+        kh = np.sqrt((kx * kx + ky * ky).astype(np.float64))
+        axis = kh == 0
+        khs = np.where(axis, 1.0, kh)
+        e1 = np.stack([np.where(axis, 1.0, ky / khs), np.where(axis, 0.0, -kx / khs), np.zeros_like(kk)])
+        e2 = np.cross(np.stack([kx, ky, kz]).astype(np.float64), e1, axis=0) / kk
+        a = _shell_amplitude(k2, slope) * (np.cos(phi) * np.exp(1j * th1) * e1 + np.sin(phi) * np.exp(1j * th2) * e2)
+        u[:, kz % N, ky % N, kx0] = a
+        if kx0 == 0:
+            u[:, (-kz) % N, (-ky) % N, 0] = np.conj(a)
+        return float(np.sum(np.abs(a) ** 2))
+
+    energy = sum(_map_planes(plane, kcut + 1))
+    u *= np.asarray(float(N) ** 3 / np.sqrt(energy)).astype(u.real.dtype)
+    return u
+
+
+def broadband_scalar(N: int, slope: float = -5.0 / 3.0, kcut: int | None = None, seed: int = 1234, tag: int = 7,
+                     dtype=np.complex128) -> np.ndarray:
+    """Half spectrum ``thhat[kz][ky][kx]`` of a random-phase real scalar field with the power-law shell
+    spectrum of ``broadband_spectrum`` (one uniform phase per canonical wavevector), unit variance-energy."""
+    if kcut is None:
+        kcut = N // 2 - 1
+    if kcut >= N // 2:
+        raise ValueError("kcut must be below the Nyquist wavenumber")
+    t = np.zeros((N, N, N // 2 + 1), dtype=dtype)
+
+    def plane(kx0: int) -> float:
+        kx, ky, kz, k2 = _canonical_plane(kx0, kcut)
+        if kx.size == 0:
+            return 0.0
+        ph = 2.0 * np.pi * _variate(_key(seed, tag, kx, ky, kz), 0)
+        a = _shell_amplitude(k2, slope) * np.exp(1j * ph)
+        t[kz % N, ky % N, kx0] = a
+        if kx0 == 0:
+            t[(-kz) % N, (-ky) % N, 0] = np.conj(a)
+        return float(np.sum(np.abs(a) ** 2))
+
+    energy = sum(_map_planes(plane, kcut + 1))
+    t *= np.asarray(float(N) ** 3 / np.sqrt(energy)).astype(t.real.dtype)
+    return t
+
+
 def grid_axes(N: int):
     """Physical coordinates X_i = 2 pi i / N as broadcastable [z][y][x] arrays (returns x, y, z)."""
     t = 2.0 * np.pi * np.arange(N) / N
@@ -183,6 +296,20 @@ def taylor_green(N: int) -> np.ndarray:
     u = np.zeros((3, N, N, N))
     u[0] = np.sin(x) * np.cos(y) * np.cos(z)
     u[1] = -np.cos(x) * np.sin(y) * np.cos(z)
+    return u
+
+
+def taylor_green_spectrum(N: int, m: int = 1, dtype=np.complex128) -> np.ndarray:
+    """Half spectrum (= N^3 x Fourier coefficient) of the Taylor-Green vortex at wavenumber m,
+    u = (sin mx cos my cos mz, -cos mx sin my cos mz, 0), written down mode by mode (no transform): eight
+    entries, u^_x[+-m][+-m][m] = -i N^3/8 and u^_y[+-m][s m][m] = i s N^3/8.  Needs no N^3 physical array, so the
+    closed-form pin reaches the last retained shell of the large grids."""
+    u = np.zeros((3, N, N, N // 2 + 1), dtype=dtype)
+    a = float(N) ** 3 / 8.0
+    for kz in (m, N - m):
+        for ky, sy in ((m, 1.0), (N - m, -1.0)):
+            u[0, kz, ky, m] = -1j * a
+            u[1, kz, ky, m] = 1j * sy * a
     return u
 
 

@@ -28,6 +28,14 @@ def main():
         for (c, r, q, p) in [(0, 1, 2, 3), (1, 127, 5, 0), (2, 3, 126, 7)]:
             v = u[c, r, q, p]
             f.write(f"solenoidal 128 4.0 32 1234 0 {c} {r} {q} {p} {float(v.real)!r} {float(v.imag)!r}\n")
+        u = synth.broadband_spectrum(64, seed=1234, tag=0)
+        for (c, r, q, p) in [(0, 1, 2, 3), (1, 63, 5, 0), (2, 50, 10, 20)]:
+            v = u[c, r, q, p]
+            f.write(f"broadband 64 1234 0 {c} {r} {q} {p} {float(v.real)!r} {float(v.imag)!r}\n")
+        t = synth.broadband_scalar(64, seed=1234)
+        for (r, q, p) in [(1, 2, 3), (63, 5, 0)]:
+            v = t[r, q, p]
+            f.write(f"broadband_scalar 64 1234 7 {r} {q} {p} {float(v.real)!r} {float(v.imag)!r}\n")
     print("wrote", out)
 
 

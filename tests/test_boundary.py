@@ -53,12 +53,26 @@ def test_error_codes(lib):
     assert lib.psfft_plan_create(ctypes.byref(h), 64, psfft.F64, 1, ctypes.c_void_p(0x1000), 8, None) == -5
     assert lib.psfft_plan_destroy(None) == -6
     assert lib.psfft_fft3d_r2c(None, None, None, None, None) == -6
-    for code in (0, -1, -2, -3, -4, -5, -6, -7):
+    assert lib.psfft_plan_query(1024, psfft.F64, 64, ctypes.byref(lay)) == -7   # batch * Nz > 65535 (y-pass grid)
+    assert lib.psfft_plan_query(1024, psfft.F64, 63, ctypes.byref(lay)) == 0
+    for code in (0, -1, -2, -3, -4, -5, -6, -7, -8):
         assert psfft.strerror(code)
+    assert "overlap" in psfft.strerror(-8)
     assert "psfft" in psfft.strerror(-2)
     with pytest.raises(psfft.PsfftError):
         psfft.plan_query(10, psfft.F64, 1)
     assert psfft.version() == "0.1"
+
+
+def test_stale_and_invented_handles_are_rejected_without_dereferencing(lib):
+    """Handles are looked up in the library's registry of live plans: an address that was never a plan (here:
+    unmapped memory, which a read of a magic word would fault on) is answered with PSFFT_E_PLAN."""
+    lay = psfft.Layout()
+    for bogus in (0x10, 0xDEAD0000, 0x7FFFFFFFF000):
+        assert lib.psfft_plan_layout(ctypes.c_void_p(bogus), ctypes.byref(lay)) == -6
+        assert lib.psfft_plan_destroy(ctypes.c_void_p(bogus)) == -6
+        assert lib.psfft_hd_rhs(ctypes.c_void_p(bogus), None, None, 0.0, None, None) == -6
+        assert lib.psfft_last_launch_count(ctypes.c_void_p(bogus)) == -6
 
 
 def test_every_supported_size_is_accepted(lib):

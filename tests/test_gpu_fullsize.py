@@ -3,10 +3,18 @@
 * 512^3 fp64 (configs[2] and the metric's HD RHS): the oracle is fast enough on the GPU box's host cores
   for a full element-by-element comparison; sampled O(N^3)-per-mode brute-force sums pin the transform
   independently of the oracle's FFT.
-* 768^3 fp32 (configs[3]) and 1024^3 fp32 MHD (configs[4]): a full-size fp64 oracle does not fit / takes
-  minutes, so parity uses the grid-independence property P12: the same band-limited
-  coefficients on a 256^3 grid give the same right-hand-side coefficients mode by mode, and everything
-  outside that box must vanish -- plus conservation invariants and the fused-vs-unfused cross-check.
+* 768^3 fp32 (configs[3]) and 1024^3 fp32 MHD (configs[4]) on the configs' own band-limited fields: parity uses
+  the grid-independence property P12: the same band-limited coefficients on a 256^3 grid
+  give the same right-hand-side coefficients mode by mode, and everything outside that box must vanish --
+  plus conservation invariants and the fused-vs-unfused cross-check.
+* FULL-SPHERE inputs (second half of this file).  The configs' fields fill < 1 % of the retained sphere at these
+  sizes, so on them the pruned column ranges, the compact kx pitch and the large-N tile policies only ever
+  move zeros in the outer shells.  Every full size therefore also runs (a) a broadband field -- power-law shell
+  spectrum filled to the Nyquist planes, synth.broadband_spectrum -- against the oracle element by element with
+  a PER-SHELL error bound (512^3 fp64, 768^3 fp32; the GPU box has 196 GB of host memory) or, at 1024^3, fused
+  against unfused after the unfused path's transforms have been oracle-checked at that size; (b) the Taylor-Green
+  closed form at a wavenumber m whose output lands in the LAST retained shell (9 * 8 m^2 < N^2); (c) the plain
+  transforms against the oracle at 768^3, 1024^3 and on the paper's 1024 x 1024 x 256 box.
 """
 import numpy as np
 import pytest
@@ -15,6 +23,7 @@ torch = pytest.importorskip("torch")
 
 import oracle  # noqa: E402
 from paper_1808_01309_b200 import psfft, synth  # noqa: E402
+from parity_util import assert_shells, assert_shells_device  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -230,3 +239,176 @@ def test_gpe_rhs_512_fp64():
     got = p.gpe_rhs(torch.from_numpy(y).cuda(), alpha, beta).cpu().numpy()
     assert box_compare(got, N, oracle.gpe_rhs(g, alpha, beta), 256, 72) < 1e-12
     assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+
+
+# =========================================================================================================
+# Full-sphere parity: inputs that populate every retained mode (and the modes the input mask must remove)
+# =========================================================================================================
+
+def free_device_memory():
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    return torch.cuda.mem_get_info()[0]
+
+
+def test_hd_rhs_512_fp64_full_sphere():
+    """The metric's kernel configuration on a developed-turbulence stand-in: E(k) ~ k^-5/3 on 1 <= |k| <= 255, so
+    every one of the 10.5 M retained half-spectrum modes is non-zero on input and on output and the modes between
+    the sphere and the Nyquist planes (which step 1 must remove) carry energy too.  Element by element against the
+    full-size oracle, shell by shell."""
+    N = 512
+    uh = synth.broadband_spectrum(N, seed=1234)
+    M = oracle.dealias_mask(N)
+    assert np.count_nonzero(uh[0][M]) > 0.99 * M.sum() and np.count_nonzero(uh[0][~M]) > 0.2 * (~M).sum()
+    p = psfft.Plan(N, torch.float64, 3, work="hd")
+    got = p.hd_rhs(torch.from_numpy(uh).cuda(), 0.0).cpu().numpy()
+    want = oracle.hd_rhs(uh, 0.0)
+    assert np.count_nonzero(want[0][M]) > 0.99 * M.sum()
+    assert rel(got, want) < 1e-12
+    assert assert_shells(got, want, N, 1e-12) < 1e-12
+    assert np.all(got[:, ~M] == 0)                                                   # mask bit-exact
+    assert np.count_nonzero(got[0][M]) > 0.99 * M.sum()
+    # with diffusion on (the sparse re-read of the input in the fwd_z epilogue), against the same oracle result
+    got = p.hd_rhs(torch.from_numpy(uh).cuda(), 2.5e-3).cpu().numpy()
+    K2 = (np.fft.fftfreq(N, 1.0 / N)[:, None, None] ** 2 + np.fft.fftfreq(N, 1.0 / N)[None, :, None] ** 2
+          + np.arange(N // 2 + 1)[None, None, :] ** 2)
+    want -= 2.5e-3 * K2 * (uh * M)
+    assert assert_shells(got, want, N, 1e-12) < 1e-12
+
+
+# Taylor-Green at wavenumber m: the 12 entries of tests/golden/taylor_green_rhs.txt at wavenumbers 2m, values x m
+# (u_m(x) = u_1(m x) => omega_m = m omega_1(m x), u_m x omega_m = m (u_1 x omega_1)(m x), and the projection
+# commutes with the dilation).  m is the largest integer with 9 * 8 m^2 < N^2: the output sits in the last shell.
+@pytest.mark.parametrize("N,m,dtype", [(512, 60, torch.float64), (768, 90, torch.float32), (768, 90, torch.float64),
+                                       (1024, 120, torch.float32), (1024, 120, torch.float64)])
+def test_taylor_green_at_the_sphere_edge(N, m, dtype, golden_dir):
+    assert 9 * 8 * m * m < N * N <= 9 * 8 * (m + 1) * (m + 1)
+    code = psfft.F64 if dtype == torch.float64 else psfft.F32
+    lay = psfft.plan_query(N, code, 1)
+    if free_device_memory() < lay.work_bytes_hd + 6 * lay.spec_bytes + (2 << 30):
+        pytest.skip("not enough free device memory")
+    cdt = np.complex128 if dtype == torch.float64 else np.complex64
+    p = psfft.Plan(N, dtype, 1, work="hd")
+    got = p.hd_rhs(torch.from_numpy(synth.taylor_green_spectrum(N, m, cdt)).cuda())
+    del p
+    tol = 1e-12 if dtype == torch.float64 else 2e-5
+    rows = np.loadtxt(f"{golden_dir}/taylor_green_rhs.txt")
+    assert rows.shape == (12, 6)
+    want_norm2 = 0.0
+    for c, kz, ky, kx, re, im in rows:
+        idx = (int(c), (m * int(kz)) % N, (m * int(ky)) % N, m * int(kx))
+        val = complex(re, im) * m * float(N) ** 3
+        g = complex(got[idx].item())
+        assert abs(g - val) < tol * abs(val), (idx, g, val)
+        got[idx] = 0
+        want_norm2 += abs(val) ** 2
+    # everything else is roundoff: its L2 norm against the norm of the 12 entries
+    assert float(torch.linalg.vector_norm(got.reshape(-1).to(torch.complex128 if dtype == torch.float64 else torch.complex64))) \
+        < tol * np.sqrt(want_norm2)
+    del got
+    torch.cuda.empty_cache()
+
+
+def test_hd_rhs_768_fp32_full_sphere():
+    """configs[3]'s kernels (radix-3 schedules, 48 KB tiles, the 128 KB fwd_z tile) on a full-sphere field against
+    the fp64 oracle at 768^3 itself (about 45 GiB of host memory, a minute of CPU)."""
+    N = 768
+    uh = synth.broadband_spectrum(N, seed=1234, dtype=np.complex64)
+    p = psfft.Plan(N, torch.float32, 1, work="hd")
+    got = p.hd_rhs(torch.from_numpy(uh).cuda()).cpu().numpy()
+    del p
+    torch.cuda.empty_cache()
+    want = oracle.hd_rhs(uh.astype(np.complex128), 0.0)
+    M = oracle.dealias_mask(N)
+    assert np.count_nonzero(want[0][M]) > 0.99 * M.sum()
+    assert rel(got, want) < 2e-5
+    assert assert_shells(got, want, N, 2e-5) < 2e-5
+    assert np.all(got[:, ~M] == 0)
+
+
+@pytest.mark.parametrize("shape,dtype", [((768, 768, 768), torch.float32), ((1024, 1024, 1024), torch.float32),
+                                         ((1024, 1024, 256), torch.float32), ((1024, 1024, 256), torch.float64)])
+def test_plain_transforms_at_the_large_sizes(shape, dtype):
+    """psfft_fft3d_r2c / c2r against the oracle at the supported sizes above 512^3 and on the paper's flat box
+    (Nx, Ny, Nz) = (1024, 1024, 256), uniform [-1, 1) input, one field."""
+    Nx, Ny, Nz = shape
+    rdt = np.float64 if dtype == torch.float64 else np.float32
+    tol = 1e-12 if dtype == torch.float64 else 2e-5
+    n = Nx * Ny * Nz
+    x = np.empty(n, dtype=rdt)
+    for s in range(0, n, 1 << 24):                            # synth.uniform_field's recipe on a non-cubic index space
+        e = min(n, s + (1 << 24))
+        x[s:e] = 2.0 * synth.uniform01(4321, np.arange(s, e, dtype=np.uint64), 53 if rdt == np.float64 else 24) - 1.0
+    x = x.reshape(1, Nz, Ny, Nx)
+    p = psfft.Plan(shape if Nz != Nx else Nx, dtype, 1)
+    xd = torch.from_numpy(x).cuda()
+    X = p.r2c(xd)
+    back = p.c2r(X)
+    assert float((back - xd).abs().max()) < (1e-13 if dtype == torch.float64 else 2e-6)
+    del xd
+    Xh = X.cpu().numpy()[0]
+    del X
+    want = oracle.r2c3d(x[0].astype(np.float64))
+    assert rel(Xh[None], want[None]) < tol
+    # per kz-plane error as well: a mis-transformed slab of columns cannot hide in the global norm
+    for kz in (0, 1, Nz // 3, Nz // 2, Nz - 1):
+        assert rel(Xh[kz], want[kz]) < tol
+    del Xh
+    # c2r of the ORACLE's spectrum (rounded to the plan dtype) returns the field: checks the inverse against the
+    # oracle's forward definition rather than against our own r2c
+    back = p.c2r(torch.from_numpy(want.astype(np.complex128 if dtype == torch.float64 else np.complex64)[None]).cuda())
+    assert rel(back.cpu().numpy(), x) < tol
+
+
+def test_hd_and_mhd_rhs_1024_fp32_full_sphere():
+    """configs[4]'s kernels (one 128 KB tile per SM, 1024-thread CTAs, 8 4 4 8 mid_x) on full-sphere fields: fused
+    against the unfused composition of the plain passes (oracle-checked at 1024^3 above), shell by shell, plus the
+    exact support of the mask and the P10 invariants over the whole sphere.  The comparisons run on the device
+    (3 x 537 M modes per field set)."""
+    N = 1024
+    lay = psfft.plan_query(N, psfft.F32, 1)
+    if free_device_memory() < lay.work_bytes_mhd + 12 * lay.spec_bytes + (2 << 30):
+        pytest.skip("not enough free device memory")
+    ud = torch.from_numpy(synth.broadband_spectrum(N, seed=1234, tag=0, dtype=np.complex64)).cuda()
+    bd = torch.from_numpy(synth.broadband_spectrum(N, seed=1234, tag=1, dtype=np.complex64)).cuda()
+    M = torch.from_numpy(oracle.dealias_mask(N)).cuda()
+    nM = int(M.sum())
+    p = psfft.Plan(N, torch.float32, 1, work="mhd")
+
+    def check(got, ref):
+        assert int(torch.count_nonzero(ref[0][M])) > 0.99 * nM and int(torch.count_nonzero(got[0][M])) > 0.99 * nM
+        assert assert_shells_device(got, ref, N, 2e-5) < 2e-5
+        for c in range(3):
+            assert int(torch.count_nonzero(got[c][~M])) == 0           # mask bit-exact
+
+    # HD
+    got = p.hd_rhs(ud)
+    unf = torch.empty_like(got)
+    psfft.hd_rhs_unfused(p.handle, ud, unf, 0.0, p._work)
+    check(got, unf)
+    del got, unf
+    # MHD
+    ru, rb = p.mhd_rhs(ud, bd)
+    wu, wb = torch.empty_like(ru), torch.empty_like(rb)
+    psfft.mhd_rhs_unfused(p.handle, ud, bd, wu, wb, 0.0, 0.0, p._work)
+    p.close()
+    del p
+    torch.cuda.empty_cache()
+    check(ru, wu)
+    check(rb, wb)
+    del wu, wb
+    # P10 over the full sphere: total energy and cross helicity are conserved by the truncated system
+    w = torch.from_numpy(half_weights(N)[0, 0]).cuda()
+
+    def dot(a, b):
+        t = 0.0
+        for c in range(3):
+            for z in range(0, N, 64):
+                x, y = a[c, z:z + 64].to(torch.complex128), b[c, z:z + 64].to(torch.complex128)
+                t += float(((x.real * y.real + x.imag * y.imag) * w * M[z:z + 64]).sum())
+        return t
+
+    s = np.sqrt(dot(ud, ud) * dot(ru, ru)) + np.sqrt(dot(bd, bd) * dot(rb, rb))
+    assert abs(dot(ud, ru) + dot(bd, rb)) / s < 1e-5
+    assert abs(dot(bd, ru) + dot(ud, rb)) / s < 1e-5

@@ -4,6 +4,8 @@ same seeded inputs.  Run on the B200 box:  python -m pytest tests -m gpu
 Tolerances (BASELINE.json north_star): relative L2 error <= 1e-12 (fp64), <= 2e-5 (fp32) over the whole
 output; the dealias mask bit-exact (masked outputs exactly +0).
 """
+import ctypes
+
 import numpy as np
 import pytest
 
@@ -11,6 +13,7 @@ torch = pytest.importorskip("torch")
 
 import oracle  # noqa: E402
 from paper_1808_01309_b200 import psfft, synth  # noqa: E402
+from parity_util import assert_shells  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -116,7 +119,7 @@ def test_anisotropic_plan_rejects_the_right_hand_sides():
     assert p.layout.work_bytes_hd == 0 and psfft.rk_work_bytes(p.handle, psfft.SYS_HD) == 0
     u = torch.zeros((3, 16, 32, 17), dtype=torch.complex128, device="cuda")
     with pytest.raises(psfft.PsfftError):
-        psfft.hd_rhs(p.handle, u, torch.empty_like(u), 0.0, u)
+        psfft.hd_rhs(p.handle, u, torch.empty_like(u), 0.0, torch.empty_like(u))
 
 
 def test_degenerate_inputs():
@@ -414,6 +417,71 @@ def test_gpe_rk_step_matches_oracle(N, ord, dtype):
     assert rel(got, want) < TOL[dtype]
 
 
+# ---- broadband (full-sphere) inputs: every retained mode populated, per-shell error bounds ----------------------
+# The band-limited config fields (k0 = 4, kcut = 32) leave the outer shells of the 2/3 sphere empty from N = 96 on
+# (ADVICE r1): the pruned column ranges, the kx_count / pitch edge and the mirrored loads of mid_x would then only
+# ever move zeros there.  synth.broadband_* fills E(k) ~ k^-5/3 up to the Nyquist planes.
+
+def broadband_state(system, N, dtype):
+    u = synth.broadband_spectrum(N, seed=77, tag=0)
+    if system == psfft.SYS_HD:
+        y = u
+    elif system == psfft.SYS_MHD:
+        y = np.concatenate([u, synth.broadband_spectrum(N, seed=77, tag=1)])
+    elif system == psfft.SYS_BOUSSINESQ:
+        y = np.concatenate([u, synth.broadband_scalar(N, seed=77)[None]])
+    else:
+        y = np.stack([synth.broadband_scalar(N, seed=77, tag=11), synth.broadband_scalar(N, seed=77, tag=12)])
+        y[0, 0, 0, 0] = float(N) ** 3
+    return np.ascontiguousarray(y.astype(CDT[dtype]))
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N", [128, 192, 256])
+@pytest.mark.parametrize("system", [0, 1, 2, 3])
+def test_rhs_broadband_per_shell(system, N, dtype):
+    y = broadband_state(system, N, dtype)
+    yw = y.astype(np.complex128)
+    M = oracle.dealias_mask(N)
+    assert np.count_nonzero(y[0][M]) > 0.99 * M.sum() and np.count_nonzero(y[0][~M]) > 0.2 * (~M).sum()
+    yd = dev(y)
+    p = psfft.Plan(N, dtype, 1, work="mhd")
+    if system == psfft.SYS_HD:
+        got = p.hd_rhs(yd, 0.003).cpu().numpy()
+        want = oracle.hd_rhs(yw, 0.003)
+    elif system == psfft.SYS_MHD:
+        ru, rb = p.mhd_rhs(yd[:3].contiguous(), yd[3:].contiguous(), 0.003, 0.002)
+        got = np.concatenate([ru.cpu().numpy(), rb.cpu().numpy()])
+        want = np.concatenate(oracle.mhd_rhs(yw[:3], yw[3:], 0.003, 0.002))
+    elif system == psfft.SYS_BOUSSINESQ:
+        ru, rt = p.boussinesq_rhs(yd[:3].contiguous(), yd[3].contiguous(), 0.003, 0.002, 1.5)
+        got = np.concatenate([ru.cpu().numpy(), rt.cpu().numpy()[None]])
+        wu, wt = oracle.boussinesq_rhs(yw[:3], yw[3], 0.003, 0.002, 1.5)
+        want = np.concatenate([wu, wt[None]])
+    else:
+        got = p.gpe_rhs(yd, 0.37, 1.3).cpu().numpy()
+        want = oracle.gpe_rhs(yw, 0.37, 1.3)
+    assert rel(got, want) < TOL[dtype]
+    for f in range(0, got.shape[0], 3):              # vector fields (and the scalar) separately, shell by shell
+        assert_shells(got[f:f + 3], want[f:f + 3], N, TOL[dtype])
+    assert np.all(got[:, ~M] == 0)
+    assert np.count_nonzero(got[0][M]) > 0.99 * M.sum()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("system", [0, 1, 2, 3])
+def test_rk2_broadband_per_shell(system, dtype):
+    N = 128
+    y = broadband_state(system, N, dtype)
+    p = psfft.Plan(N, dtype, 1)
+    par = (0.37, 1.3, 0.0) if system == psfft.SYS_GPE else (0.003, 0.002, 1.5)
+    got = p.rk_step(system, dev(y), 2, 0.01, *par).cpu().numpy()
+    want = oracle.rk_step(system, y.astype(np.complex128), 2, 0.01, *par)
+    assert rel(got, want) < TOL[dtype]
+    assert_shells(got, want, N, TOL[dtype])
+    assert np.all(got[:, ~oracle.dealias_mask(N)] == 0)
+
+
 # ---- host-buffer (end-to-end) entry points -----------------------------------------------------------
 
 def test_host_entry_points():
@@ -453,6 +521,44 @@ def test_unfused_rhs_matches_oracle(N, dtype):
     psfft.mhd_rhs_unfused(p.handle, du, db, ru, rb, 0.01, 0.02, p._work)
     wu, wb = oracle.mhd_rhs(uh.astype(np.complex128), bh.astype(np.complex128), 0.01, 0.02)
     assert rel(ru.cpu().numpy(), wu) < TOL[dtype] and rel(rb.cpu().numpy(), wb) < TOL[dtype]
+
+
+# ---- argument checks that need a live plan ---------------------------------------------------------------------
+
+def test_overlapping_buffers_and_dead_handles_are_rejected():
+    """psfft.h: "input and output of one call must not overlap; the workspace must overlap neither" -- every
+    execute call checks the byte ranges it will touch and returns PSFFT_E_OVERLAP (-8) before enqueuing."""
+    N = 32
+    p = psfft.Plan(N, torch.float64, 1, work="mhd")
+    C = p.layout.spec_bytes
+    buf = torch.zeros(16 * C, dtype=torch.uint8, device="cuda")
+    work = p.ensure_work("rk_mhd")
+    u, b, ru, rb = buf[:3 * C], buf[3 * C:6 * C], buf[6 * C:9 * C], buf[9 * C:12 * C]
+    L = psfft.lib()
+    st = torch.cuda.current_stream().cuda_stream
+    h = p.handle
+    ptr = lambda t: ctypes.c_void_p(t.data_ptr())
+    assert L.psfft_hd_rhs(h, ptr(u), ptr(u), 0.0, ptr(work), st) == -8                      # in place
+    assert L.psfft_hd_rhs(h, ptr(u), ptr(buf[C:4 * C]), 0.0, ptr(work), st) == -8           # partial overlap
+    assert L.psfft_hd_rhs(h, ptr(u), ptr(ru), 0.0, ptr(buf[8 * C:]), st) == -8              # workspace over the output
+    assert L.psfft_hd_rhs(h, ptr(u), ptr(ru), 0.0, ptr(u), st) == -8                        # workspace over the input
+    assert L.psfft_mhd_rhs(h, ptr(u), ptr(b), ptr(ru), ptr(ru), 0.0, 0.0, ptr(work), st) == -8
+    assert L.psfft_mhd_rhs(h, ptr(u), ptr(u), ptr(ru), ptr(rb), 0.0, 0.0, ptr(work), st) == 0   # inputs may alias
+    assert psfft.last_launch_count(h) == 5
+    assert L.psfft_boussinesq_rhs(h, ptr(u), ptr(b), ptr(ru), ptr(buf[8 * C:9 * C]), 0.0, 0.0, 0.0, ptr(work), st) == -8
+    assert L.psfft_gpe_rhs(h, ptr(u), ptr(buf[C:3 * C]), 0.1, 1.0, ptr(work), st) == -8
+    par = (ctypes.c_double * 3)(0.0, 0.0, 0.0)
+    assert L.psfft_rk_step(h, 0, ptr(u), ptr(u), 2, 0.01, par, ptr(work), st) == -8
+    assert L.psfft_rk_step(h, 0, ptr(u), ptr(buf[2 * C:5 * C]), 2, 0.01, par, ptr(work), st) == -8
+    assert L.psfft_rk_step(h, 0, ptr(u), ptr(ru), 2, 0.01, par, ptr(ru), st) == -8
+    assert L.psfft_fft3d_c2r(h, ptr(u), ptr(u), ptr(work), st) == -8
+    assert L.psfft_fft3d_r2c(h, ptr(u), ptr(u), None, st) == -8
+    torch.cuda.synchronize()
+    assert psfft.last_launch_count(h) == 5               # still the accepted MHD call: the rejected ones enqueued nothing
+    # a destroyed plan is gone from the registry: every later use of the handle is PSFFT_E_PLAN
+    p.close()
+    assert L.psfft_hd_rhs(h, ptr(u), ptr(ru), 0.0, ptr(work), st) == -6
+    assert L.psfft_plan_destroy(h) == -6
 
 
 # ---- guard bands: no call writes outside the buffers it was given ------------------------------------------

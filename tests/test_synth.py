@@ -19,6 +19,12 @@ def test_golden_values(golden_dir):
             u = synth.solenoidal_spectrum(int(t[1]), float(t[2]), int(t[3]), int(t[4]), int(t[5]))
             v = u[int(t[6]), int(t[7]), int(t[8]), int(t[9])]
             assert v.real == float(t[10]) and v.imag == float(t[11])
+        elif t[0] == "broadband":        # (the global energy sum may round differently across numpy builds)
+            v = synth.broadband_spectrum(int(t[1]), seed=int(t[2]), tag=int(t[3]))[int(t[4]), int(t[5]), int(t[6]), int(t[7])]
+            assert abs(v - complex(float(t[8]), float(t[9]))) <= 1e-13 * abs(v)
+        elif t[0] == "broadband_scalar":
+            v = synth.broadband_scalar(int(t[1]), seed=int(t[2]), tag=int(t[3]))[int(t[4]), int(t[5]), int(t[6])]
+            assert abs(v - complex(float(t[7]), float(t[8]))) <= 1e-13 * abs(v)
 
 
 def test_uniform_field_range_and_batch_indexing():
@@ -58,3 +64,42 @@ def test_solenoidal_field_is_grid_independent():
     # different tags give different fields
     c = synth.solenoidal_spectrum(24, 2.0, 6, 5, tag=1) / 24**3
     assert np.abs(a - c).max() > 1e-3
+
+
+def test_broadband_fields_fill_the_spectrum_below_nyquist():
+    """Unit energy, solenoidal, Hermitian kx = 0 plane, E(k) ~ k^-5/3 shell by shell, every mode with
+    1 <= |k| <= N/2 - 1 populated (inside AND outside the 2/3 sphere), grid independent up to the normalisation."""
+    N = 48
+    u = synth.broadband_spectrum(N, seed=3)
+    th = synth.broadband_scalar(N, seed=3)
+    k = np.arange(N)
+    k = np.where(k < N // 2, k, k - N)
+    kx, ky, kz = np.arange(N // 2 + 1)[None, None, :], k[None, :, None], k[:, None, None]
+    w = np.full(N // 2 + 1, 2.0)
+    w[0] = w[-1] = 1.0
+    a = u / N**3
+    assert abs(0.5 * np.sum(w * np.abs(a) ** 2) - 1.0) < 1e-13
+    assert abs(0.5 * np.sum(w * np.abs(th / N**3) ** 2) - 1.0) < 1e-13
+    assert np.abs(kx * a[0] + ky * a[1] + kz * a[2]).max() < 1e-15
+    for f in (a[0], a[1], a[2], th):
+        assert np.abs(f[(-k[:, None]) % N, (-k[None, :]) % N, 0] - np.conj(f[k[:, None] % N, k[None, :] % N, 0])).max() == 0
+    k2 = kx**2 + ky**2 + kz**2 + 0 * a[0].real
+    inside = (k2 >= 1) & (k2 <= (N // 2 - 1) ** 2)
+    assert np.all(np.abs(th[inside]) > 0) and np.all(th[~inside] == 0)
+    assert np.all(np.sum(np.abs(a), axis=0)[inside] > 0) and np.all(a[:, ~inside] == 0)
+    shell = np.rint(np.sqrt(k2)).astype(int)
+    E = np.bincount(shell.ravel(), weights=(0.5 * w * np.sum(np.abs(a) ** 2, axis=0)).ravel())
+    comp = E[4:N // 2 - 1] * np.arange(4, N // 2 - 1) ** (5.0 / 3.0)
+    assert comp.max() / comp.min() < 1.35                               # flat compensated spectrum (lattice noise)
+    b = synth.broadband_spectrum(64, kcut=N // 2 - 1, seed=3) / 64**3   # same kcut => same normalisation
+    assert abs(b[1, 64 - 3, 5, 7] - a[1, N - 3, 5, 7]) < 1e-15 * abs(b[1, 64 - 3, 5, 7])
+
+
+def test_taylor_green_spectrum_is_the_transform_of_the_field():
+    N, m = 16, 3
+    x, y, z = synth.grid_axes(N)
+    u = np.stack([np.sin(m * x) * np.cos(m * y) * np.cos(m * z), -np.cos(m * x) * np.sin(m * y) * np.cos(m * z),
+                  np.zeros((N, N, N))])
+    want = np.fft.rfftn(u, axes=(1, 2, 3))
+    assert np.abs(synth.taylor_green_spectrum(N, m) - want).max() < 1e-10
+    assert np.count_nonzero(synth.taylor_green_spectrum(N, m)) == 8
