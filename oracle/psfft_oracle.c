@@ -21,8 +21,10 @@
  *
  * Conventions: real field [z][y][x], x contiguous; half spectrum
  * [kz][ky][kx], kx in [0, Nx/2]; forward sign -, unnormalised; inverse sign +, scaled by
- * 1/(Nx Ny Nz); box 2*pi-periodic so wavenumbers are the integers k = p (p < n/2) or
- * p - n (p >= n/2).
+ * 1/(Nx Ny Nz); wavenumbers k_i = n_i (2 pi / L_i) with n_i = p (p < N_i/2) or p - N_i (p >= N_i/2):
+ * the integers themselves in the 2 pi-periodic box of every BASELINE.json config; the general grid
+ * (Nx, Ny, Nz) and box (Lx, Ly, Lz) of PAPER.md:64 through the *3 entry points (pins:
+ * tests/test_oracle_aniso.py).
  */
 #include <complex.h>
 #include <math.h>
@@ -307,93 +309,112 @@ void orc_idft3d_point(int Nz, int Ny, int Nx, const cplx *X, int k, int j, int i
 }
 
 /* ---------------------------------------------------------------------------------------
- * spectral helpers on a cubic N^3 grid (BASELINE.json configs are cubes)
+ * Grid and box.  PAPER.md:64 (Sec. 2, below Eq. 8): "both the physical box size, L_i, and the number of
+ * physical space points, N_i, may be specified independently in each direction".
+ *   wavenumbers   k_i = n_i (2 pi / L_i), n_i the integer index p (p < N_i/2) or p - N_i (DESIGN.md
+ *                 reading G24; the factor 2 pi / L_i is evaluated once in fp64 and is exactly 1 for L_i = 2 pi)
+ *   2/3 rule      ellipsoidal truncation in INDEX space, sum_i (n_i / N_i)^2 < 1/9, whatever the box
+ *                 (reading G25), evaluated in integers: with L = lcm(Nx, Ny, Nz) and r_i = L / N_i,
+ *                 keep iff 9 sum_i (r_i n_i)^2 < L^2.  For Nx = Ny = Nz = N this is 9 |n|^2 < N^2 (G4).
+ * The cubic 2 pi box (every BASELINE.json config) is the special case r_i = 1, k_i = n_i.
  * ------------------------------------------------------------------------------------- */
-static inline int wavenumber(int idx, int n) { return idx < n / 2 ? idx : idx - n; } /* n/2 -> -n/2 (G8) */
+typedef struct {
+    int Nx, Ny, Nz, H;      /* H = Nx/2 + 1 */
+    long nf, nr;            /* modes of a half spectrum, points of a real field */
+    double kfx, kfy, kfz;   /* 2 pi / L_i */
+    long rx, ry, rz, L;     /* L = lcm(Nx, Ny, Nz), r_i = L / N_i */
+} grid_t;
 
-/* a9: 2/3-rule spherical truncation, integer arithmetic: keep iff 9 |k|^2 < N^2 (G4) */
-static inline int keep_mode(int N, int kx, int ky, int kz)
+static long gcd_l(long a, long b) { while (b) { long t = a % b; a = b; b = t; } return a; }
+
+static grid_t grid_make(int Nz, int Ny, int Nx, const double *box /* Lx, Ly, Lz; NULL = 2 pi each */)
 {
-    long k2 = (long)kx * kx + (long)ky * ky + (long)kz * kz;
-    return 9 * k2 < (long)N * N;
+    grid_t g;
+    g.Nx = Nx; g.Ny = Ny; g.Nz = Nz; g.H = Nx / 2 + 1;
+    g.nf = (long)Nz * Ny * g.H;
+    g.nr = (long)Nz * Ny * Nx;
+    g.kfx = box ? TWO_PI / box[0] : 1.0;
+    g.kfy = box ? TWO_PI / box[1] : 1.0;
+    g.kfz = box ? TWO_PI / box[2] : 1.0;
+    long l = (long)Nx / gcd_l(Nx, Ny) * Ny;
+    g.L = l / gcd_l(l, Nz) * Nz;
+    g.rx = g.L / Nx; g.ry = g.L / Ny; g.rz = g.L / Nz;
+    return g;
 }
 
-void orc_dealias_mask(int N, unsigned char *mask)
+static inline int wavenumber(int idx, int n) { return idx < n / 2 ? idx : idx - n; } /* n/2 -> -n/2 (G8) */
+
+/* a9: 2/3-rule truncation, integer arithmetic (G4, G25) */
+static inline int keep_mode(const grid_t *g, int nx, int ny, int nz)
 {
-    int H = N / 2 + 1;
-#pragma omp parallel for schedule(static)
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p)
-                mask[((long)r * N + q) * H + p] =
-                    (unsigned char)keep_mode(N, p, wavenumber(q, N), wavenumber(r, N));
+    long a = g->rx * nx, b = g->ry * ny, c = g->rz * nz;
+    return 9 * (a * a + b * b + c * c) < g->L * g->L;
+}
+
+/* loop over the half spectrum: o = linear index, (kx, ky, kz) = real wavenumbers, keep = mask bit */
+#define FOR_MODES(g)                                                         \
+    _Pragma("omp parallel for schedule(static)")                             \
+    for (int r = 0; r < (g)->Nz; ++r)                                        \
+        for (int q = 0; q < (g)->Ny; ++q)                                    \
+            for (int p = 0; p < (g)->H; ++p)
+#define MODE_VARS(g)                                                         \
+    const long o = ((long)r * (g)->Ny + q) * (g)->H + p;                     \
+    const int nx = p, ny = wavenumber(q, (g)->Ny), nz = wavenumber(r, (g)->Nz); \
+    const double kx = nx * (g)->kfx, ky = ny * (g)->kfy, kz = nz * (g)->kfz; \
+    (void)o; (void)kx; (void)ky; (void)kz;
+
+static void dealias_mask_g(const grid_t *g, unsigned char *mask)
+{
+    FOR_MODES(g) { MODE_VARS(g) mask[o] = (unsigned char)keep_mode(g, nx, ny, nz); }
 }
 
 /* step 1 / step 6 of O6: f <- M f; masked entries become +0.0 (both parts) */
-void orc_apply_mask(int N, int ncomp, cplx *f)
+static void apply_mask_g(const grid_t *g, int ncomp, cplx *f)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H;
-#pragma omp parallel for schedule(static)
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p)
-                if (!keep_mode(N, p, wavenumber(q, N), wavenumber(r, N)))
-                    for (int c = 0; c < ncomp; ++c) f[c * nf + ((long)r * N + q) * H + p] = 0.0;
+    FOR_MODES(g) {
+        MODE_VARS(g)
+        if (!keep_mode(g, nx, ny, nz))
+            for (int c = 0; c < ncomp; ++c) f[c * g->nf + o] = 0.0;
+    }
 }
 
 /* a7: w = i k x u  (w_x = i (k_y u_z - k_z u_y), cyclic) */
-void orc_curl(int N, const cplx *u, cplx *w)
+static void curl_g(const grid_t *g, const cplx *u, cplx *w)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H;
-#pragma omp parallel for schedule(static)
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p) {
-                long o = ((long)r * N + q) * H + p;
-                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                cplx ux = u[o], uy = u[nf + o], uz = u[2 * nf + o];
-                w[o] = I * (ky * uz - kz * uy);
-                w[nf + o] = I * (kz * ux - kx * uz);
-                w[2 * nf + o] = I * (kx * uy - ky * ux);
-            }
+    const long nf = g->nf;
+    FOR_MODES(g) {
+        MODE_VARS(g)
+        cplx ux = u[o], uy = u[nf + o], uz = u[2 * nf + o];
+        w[o] = I * (ky * uz - kz * uy);
+        w[nf + o] = I * (kz * ux - kx * uz);
+        w[2 * nf + o] = I * (kx * uy - ky * ux);
+    }
 }
 
 /* a10: f <- f - k (k.f)/|k|^2 for k != 0; identity at k = 0 (G6, G7) */
-void orc_project(int N, cplx *f)
+static void project_g(const grid_t *g, cplx *f)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H;
-#pragma omp parallel for schedule(static)
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p) {
-                long o = ((long)r * N + q) * H + p;
-                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                double k2 = kx * kx + ky * ky + kz * kz;
-                if (k2 == 0.0) continue;
-                cplx d = (kx * f[o] + ky * f[nf + o] + kz * f[2 * nf + o]) / k2;
-                f[o] -= kx * d;
-                f[nf + o] -= ky * d;
-                f[2 * nf + o] -= kz * d;
-            }
+    const long nf = g->nf;
+    FOR_MODES(g) {
+        MODE_VARS(g)
+        double k2 = kx * kx + ky * ky + kz * kz;
+        if (k2 == 0.0) continue;
+        cplx d = (kx * f[o] + ky * f[nf + o] + kz * f[2 * nf + o]) / k2;
+        f[o] -= kx * d;
+        f[nf + o] -= ky * d;
+        f[2 * nf + o] -= kz * d;
+    }
 }
 
 /* a11: f <- f - nu |k|^2 u */
-static void add_diffusion(int N, double nu, const cplx *u, cplx *f)
+static void add_diffusion(const grid_t *g, double nu, const cplx *u, cplx *f)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H;
-#pragma omp parallel for schedule(static)
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p) {
-                long o = ((long)r * N + q) * H + p;
-                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                double k2 = kx * kx + ky * ky + kz * kz;
-                for (int c = 0; c < 3; ++c) f[c * nf + o] -= nu * k2 * u[c * nf + o];
-            }
+    const long nf = g->nf;
+    FOR_MODES(g) {
+        MODE_VARS(g)
+        double k2 = kx * kx + ky * ky + kz * kz;
+        for (int c = 0; c < 3; ++c) f[c * nf + o] -= nu * k2 * u[c * nf + o];
+    }
 }
 
 /* a8: c = a x b pointwise on n points, 3-component fields laid out [3][n] */
@@ -409,38 +430,40 @@ static void cross_add(long n, const double *a, const double *b, double *c, int a
     }
 }
 
+static void inv3(const grid_t *g, const cplx *X, double *x) { orc_c2r3d(g->Nz, g->Ny, g->Nx, X, x); }
+static void fwd3(const grid_t *g, const double *x, cplx *X) { orc_r2c3d(g->Nz, g->Ny, g->Nx, x, X); }
+
 /* ---------------------------------------------------------------------------------------
  * O6  hd_rhs(uhat, nu) = M P F[ F^-1(M uhat) x F^-1(i k x M uhat) ] - nu |k|^2 M uhat
  *     (Eq. 1 with theta = 0, Eq. 3; nonlinear term in physical
  *     space, projection in spectral space; rotational form, 2/3 rule and the transform
  *     count 6 + 3 from BASELINE.json config 2).  Steps 1-8 of SURVEY.md §8(c) O6.
- *     uhat, rhs: [3][kz][ky][kx], values = N^3 x Fourier coefficient.
+ *     uhat, rhs: [3][kz][ky][kx], values = (Nx Ny Nz) x Fourier coefficient.
  * ------------------------------------------------------------------------------------- */
-void orc_hd_rhs(int N, const cplx *uhat, double nu, cplx *rhs)
+static void hd_rhs_g(const grid_t *g, const cplx *uhat, double nu, cplx *rhs)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H, nr = (long)N * N * N;
+    const long nf = g->nf, nr = g->nr;
     cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
     cplx *wh = (cplx *)malloc(sizeof(cplx) * 3 * nf);
     double *u = (double *)malloc(sizeof(double) * 3 * nr);
     double *w = (double *)malloc(sizeof(double) * 3 * nr);
     memcpy(um, uhat, sizeof(cplx) * 3 * nf);
-    orc_apply_mask(N, 3, um);                                   /* 1 */
-    orc_curl(N, um, wh);                                        /* 2 */
+    apply_mask_g(g, 3, um);                                     /* 1 */
+    curl_g(g, um, wh);                                          /* 2 */
     for (int c = 0; c < 3; ++c) {                               /* 3 */
-        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
-        orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);
+        inv3(g, um + c * nf, u + c * nr);
+        inv3(g, wh + c * nf, w + c * nr);
     }
     free(wh);
     double *n = (double *)malloc(sizeof(double) * 3 * nr);
     cross_add(nr, u, w, n, 0);                                  /* 4 */
     free(u);
     free(w);
-    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, n + c * nr, rhs + c * nf); /* 5 */
+    for (int c = 0; c < 3; ++c) fwd3(g, n + c * nr, rhs + c * nf); /* 5 */
     free(n);
-    orc_apply_mask(N, 3, rhs);                                  /* 6 */
-    orc_project(N, rhs);                                        /* 7 */
-    if (nu != 0.0) add_diffusion(N, nu, um, rhs);               /* 8 */
+    apply_mask_g(g, 3, rhs);                                    /* 6 */
+    project_g(g, rhs);                                          /* 7 */
+    if (nu != 0.0) add_diffusion(g, nu, um, rhs);               /* 8 */
     free(um);
 }
 
@@ -450,11 +473,10 @@ void orc_hd_rhs(int N, const cplx *uhat, double nu, cplx *rhs)
  *     R_u = M P F[m] - nu |k|^2 M uhat;   R_b = M i k x F[e] - eta |k|^2 M bhat.
  *     (B.grad B - grad(p + |B|^2/2) = j x b under the projection, as for u.)
  * ------------------------------------------------------------------------------------- */
-void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double eta, cplx *ru,
-                 cplx *rb)
+static void mhd_rhs_g(const grid_t *g, const cplx *uhat, const cplx *bhat, double nu, double eta, cplx *ru,
+                      cplx *rb)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H, nr = (long)N * N * N;
+    const long nf = g->nf, nr = g->nr;
     cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
     cplx *bm = (cplx *)malloc(sizeof(cplx) * 3 * nf);
     cplx *th = (cplx *)malloc(sizeof(cplx) * 3 * nf);
@@ -464,31 +486,31 @@ void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double et
     double *m = (double *)malloc(sizeof(double) * 3 * nr);
     memcpy(um, uhat, sizeof(cplx) * 3 * nf);
     memcpy(bm, bhat, sizeof(cplx) * 3 * nf);
-    orc_apply_mask(N, 3, um);
-    orc_apply_mask(N, 3, bm);
+    apply_mask_g(g, 3, um);
+    apply_mask_g(g, 3, bm);
     for (int c = 0; c < 3; ++c) {
-        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
-        orc_c2r3d(N, N, N, bm + c * nf, b + c * nr);
+        inv3(g, um + c * nf, u + c * nr);
+        inv3(g, bm + c * nf, b + c * nr);
     }
-    orc_curl(N, um, th);                                   /* w^ */
-    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, th + c * nf, t + c * nr);
+    curl_g(g, um, th);                                     /* w^ */
+    for (int c = 0; c < 3; ++c) inv3(g, th + c * nf, t + c * nr);
     cross_add(nr, u, t, m, 0);                             /* m = u x w */
-    orc_curl(N, bm, th);                                   /* j^ */
-    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, th + c * nf, t + c * nr);
+    curl_g(g, bm, th);                                     /* j^ */
+    for (int c = 0; c < 3; ++c) inv3(g, th + c * nf, t + c * nr);
     cross_add(nr, t, b, m, 1);                             /* m += j x b */
     cross_add(nr, u, b, t, 0);                             /* e = u x b */
     free(u);
     free(b);
-    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, m + c * nr, ru + c * nf);
-    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, t + c * nr, th + c * nf);
+    for (int c = 0; c < 3; ++c) fwd3(g, m + c * nr, ru + c * nf);
+    for (int c = 0; c < 3; ++c) fwd3(g, t + c * nr, th + c * nf);
     free(m);
     free(t);
-    orc_apply_mask(N, 3, ru);
-    orc_project(N, ru);
-    if (nu != 0.0) add_diffusion(N, nu, um, ru);
-    orc_apply_mask(N, 3, th);
-    orc_curl(N, th, rb);
-    if (eta != 0.0) add_diffusion(N, eta, bm, rb);
+    apply_mask_g(g, 3, ru);
+    project_g(g, ru);
+    if (nu != 0.0) add_diffusion(g, nu, um, ru);
+    apply_mask_g(g, 3, th);
+    curl_g(g, th, rb);
+    if (eta != 0.0) add_diffusion(g, eta, bm, rb);
     free(th);
     free(um);
     free(bm);
@@ -509,13 +531,12 @@ void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double et
  *       7. n^_z <- n^_z - N_bv tm;  n^ <- P n^            (buoyancy is inside the projection: Eq. 1)
  *       8. R_u = n^ - nu |k|^2 um
  *       9. R_th = -s^ + N_bv um_z - kappa |k|^2 tm
- *     uhat, ru: [3][kz][ky][kx]; thhat, rt: [kz][ky][kx]; values = N^3 x Fourier coefficient.
+ *     uhat, ru: [3][kz][ky][kx]; thhat, rt: [kz][ky][kx]; values = (Nx Ny Nz) x Fourier coefficient.
  * ------------------------------------------------------------------------------------- */
-void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, double kappa,
-                        double nbv, cplx *ru, cplx *rt)
+static void boussinesq_rhs_g(const grid_t *g, const cplx *uhat, const cplx *thhat, double nu, double kappa,
+                             double nbv, cplx *ru, cplx *rt)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H, nr = (long)N * N * N;
+    const long nf = g->nf, nr = g->nr;
     cplx *um = (cplx *)malloc(sizeof(cplx) * 3 * nf);
     cplx *tm = (cplx *)malloc(sizeof(cplx) * nf);
     cplx *wh = (cplx *)malloc(sizeof(cplx) * 3 * nf);
@@ -523,90 +544,44 @@ void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, d
     double *w = (double *)malloc(sizeof(double) * 3 * nr);
     memcpy(um, uhat, sizeof(cplx) * 3 * nf);
     memcpy(tm, thhat, sizeof(cplx) * nf);
-    orc_apply_mask(N, 3, um);                                   /* 1 */
-    orc_apply_mask(N, 1, tm);
-    orc_curl(N, um, wh);                                        /* 2 (curl) */
+    apply_mask_g(g, 3, um);                                     /* 1 */
+    apply_mask_g(g, 1, tm);
+    curl_g(g, um, wh);                                          /* 2 (curl) */
     for (int c = 0; c < 3; ++c) {                               /* 3 (u, w) */
-        orc_c2r3d(N, N, N, um + c * nf, u + c * nr);
-        orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);
+        inv3(g, um + c * nf, u + c * nr);
+        inv3(g, wh + c * nf, w + c * nr);
     }
     double *n = (double *)malloc(sizeof(double) * 3 * nr);
     cross_add(nr, u, w, n, 0);                                  /* 4 (n = u x w) */
-#pragma omp parallel for schedule(static)                       /* 2 (gradient), reusing wh */
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p) {
-                long o = ((long)r * N + q) * H + p;
-                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                wh[o] = I * kx * tm[o];
-                wh[nf + o] = I * ky * tm[o];
-                wh[2 * nf + o] = I * kz * tm[o];
-            }
-    for (int c = 0; c < 3; ++c) orc_c2r3d(N, N, N, wh + c * nf, w + c * nr);   /* 3 (g) */
+    FOR_MODES(g) {                                              /* 2 (gradient), reusing wh */
+        MODE_VARS(g)
+        wh[o] = I * kx * tm[o];
+        wh[nf + o] = I * ky * tm[o];
+        wh[2 * nf + o] = I * kz * tm[o];
+    }
+    for (int c = 0; c < 3; ++c) inv3(g, wh + c * nf, w + c * nr);   /* 3 (g) */
     free(wh);
     double *s = (double *)malloc(sizeof(double) * nr);
 #pragma omp parallel for schedule(static)                       /* 4 (s = u . g) */
     for (long i = 0; i < nr; ++i) s[i] = u[i] * w[i] + u[nr + i] * w[nr + i] + u[2 * nr + i] * w[2 * nr + i];
     free(u);
     free(w);
-    for (int c = 0; c < 3; ++c) orc_r2c3d(N, N, N, n + c * nr, ru + c * nf);   /* 5 */
-    orc_r2c3d(N, N, N, s, rt);
+    for (int c = 0; c < 3; ++c) fwd3(g, n + c * nr, ru + c * nf);   /* 5 */
+    fwd3(g, s, rt);
     free(n);
     free(s);
-    orc_apply_mask(N, 3, ru);                                   /* 6 */
-    orc_apply_mask(N, 1, rt);
+    apply_mask_g(g, 3, ru);                                     /* 6 */
+    apply_mask_g(g, 1, rt);
     for (long o = 0; o < nf; ++o) ru[2 * nf + o] -= nbv * tm[o];               /* 7 */
-    orc_project(N, ru);
-    if (nu != 0.0) add_diffusion(N, nu, um, ru);                /* 8 */
-#pragma omp parallel for schedule(static)                       /* 9 */
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int p = 0; p < H; ++p) {
-                long o = ((long)r * N + q) * H + p;
-                double kx = p, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                double k2 = kx * kx + ky * ky + kz * kz;
-                rt[o] = -rt[o] + nbv * um[2 * nf + o] - kappa * k2 * tm[o];
-            }
+    project_g(g, ru);
+    if (nu != 0.0) add_diffusion(g, nu, um, ru);                /* 8 */
+    FOR_MODES(g) {                                              /* 9 */
+        MODE_VARS(g)
+        double k2 = kx * kx + ky * ky + kz * kz;
+        rt[o] = -rt[o] + nbv * um[2 * nf + o] - kappa * k2 * tm[o];
+    }
     free(um);
     free(tm);
-}
-
-/* ---------------------------------------------------------------------------------------
- * O9  rk_step: one explicit Runge-Kutta time step around the right-hand sides above.
- *     PAPER.md:66: "the system of ODEs is solved using an explicit Runge-Kutta scheme (of
- *     2nd-4th order); explicit time stepping is used to resolve all wave modes".  The paper does
- *     not print the scheme; DESIGN.md reading G21 takes the low-storage form with `ord` stages
- *         y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0)
- *     (R = O6 / O7 / O8, M = the 2/3 mask).  For a linear R = L y this is the degree-`ord` Taylor
- *     polynomial of exp(dt L), i.e. order `ord`; for the nonlinear terms it is second order.
- *     sys: 0 = HD (y = u^, 3 fields), 1 = MHD (y = u^, b^: 6 fields), 2 = Boussinesq (y = u^, theta^: 4),
- *     3 = GPE (y = p^, q^: 2 fields).  par = { nu, eta (MHD) or kappa (Boussinesq), N_bv }; GPE: { alpha, beta }.
- * ------------------------------------------------------------------------------------- */
-void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs);   /* O10, below */
-static void rk_rhs(int N, int sys, const double *par, const cplx *y, cplx *r)
-{
-    long nf = (long)N * N * (N / 2 + 1);
-    if (sys == 0) orc_hd_rhs(N, y, par[0], r);
-    else if (sys == 1) orc_mhd_rhs(N, y, y + 3 * nf, par[0], par[1], r, r + 3 * nf);
-    else if (sys == 3) orc_gpe_rhs(N, y, par[0], par[1], r);
-    else orc_boussinesq_rhs(N, y, y + 3 * nf, par[0], par[1], par[2], r, r + 3 * nf);
-}
-
-void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cplx *y0, cplx *y1)
-{
-    int nfields = sys == 0 ? 3 : sys == 1 ? 6 : sys == 3 ? 2 : 4;
-    long nf = (long)N * N * (N / 2 + 1), n = nfields * nf;
-    cplx *ym = (cplx *)malloc(sizeof(cplx) * n);   /* M y_n */
-    cplx *r = (cplx *)malloc(sizeof(cplx) * n);
-    memcpy(ym, y0, sizeof(cplx) * n);
-    orc_apply_mask(N, nfields, ym);
-    memcpy(y1, y0, sizeof(cplx) * n);              /* y^(ord) = y_n */
-    for (int o = ord; o >= 1; --o) {
-        rk_rhs(N, sys, par, y1, r);
-        for (long i = 0; i < n; ++i) y1[i] = ym[i] + (dt / o) * r[i];
-    }
-    free(ym);
-    free(r);
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -623,18 +598,17 @@ void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cp
  *       3. a = (p^2 + q^2) q,  b = (p^2 + q^2) p              (pointwise)
  *       4. a^ = M r2c3d(a),  b^ = M r2c3d(b)                  (2 forward transforms)
  *       5. R_p = beta a^ + alpha |k|^2 qm,   R_q = -beta b^ - alpha |k|^2 pm
- *     psihat, rhs: [2][kz][ky][kx] = (p^, q^); values = N^3 x Fourier coefficient.
+ *     psihat, rhs: [2][kz][ky][kx] = (p^, q^); values = (Nx Ny Nz) x Fourier coefficient.
  * ------------------------------------------------------------------------------------- */
-void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs)
+static void gpe_rhs_g(const grid_t *g, const cplx *psihat, double alpha, double beta, cplx *rhs)
 {
-    int H = N / 2 + 1;
-    long nf = (long)N * N * H, nr = (long)N * N * N;
+    const long nf = g->nf, nr = g->nr;
     cplx *pm = (cplx *)malloc(sizeof(cplx) * 2 * nf);
     double *p = (double *)malloc(sizeof(double) * 2 * nr);
     double *a = (double *)malloc(sizeof(double) * 2 * nr);
     memcpy(pm, psihat, sizeof(cplx) * 2 * nf);
-    orc_apply_mask(N, 2, pm);                                            /* 1 */
-    for (int c = 0; c < 2; ++c) orc_c2r3d(N, N, N, pm + c * nf, p + c * nr);   /* 2 */
+    apply_mask_g(g, 2, pm);                                              /* 1 */
+    for (int c = 0; c < 2; ++c) inv3(g, pm + c * nf, p + c * nr);        /* 2 */
 #pragma omp parallel for schedule(static)                                /* 3 */
     for (long i = 0; i < nr; ++i) {
         double rho = p[i] * p[i] + p[nr + i] * p[nr + i];
@@ -642,19 +616,114 @@ void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs
         a[nr + i] = rho * p[i];
     }
     free(p);
-    for (int c = 0; c < 2; ++c) orc_r2c3d(N, N, N, a + c * nr, rhs + c * nf); /* 4 */
+    for (int c = 0; c < 2; ++c) fwd3(g, a + c * nr, rhs + c * nf);       /* 4 */
     free(a);
-    orc_apply_mask(N, 2, rhs);
-#pragma omp parallel for schedule(static)                                /* 5 */
-    for (int r = 0; r < N; ++r)
-        for (int q = 0; q < N; ++q)
-            for (int x = 0; x < H; ++x) {
-                long o = ((long)r * N + q) * H + x;
-                double kx = x, ky = wavenumber(q, N), kz = wavenumber(r, N);
-                double k2 = kx * kx + ky * ky + kz * kz;
-                cplx ra = rhs[o], rb = rhs[nf + o];
-                rhs[o] = beta * ra + alpha * k2 * pm[nf + o];
-                rhs[nf + o] = -beta * rb - alpha * k2 * pm[o];
-            }
+    apply_mask_g(g, 2, rhs);
+    FOR_MODES(g) {                                                       /* 5 */
+        MODE_VARS(g)
+        double k2 = kx * kx + ky * ky + kz * kz;
+        cplx ra = rhs[o], rb = rhs[nf + o];
+        rhs[o] = beta * ra + alpha * k2 * pm[nf + o];
+        rhs[nf + o] = -beta * rb - alpha * k2 * pm[o];
+    }
     free(pm);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O9  rk_step: one explicit Runge-Kutta time step around the right-hand sides above.
+ *     PAPER.md:66: "the system of ODEs is solved using an explicit Runge-Kutta scheme (of
+ *     2nd-4th order); explicit time stepping is used to resolve all wave modes".  The paper does
+ *     not print the scheme; DESIGN.md reading G21 takes the low-storage form with `ord` stages
+ *         y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0)
+ *     (R = O6 / O7 / O8 / O10, M = the 2/3 mask).  For a linear R = L y this is the degree-`ord` Taylor
+ *     polynomial of exp(dt L), i.e. order `ord`; for the nonlinear terms it is second order.
+ *     sys: 0 = HD (y = u^, 3 fields), 1 = MHD (y = u^, b^: 6 fields), 2 = Boussinesq (y = u^, theta^: 4),
+ *     3 = GPE (y = p^, q^: 2 fields).  par = { nu, eta (MHD) or kappa (Boussinesq), N_bv }; GPE: { alpha, beta }.
+ * ------------------------------------------------------------------------------------- */
+static void rk_rhs(const grid_t *g, int sys, const double *par, const cplx *y, cplx *r)
+{
+    const long nf = g->nf;
+    if (sys == 0) hd_rhs_g(g, y, par[0], r);
+    else if (sys == 1) mhd_rhs_g(g, y, y + 3 * nf, par[0], par[1], r, r + 3 * nf);
+    else if (sys == 3) gpe_rhs_g(g, y, par[0], par[1], r);
+    else boussinesq_rhs_g(g, y, y + 3 * nf, par[0], par[1], par[2], r, r + 3 * nf);
+}
+
+static void rk_step_g(const grid_t *g, int sys, int ord, double dt, const double *par, const cplx *y0, cplx *y1)
+{
+    int nfields = sys == 0 ? 3 : sys == 1 ? 6 : sys == 3 ? 2 : 4;
+    long n = nfields * g->nf;
+    cplx *ym = (cplx *)malloc(sizeof(cplx) * n);   /* M y_n */
+    cplx *r = (cplx *)malloc(sizeof(cplx) * n);
+    memcpy(ym, y0, sizeof(cplx) * n);
+    apply_mask_g(g, nfields, ym);
+    memcpy(y1, y0, sizeof(cplx) * n);              /* y^(ord) = y_n */
+    for (int o = ord; o >= 1; --o) {
+        rk_rhs(g, sys, par, y1, r);
+        for (long i = 0; i < n; ++i) y1[i] = ym[i] + (dt / o) * r[i];
+    }
+    free(ym);
+    free(r);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * exported entry points: the cubic 2 pi box (N) and the general grid and box (Nz, Ny, Nx, box = {Lx, Ly, Lz})
+ * ------------------------------------------------------------------------------------- */
+void orc_dealias_mask(int N, unsigned char *mask) { grid_t g = grid_make(N, N, N, NULL); dealias_mask_g(&g, mask); }
+void orc_apply_mask(int N, int ncomp, cplx *f) { grid_t g = grid_make(N, N, N, NULL); apply_mask_g(&g, ncomp, f); }
+void orc_curl(int N, const cplx *u, cplx *w) { grid_t g = grid_make(N, N, N, NULL); curl_g(&g, u, w); }
+void orc_project(int N, cplx *f) { grid_t g = grid_make(N, N, N, NULL); project_g(&g, f); }
+void orc_hd_rhs(int N, const cplx *uhat, double nu, cplx *rhs) { grid_t g = grid_make(N, N, N, NULL); hd_rhs_g(&g, uhat, nu, rhs); }
+void orc_mhd_rhs(int N, const cplx *uhat, const cplx *bhat, double nu, double eta, cplx *ru, cplx *rb)
+{
+    grid_t g = grid_make(N, N, N, NULL);
+    mhd_rhs_g(&g, uhat, bhat, nu, eta, ru, rb);
+}
+void orc_boussinesq_rhs(int N, const cplx *uhat, const cplx *thhat, double nu, double kappa, double nbv, cplx *ru,
+                        cplx *rt)
+{
+    grid_t g = grid_make(N, N, N, NULL);
+    boussinesq_rhs_g(&g, uhat, thhat, nu, kappa, nbv, ru, rt);
+}
+void orc_gpe_rhs(int N, const cplx *psihat, double alpha, double beta, cplx *rhs)
+{
+    grid_t g = grid_make(N, N, N, NULL);
+    gpe_rhs_g(&g, psihat, alpha, beta, rhs);
+}
+void orc_rk_step(int N, int sys, int ord, double dt, const double *par, const cplx *y0, cplx *y1)
+{
+    grid_t g = grid_make(N, N, N, NULL);
+    rk_step_g(&g, sys, ord, dt, par, y0, y1);
+}
+
+void orc_dealias_mask3(int Nz, int Ny, int Nx, unsigned char *mask) { grid_t g = grid_make(Nz, Ny, Nx, NULL); dealias_mask_g(&g, mask); }
+void orc_curl3(int Nz, int Ny, int Nx, const double *box, const cplx *u, cplx *w) { grid_t g = grid_make(Nz, Ny, Nx, box); curl_g(&g, u, w); }
+void orc_project3(int Nz, int Ny, int Nx, const double *box, cplx *f) { grid_t g = grid_make(Nz, Ny, Nx, box); project_g(&g, f); }
+void orc_hd_rhs3(int Nz, int Ny, int Nx, const double *box, const cplx *uhat, double nu, cplx *rhs)
+{
+    grid_t g = grid_make(Nz, Ny, Nx, box);
+    hd_rhs_g(&g, uhat, nu, rhs);
+}
+void orc_mhd_rhs3(int Nz, int Ny, int Nx, const double *box, const cplx *uhat, const cplx *bhat, double nu, double eta,
+                  cplx *ru, cplx *rb)
+{
+    grid_t g = grid_make(Nz, Ny, Nx, box);
+    mhd_rhs_g(&g, uhat, bhat, nu, eta, ru, rb);
+}
+void orc_boussinesq_rhs3(int Nz, int Ny, int Nx, const double *box, const cplx *uhat, const cplx *thhat, double nu,
+                         double kappa, double nbv, cplx *ru, cplx *rt)
+{
+    grid_t g = grid_make(Nz, Ny, Nx, box);
+    boussinesq_rhs_g(&g, uhat, thhat, nu, kappa, nbv, ru, rt);
+}
+void orc_gpe_rhs3(int Nz, int Ny, int Nx, const double *box, const cplx *psihat, double alpha, double beta, cplx *rhs)
+{
+    grid_t g = grid_make(Nz, Ny, Nx, box);
+    gpe_rhs_g(&g, psihat, alpha, beta, rhs);
+}
+void orc_rk_step3(int Nz, int Ny, int Nx, const double *box, int sys, int ord, double dt, const double *par,
+                  const cplx *y0, cplx *y1)
+{
+    grid_t g = grid_make(Nz, Ny, Nx, box);
+    rk_step_g(&g, sys, ord, dt, par, y0, y1);
 }

@@ -15,6 +15,8 @@ define the synthetic stand-ins generated here:
 * ``broadband_spectrum`` / ``broadband_scalar`` -- the same construction with a power-law shell
                               spectrum filled to the Nyquist planes (developed-turbulence stand-in; the
                               full-size parity inputs).
+* ``aniso_spectrum``       -- the broadband construction on an anisotropic grid (Nx, Ny, Nz) in a box
+                              (Lx, Ly, Lz) (the paper's 1024 x 1024 x 256 Boussinesq runs).
 * ``taylor_green`` / ``abc_flow`` / ``single_mode`` -- closed-form physical-space fields
                               used by the oracle's pins.
 
@@ -282,6 +284,70 @@ def broadband_scalar(N: int, slope: float = -5.0 / 3.0, kcut: int | None = None,
     energy = sum(_map_planes(plane, kcut + 1))
     t *= np.asarray(float(N) ** 3 / np.sqrt(energy)).astype(t.real.dtype)
     return t
+
+
+def aniso_spectrum(shape, box=None, slope: float = -5.0 / 3.0, seed: int = 1234, tag: int = 0, ncomp: int = 3,
+                   fill: float = 0.5, dtype=np.complex128) -> np.ndarray:
+    """Random-phase field on an ANISOTROPIC grid ``shape = (Nx, Ny, Nz)`` in the box ``box = (Lx, Ly, Lz)``
+    (grid points and box lengths independent per direction; default box 2 pi each): half spectrum
+    ``[ncomp][kz][ky][kx]``, value = Nx Ny Nz x Fourier coefficient.  The stand-in for the paper's flat-box
+    Boussinesq runs (1024 x 1024 x 256).
+
+    Every integer index vector n inside the ellipsoid sum (n_i / N_i)^2 < fill^2 (fill = 1/2: up to the Nyquist
+    planes, so the 2/3-rule mask of the right-hand side has something to remove) carries a mode keyed on
+    ``(seed, tag, nx, ny, nz)`` -- the same physical field on any grid that holds it -- with the power-law shell
+    amplitude of ``broadband_spectrum`` in the PHYSICAL wavenumber |k|, k_i = 2 pi n_i / L_i.  ncomp = 3: solenoidal
+    (k . a = 0 with the physical k), same polarisation construction as ``solenoidal_coefficients``; ncomp = 1: a real
+    scalar (returned with the leading axis dropped).  Unit energy, 1/2 <|u|^2> = 1."""
+    Nx, Ny, Nz = (int(v) for v in shape)
+    kf = [1.0, 1.0, 1.0] if box is None else [2.0 * np.pi / float(b) for b in box]
+    u = np.zeros((ncomp, Nz, Ny, Nx // 2 + 1), dtype=dtype)
+    ry = np.arange(-(Ny // 2) + 1, Ny // 2)
+    rz = np.arange(-(Nz // 2) + 1, Nz // 2)
+    ny_, nz_ = (a.ravel() for a in np.meshgrid(ry, rz, indexing="ij"))
+
+    def plane(nx0: int) -> float:
+        rho2 = (nx0 / Nx) ** 2 + (ny_ / Ny) ** 2 + (nz_ / Nz) ** 2
+        canon = (nx0 > 0) | ((ny_ > 0) | ((ny_ == 0) & (nz_ > 0)))
+        sel = canon & (rho2 < fill * fill) & ((nx0 != 0) | (ny_ != 0) | (nz_ != 0))
+        ny, nz = ny_[sel], nz_[sel]
+        if ny.size == 0:
+            return 0.0
+        nx = np.full(ny.size, nx0)
+        kx, ky, kz = nx * kf[0], ny * kf[1], nz * kf[2]
+        k2 = kx * kx + ky * ky + kz * kz
+        kk = np.sqrt(k2)
+        key = _key(seed, tag, nx, ny, nz)
+        if ncomp == 1:
+            a = (_shell_amplitude(k2, slope) * np.exp(2j * np.pi * _variate(key, 0)))[None]
+        else:
+            th1 = 2.0 * np.pi * _variate(key, 0)
+            th2 = 2.0 * np.pi * _variate(key, 1)
+            phi = 2.0 * np.pi * _variate(key, 2)
+            kh = np.sqrt(kx * kx + ky * ky)
+            axis = kh == 0
+            khs = np.where(axis, 1.0, kh)
+            e1 = np.stack([np.where(axis, 1.0, ky / khs), np.where(axis, 0.0, -kx / khs), np.zeros_like(kk)])
+            e2 = np.cross(np.stack([kx, ky, kz]), e1, axis=0) / kk
+            a = _shell_amplitude(k2, slope) * (np.cos(phi) * np.exp(1j * th1) * e1 + np.sin(phi) * np.exp(1j * th2) * e2)
+        u[:, nz % Nz, ny % Ny, nx0] = a
+        if nx0 == 0:
+            u[:, (-nz) % Nz, (-ny) % Ny, 0] = np.conj(a)
+        return float(np.sum(np.abs(a) ** 2))
+
+    nxmax = int(np.ceil(fill * Nx))
+    energy = sum(_map_planes(plane, min(nxmax, Nx // 2 - 1) + 1))
+    u *= np.asarray(float(Nx) * Ny * Nz / np.sqrt(energy)).astype(u.real.dtype)
+    return u[0] if ncomp == 1 else u
+
+
+def box_axes(shape, box=None):
+    """Physical coordinates of the grid ``shape = (Nx, Ny, Nz)`` in the box ``(Lx, Ly, Lz)``: x_i = L_x i / N_x ...
+    as broadcastable [z][y][x] arrays (returns x, y, z)."""
+    Nx, Ny, Nz = shape
+    Lx, Ly, Lz = (2.0 * np.pi,) * 3 if box is None else box
+    return (Lx * np.arange(Nx) / Nx)[None, None, :], (Ly * np.arange(Ny) / Ny)[None, :, None], \
+        (Lz * np.arange(Nz) / Nz)[:, None, None]
 
 
 def grid_axes(N: int):
