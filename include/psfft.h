@@ -15,7 +15,8 @@
  *   Layout   real field      [b][z][y][x], x contiguous            (N^3 reals per field)
  *            half spectrum   [b][kz][ky][kx], kx in [0, N/2] contiguous, row stride ldk = N/2+1
  *                            (ldk*N*N complex per field); index q along y/z is wavenumber q for
- *                            q < N/2 and q-N otherwise; the box is 2*pi-periodic (integer k).
+ *                            q < N/2 and q-N otherwise; the box is 2*pi-periodic (integer k) unless
+ *                            psfft_plan_set_box says otherwise.
  *            complex = interleaved (re, im) of the plan's dtype.
  *   Values   forward: X[r,q,p] = sum x[k,j,i] exp(-2 pi i (p i + q j + r k)/N), unnormalised
  *            (Eq. 8); inverse: sign +, scaled by 1/N^3 so c2r(r2c(x)) = x.
@@ -51,7 +52,7 @@ extern "C" {
 
 #define PSFFT_OK 0
 #define PSFFT_E_NULL (-1)        /* a required pointer is NULL */
-#define PSFFT_E_SIZE (-2)        /* unsupported N (see psfft_plan_query) or batch < 1 */
+#define PSFFT_E_SIZE (-2)        /* unsupported N (see psfft_plan_query), batch < 1, bad system / order / box length */
 #define PSFFT_E_DTYPE (-3)       /* dtype is not PSFFT_F32 / PSFFT_F64 */
 #define PSFFT_E_ALIGN (-4)       /* a device pointer is not 16-byte aligned */
 #define PSFFT_E_TABLE (-5)       /* table buffer smaller than layout.table_bytes */
@@ -73,7 +74,7 @@ typedef struct psfft_layout {
     size_t spec_bytes;           /* bytes of one spectral field */
     size_t table_bytes;          /* size of the twiddle-table buffer for psfft_plan_create */
     size_t work_bytes_fft;       /* workspace for psfft_fft3d_r2c / c2r (batch fields) */
-    size_t work_bytes_hd;        /* workspace for psfft_hd_rhs */
+    size_t work_bytes_hd;        /* workspace for psfft_hd_rhs (cubic plans: also enough for psfft_hd_rhs_unfused) */
     size_t work_bytes_mhd;       /* workspace for psfft_mhd_rhs */
     size_t work_bytes_boussinesq; /* workspace for psfft_boussinesq_rhs */
     int Ny, Nz;                  /* grid points along y, z (= N except for psfft_plan_create3 plans) */
@@ -95,12 +96,24 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
 /* Anisotropic grids ("we also update the formulation ... to accommodate anisotropic grids";
  * its largest runs are 1024 x 1024 x 256 and 2048 x 2048 x 512): a plan for an Nx x Ny x Nz grid,
  * each size from the supported list.  Real field [b][z][y][x] (Nx contiguous), half spectrum [b][kz][ky][kx]
- * with ldk = Nx/2 + 1; psfft_fft3d_r2c / c2r work as above (inverse scaled by 1/(Nx Ny Nz)).  The right-hand-side
- * and Runge-Kutta calls need a cubic plan and return PSFFT_E_SIZE otherwise (the work_bytes_* of the RHS are 0
- * in the layout of a non-cubic plan).  layout.N is Nx. */
+ * with ldk = Nx/2 + 1; psfft_fft3d_r2c / c2r work as above (inverse scaled by 1/(Nx Ny Nz)).  layout.N is Nx.
+ * Every right-hand-side and Runge-Kutta call works on such a plan (only the *_unfused cross-check variants need a
+ * cubic one and return PSFFT_E_SIZE otherwise); spectra are Nx Ny Nz x Fourier coefficient, and
+ *   the 2/3 rule is the ellipsoidal truncation in index space, keep iff sum_i (n_i / N_i)^2 < 1/9, evaluated in
+ *   integers as 9 sum_i (n_i L / N_i)^2 < L^2 with L = lcm(Nx, Ny, Nz) -- for a cube this is 9 |n|^2 < N^2;
+ *   n_i = the integer index p (p < N_i / 2) or p - N_i. */
 int psfft_plan_query3(int Nx, int Ny, int Nz, int dtype, int batch, psfft_layout *out);
 int psfft_plan_create3(psfft_plan *plan, int Nx, int Ny, int Nz, int dtype, int batch, void *d_tables,
                        size_t table_bytes, void *stream);
+
+/* Physical box (Sec. 2 below Eq. 8: "both the physical box size, L_i, and the number of physical space
+ * points, N_i, may be specified independently in each direction").  Sets the box lengths of the plan; from then on
+ * every derivative, projection and diffusion term of the right-hand-side calls uses the wavenumbers
+ *     k_i = n_i * (2 pi / L_i),      2 pi / L_i evaluated once in fp64 and rounded to the plan dtype
+ * (exactly 1, i.e. integer wavenumbers, for L_i = 2 pi -- the default of a new plan).  The dealiasing mask does not
+ * depend on the box (see above); the transforms do not either.  Host-only, no device work.
+ * Returns PSFFT_E_SIZE unless every length is positive and finite. */
+int psfft_plan_set_box(psfft_plan plan, double Lx, double Ly, double Lz);
 
 /* Free host-side state (PAPER.md:187 clean-up).  Never touches caller memory. */
 int psfft_plan_destroy(psfft_plan plan);
@@ -214,6 +227,46 @@ int psfft_fft3d_c2r_host(psfft_plan plan, const void *h_spec, void *h_real, void
                          void *d_work, void *stream);
 int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in,
                       void *d_out, void *d_work, void *stream);
+
+/* ---- Slab-decomposed transform over P GPUs (Sec. 2, Fig. 1) ------------------------------------
+ * The paper's decomposition: task p of P owns the z-slab of Mz = Nz / P planes.  Forward: (1) local 2D transform
+ * (x, y) of the slab, (2) global transpose -- the all-to-all, "the only communication involved" -- (3)
+ * local 1D transform along z of data that is now x-incomplete.  Here task q ends up with the x-slab
+ *     [kz = 0..Nz)[ky = 0..Ny)[kx = x0[q]..x0[q+1])    (row pitch w_q = x0[q+1] - x0[q], x0[q] = floor(q ldk / P))
+ * in the natural (not transposed) order.  Steps (1)+(2) are one call: the y-pass stores every finished column
+ * straight into the block of the task that owns its kx -- no pack buffer, no local transpose, no unpack.
+ *   d_blocks   HOST array of P DEVICE pointers; d_blocks[q] = where the block of rank q lives, addressed as
+ *              [zoff + local plane][ky][kx - x0[q]] with pitch w_q.  Two ways to use it:
+ *                direct:  d_blocks[q] = rank q's x-slab mapped into this process (NVLink peer / symmetric memory),
+ *                         zoff = rank * Mz.  The stores are the all-to-all; the caller only has to make sure every
+ *                         rank's phase 1 is complete (stream sync + barrier) before any rank starts phase 2.
+ *                packed:  d_blocks[q] = a send buffer + sum_{q' < q} Mz Ny w_q' elements, zoff = 0; then ONE all-to-all of
+ *                         contiguous slices (e.g. NCCL all_to_all_single with those split sizes) into the x-slab buffer,
+ *                         whose layout [sender p][Mz][Ny][w] is already [Nz][Ny][w].
+ * One field per call.  The results are bit for bit those of psfft_fft3d_r2c / c2r on the same data (same kernels,
+ * same butterfly order per column).  Inverse: psfft_slab_z(dir = +1) on the x-slab, exchange (direct: nothing to do;
+ * packed: all-to-all of the contiguous z-ranges [p Mz, (p+1) Mz) of the x-slabs), then psfft_slab_c2r_yx, whose y-pass
+ * loads its columns from the blocks.
+ * Returns PSFFT_E_SIZE unless 1 <= P <= PSFFT_MAX_RANKS, P divides Nz, P <= ldk, 0 <= rank < P. */
+#define PSFFT_MAX_RANKS 16
+typedef struct psfft_slab_layout {
+    int P, rank;
+    int Mz, z0;                  /* planes of this rank's z-slab, first global plane */
+    int w;                       /* kx columns of this rank's x-slab */
+    int x0[PSFFT_MAX_RANKS + 1]; /* kx range of every rank: [x0[q], x0[q+1]) */
+    size_t real_elems, real_bytes;    /* z-slab in physical space: Mz Ny Nx reals */
+    size_t zspec_elems, zspec_bytes;  /* z-slab after the x-pass: Mz Ny ldk complex (work buffer of phase 1) */
+    size_t xslab_elems, xslab_bytes;  /* this rank's x-slab: Nz Ny w complex */
+} psfft_slab_layout;
+int psfft_slab_query(psfft_plan plan, int P, int rank, psfft_slab_layout *out);
+/* forward phase 1: x-pass (r2c) of the z-slab into d_zspec (overwritten work buffer), y-pass from d_zspec into the blocks */
+int psfft_slab_r2c_xy(psfft_plan plan, int P, int rank, const void *d_real_slab, void *d_zspec, void *const *d_blocks,
+                      long zoff, void *stream);
+/* forward phase 2 (dir = -1) / inverse phase 1 (dir = +1): z-pass of this rank's x-slab, in place, unnormalised */
+int psfft_slab_z(psfft_plan plan, int P, int rank, int dir, void *d_xslab, void *stream);
+/* inverse phase 2: y-pass loading from the blocks into d_zspec, then the c2r x-pass (scaled 1/(Nx Ny Nz)) into the z-slab */
+int psfft_slab_c2r_yx(psfft_plan plan, int P, int rank, void *const *d_blocks, long zoff, void *d_zspec,
+                      void *d_real_slab, void *stream);
 
 /* Per-launch timing for measurement (bench.py's roofline object).  While enabled, every kernel an
  * execute call enqueues is bracketed by two CUDA events recorded on the launching stream (so the

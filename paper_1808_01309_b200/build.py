@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libpsfft.so")
-SOURCES = ["psfft_api.cu"] + [f"psfft_{dt}_{grp}.cu" for dt in ("f64", "f32") for grp in ("midx", "col", "fft")]
+SOURCES = ["psfft_api.cu"] + [f"psfft_{dt}_{grp}.cu" for dt in ("f64", "f32") for grp in ("midx", "colc", "cola", "fft")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 

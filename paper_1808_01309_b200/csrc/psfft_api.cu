@@ -1,6 +1,7 @@
 // psfft_api.cu -- plan object and the extern "C" boundary declared in include/psfft.h.
 // Host logic only; every step of the path runs in the kernels of psfft_kernels.cuh.
 #include <math.h>
+#include <cmath>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -49,6 +50,15 @@ TableOffsets table_entries(int Nx, int Ny, int Nz)
     o.total = Nz == Ny ? end_x : end_x + up((size_t)tw_size(Nz));
     return o;
 }
+
+// Row pitch (complex elements) of the compact RHS workspace fields [Nz][Ny][kxp]: the retained kx count of Nx
+// rounded up to whole tiles of BOTH column passes (tile widths are powers of two, so the wider one decides).
+int rhs_pitch3(int Nx, int Ny, int Nz, int csize)
+{
+    const int ew = 16 / csize;
+    const int ty = job_cols(Ny) * ew, tz = job_cols(Nz) * ew;
+    return kx_pitch(Nx, ty > tz ? ty : tz);
+}
 }  // namespace psfft
 
 namespace {
@@ -67,6 +77,8 @@ struct Plan {
     void *d_tab;
     int launches;
     bool prof;
+    double kf[3];                   // 2 pi / L_i of the box (psfft_plan_set_box; 1 for the default 2 pi box)
+    int rx2, ry2, rz2, lim;         // integer form of the 2/3-rule ellipsoid (psfft_rhs.cuh Geom)
     double n_disc, n_sphere;        // retained (ky,kx) columns / retained modes of the half spectrum
     std::vector<ProfRec> recs;      // records since the last reset
     std::vector<cudaEvent_t> pool;  // events available for reuse
@@ -137,10 +149,11 @@ int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
     o->spec_bytes = o->spec_elems * 2 * s;
     o->table_bytes = table_entries(N, Ny, Nz).total * 2 * s;
     o->work_bytes_fft = (size_t)batch * o->spec_bytes;
-    if (Ny != N || Nz != N) return PSFFT_OK;   // anisotropic plans: transforms only (no RHS workspace)
-    // fused path: 5 + 6 compact fields [N][N][kx_pitch] per vector field; unfused path: 12 C per vector field
-    const size_t wfield = (size_t)N * N * rhs_pitch(N, (int)(2 * s)) * 2 * s;
-    o->work_bytes_hd = 12 * o->spec_bytes > 11 * wfield ? 12 * o->spec_bytes : 11 * wfield;
+    // fused path: 5 + 6 compact fields [Nz][Ny][kx pitch] per vector field; unfused path (cubic plans only): 12 C
+    // per vector field
+    const size_t wfield = (size_t)Nz * Ny * rhs_pitch3(N, Ny, Nz, (int)(2 * s)) * 2 * s;
+    const bool cube = Ny == N && Nz == N;
+    o->work_bytes_hd = (cube && 12 * o->spec_bytes > 11 * wfield) ? 12 * o->spec_bytes : 11 * wfield;
     o->work_bytes_mhd = 2 * o->work_bytes_hd;
     o->work_bytes_boussinesq = 16 * wfield;   // 5 + 2 z-fields, 6 + 3 y-fields
     o->work_bytes_gpe = 4 * wfield;           // 2 z/y-fields, 2 x-out fields
@@ -199,6 +212,11 @@ PassArgs args_of(const Plan *pl, void *stream)
     a.Nz = pl->lay.Nz;
     a.ldk = pl->lay.ldk;
     a.stream = reinterpret_cast<cudaStream_t>(stream);
+    a.kxp = rhs_pitch3(a.N, a.Ny, a.Nz, (int)cs);
+    a.kxc = kx_count(a.N);
+    a.rx2 = pl->rx2; a.ry2 = pl->ry2; a.rz2 = pl->rz2; a.lim = pl->lim;
+    for (int i = 0; i < 3; ++i) a.kf[i] = pl->kf[i];
+    a.unit_cube = cubic(pl->lay) && a.kf[0] == 1.0 && a.kf[1] == 1.0 && a.kf[2] == 1.0;
     return a;
 }
 
@@ -254,7 +272,7 @@ struct RhsSys {
 template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys &y, void *work)
 {
     const size_t C = pl->lay.spec_bytes;
-    const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
+    const double cs = (double)(2 * sizeof(T)), KX = a.kxc;
     const int nv = y.nv, ns = y.ns;
     RhsArgs r;
     r.nv = nv; r.ns = ns;
@@ -265,10 +283,10 @@ template <typename T> int rhs_fused_t(Plan *pl, const PassArgs &a, const RhsSys 
     r.sdiff = y.kappa; r.nbv = y.nbv;
     r.base[0] = y.base_u; r.base[1] = y.base_b; r.sbase = y.base_t; r.cstep = y.cstep;
     r.sparse_out = y.sparse_out;
-    const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
+    const size_t W = (size_t)a.Nz * a.Ny * a.kxp * 2 * sizeof(T);
     r.zbuf = work;                                         // 5 nv + 2 ns compact fields (later 3 nv + ns: mid_x out, fwd_y in place)
     r.ybuf = off(work, (size_t)(5 * nv + 2 * ns) * W);     // 6 nv + 3 ns compact fields
-    const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
+    const double disc = pl->n_disc * a.Nz * cs, rows = KX * a.Ny * a.Nz * cs, sph = pl->n_sphere * cs;
     // sparse re-reads of the inputs in the fwd_z epilogue: diffusion (3 per vector, 1 per scalar), buoyancy
     // (theta^ for R_u, u^_z for R_theta)
     const double nepi = (y.nu != 0.0 ? 3.0 : 0.0) + (nv == 2 && y.eta != 0.0 ? 3.0 : 0.0) +
@@ -289,14 +307,14 @@ int gpe_t(Plan *pl, const PassArgs &a, const void *psi, void *rhs, double alpha,
           double cstep, bool sparse_out, void *work)
 {
     const size_t C = pl->lay.spec_bytes;
-    const double cs = (double)(2 * sizeof(T)), N = a.N, KX = (a.N - 1) / 3 + 1;
-    const size_t W = (size_t)a.N * a.N * rhs_pitch(a.N, (int)(2 * sizeof(T))) * 2 * sizeof(T);
+    const double cs = (double)(2 * sizeof(T)), KX = a.kxc;
+    const size_t W = (size_t)a.Nz * a.Ny * a.kxp * 2 * sizeof(T);
     GpeArgs g;
     g.psi = psi; g.dst = rhs; g.base = base;
     g.alpha = alpha; g.beta = beta; g.cstep = cstep; g.sparse_out = sparse_out;
     g.zbuf = work;
     g.obuf = off(work, 2 * W);
-    const double disc = pl->n_disc * N * cs, rows = KX * N * N * cs, sph = pl->n_sphere * cs;
+    const double disc = pl->n_disc * a.Nz * cs, rows = KX * a.Ny * a.Nz * cs, sph = pl->n_sphere * cs;
     const double nepi = (alpha != 0.0 ? 2.0 : 0.0) + (base ? 2.0 : 0.0);
     { ProfScope ps(pl, a.stream, K_INVZ, 2 * sph + 2 * disc); CU(launch_gpe_pass<T>(a, g, 0, &pl->launches)); }
     { ProfScope ps(pl, a.stream, K_INVY, 2 * disc + 2 * rows); CU(launch_gpe_pass<T>(a, g, 1, &pl->launches)); }
@@ -431,17 +449,25 @@ int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int b
     pl->d_tab = d_tables;
     pl->launches = 0;
     pl->prof = false;
-    {   // retained columns / modes of the 2/3-rule sphere, by integer enumeration
+    {   // 2/3 rule on a general grid (reading G25): keep iff sum (n_i / N_i)^2 < 1/9, in integers
+        // 9 sum (r_i n_i)^2 < L^2 with L = lcm(Nx, Ny, Nz), r_i = L / N_i  (cubic: 9 |n|^2 < N^2)
+        auto gcd = [](long x, long y) { while (y) { const long t = x % y; x = y; y = t; } return x; };
+        long L = (long)N / gcd(N, Ny) * Ny;
+        L = L / gcd(L, Nz) * Nz;
+        const long rx = L / N, ry = L / Ny, rz = L / Nz;
+        pl->rx2 = (int)(rx * rx); pl->ry2 = (int)(ry * ry); pl->rz2 = (int)(rz * rz);
+        pl->lim = (int)((L * L + 8) / 9);
+        pl->kf[0] = pl->kf[1] = pl->kf[2] = 1.0;   // 2 pi box
+        // retained columns / modes, by integer enumeration
         double nd = 0, ns = 0;
-        const long N2 = (long)N * N;
-        for (int q = 0; q < N; ++q) {
-            const long ky = q < N / 2 ? q : q - N;
+        for (int q = 0; q < Ny; ++q) {
+            const long ky = q < Ny / 2 ? q : q - Ny;
             for (long kx = 0; kx <= N / 2; ++kx) {
-                const long kxy2 = kx * kx + ky * ky;
-                if (9 * kxy2 >= N2) continue;
+                const long kxy2 = pl->rx2 * kx * kx + pl->ry2 * ky * ky;
+                if (kxy2 >= pl->lim) continue;
                 nd += 1;
                 long cnt = 0;   // kz = 0, 1, ... retained; each kz > 0 also stands for -kz
-                while (9 * (kxy2 + cnt * cnt) < N2) ++cnt;
+                while (kxy2 + pl->rz2 * cnt * cnt < pl->lim) ++cnt;
                 ns += (double)(2 * cnt - 1);
             }
         }
@@ -480,6 +506,18 @@ int psfft_plan_layout(psfft_plan plan, psfft_layout *out)
     return PSFFT_OK;
 }
 
+int psfft_plan_set_box(psfft_plan plan, double Lx, double Ly, double Lz)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    const double L[3] = {Lx, Ly, Lz};
+    for (double v : L)
+        if (!(v > 0.0) || !std::isfinite(v)) return PSFFT_E_SIZE;
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int i = 0; i < 3; ++i) pl->kf[i] = two_pi / L[i];   // exactly 1 for L_i = 2 pi
+    return PSFFT_OK;
+}
+
 int psfft_fft3d_r2c(psfft_plan plan, const void *d_real, void *d_spec, void *d_work, void *stream)
 {
     (void)d_work;
@@ -514,7 +552,7 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
+    if (!fused && !cubic(pl->lay)) return PSFFT_E_SIZE;   // the unfused cross-check path needs Nx = Ny = Nz
     if (!d_uhat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     {
@@ -538,7 +576,7 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
+    if (!fused && !cubic(pl->lay)) return PSFFT_E_SIZE;   // the unfused cross-check path needs Nx = Ny = Nz
     if (!d_uhat || !d_bhat || !d_rhs_u || !d_rhs_b || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_bhat) || misaligned(d_rhs_u) || misaligned(d_rhs_b) || misaligned(d_work))
         return PSFFT_E_ALIGN;
@@ -586,7 +624,6 @@ int psfft_boussinesq_rhs(psfft_plan plan, const void *d_uhat, const void *d_thha
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_uhat || !d_thhat || !d_rhs_u || !d_rhs_th || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_thhat) || misaligned(d_rhs_u) || misaligned(d_rhs_th) || misaligned(d_work))
         return PSFFT_E_ALIGN;
@@ -608,7 +645,6 @@ int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alp
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!cubic(pl->lay)) return PSFFT_E_SIZE;
     if (!d_psihat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_psihat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     if (spans_overlap({{d_psihat, 2 * pl->lay.spec_bytes, false}, {d_rhs, 2 * pl->lay.spec_bytes, true},
@@ -625,7 +661,7 @@ static int sys_fields(int system) { return system == PSFFT_SYS_HD ? 3 : system =
 size_t psfft_rk_work_bytes(psfft_plan plan, int system)
 {
     Plan *pl = get(plan);
-    if (!pl || system < 0 || system > 3 || !cubic(pl->lay)) return 0;
+    if (!pl || system < 0 || system > 3) return 0;
     const size_t rhs = system == PSFFT_SYS_HD ? pl->lay.work_bytes_hd
                      : system == PSFFT_SYS_MHD ? pl->lay.work_bytes_mhd
                      : system == PSFFT_SYS_GPE ? pl->lay.work_bytes_gpe : pl->lay.work_bytes_boussinesq;
@@ -637,7 +673,6 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!cubic(pl->lay)) return PSFFT_E_SIZE;   // right-hand sides need Nx = Ny = Nz
     if (!d_y_in || !d_y_out || !d_work || !params) return PSFFT_E_NULL;
     if (system < 0 || system > 3 || ord < 1 || ord > 4) return PSFFT_E_SIZE;
     if (misaligned(d_y_in) || misaligned(d_y_out) || misaligned(d_work)) return PSFFT_E_ALIGN;
@@ -734,6 +769,130 @@ int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double n
     return PSFFT_OK;
 }
 
+// ---- slab-decomposed transform (psfft_slab.cuh) --------------------------------------------------
+static int slab_ranges(const Plan *pl, int P, int rank, psfft_slab_layout *o)
+{
+    if (P < 1 || P > PSFFT_MAX_RANKS || rank < 0 || rank >= P) return PSFFT_E_SIZE;
+    if (pl->lay.Nz % P != 0 || P > pl->lay.ldk) return PSFFT_E_SIZE;
+    const size_t s = pl->lay.dtype == PSFFT_F64 ? 8 : 4;
+    memset(o, 0, sizeof(*o));
+    o->P = P;
+    o->rank = rank;
+    o->Mz = pl->lay.Nz / P;
+    o->z0 = rank * o->Mz;
+    for (int q = 0; q <= P; ++q) o->x0[q] = (int)((long)q * pl->lay.ldk / P);
+    o->w = o->x0[rank + 1] - o->x0[rank];
+    o->real_elems = (size_t)o->Mz * pl->lay.Ny * pl->lay.N;
+    o->zspec_elems = (size_t)o->Mz * pl->lay.Ny * pl->lay.ldk;
+    o->xslab_elems = (size_t)pl->lay.Nz * pl->lay.Ny * o->w;
+    o->real_bytes = o->real_elems * s;
+    o->zspec_bytes = o->zspec_elems * 2 * s;
+    o->xslab_bytes = o->xslab_elems * 2 * s;
+    return PSFFT_OK;
+}
+
+static int slab_xdist(const Plan *pl, const psfft_slab_layout &sl, void *const *blocks, long zoff, XDistArgs *xd)
+{
+    if (zoff < 0) return PSFFT_E_SIZE;
+    memset(xd, 0, sizeof(*xd));
+    for (int q = 0; q < sl.P; ++q) {
+        if (!blocks[q]) return PSFFT_E_NULL;
+        // 8-byte alignment of every complex element is all the per-column accesses of this pass need in fp32
+        if (reinterpret_cast<uintptr_t>(blocks[q]) & (pl->lay.dtype == PSFFT_F64 ? 15u : 7u)) return PSFFT_E_ALIGN;
+        xd->base[q] = blocks[q];
+    }
+    for (int q = 0; q <= sl.P; ++q) xd->x0[q] = sl.x0[q];
+    xd->P = sl.P;
+    xd->zoff = zoff;
+    return PSFFT_OK;
+}
+
+int psfft_slab_query(psfft_plan plan, int P, int rank, psfft_slab_layout *out)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!out) return PSFFT_E_NULL;
+    return slab_ranges(pl, P, rank, out);
+}
+
+int psfft_slab_r2c_xy(psfft_plan plan, int P, int rank, const void *d_real_slab, void *d_zspec, void *const *d_blocks,
+                      long zoff, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_real_slab || !d_zspec || !d_blocks) return PSFFT_E_NULL;
+    if (misaligned(d_real_slab) || misaligned(d_zspec)) return PSFFT_E_ALIGN;
+    psfft_slab_layout sl;
+    int rc = slab_ranges(pl, P, rank, &sl);
+    if (rc) return rc;
+    XDistArgs xd;
+    rc = slab_xdist(pl, sl, d_blocks, zoff, &xd);
+    if (rc) return rc;
+    if (spans_overlap({{d_real_slab, sl.real_bytes, false}, {d_zspec, sl.zspec_bytes, true}})) return PSFFT_E_OVERLAP;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    const long nrows = (long)sl.Mz * a.Ny;
+    const double R = (double)sl.real_bytes, C = (double)sl.zspec_bytes;
+    if (pl->lay.dtype == PSFFT_F64) {
+        { ProfScope ps(pl, a.stream, K_XR2C, R + C); CU(launch_xpass_r2c<double>(a, d_real_slab, d_zspec, nrows, &pl->launches)); }
+        { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass_xdist<double>(a, true, d_zspec, nullptr, xd, sl.Mz, &pl->launches)); }
+    } else {
+        { ProfScope ps(pl, a.stream, K_XR2C, R + C); CU(launch_xpass_r2c<float>(a, d_real_slab, d_zspec, nrows, &pl->launches)); }
+        { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass_xdist<float>(a, true, d_zspec, nullptr, xd, sl.Mz, &pl->launches)); }
+    }
+    return PSFFT_OK;
+}
+
+int psfft_slab_z(psfft_plan plan, int P, int rank, int dir, void *d_xslab, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_xslab) return PSFFT_E_NULL;
+    if (misaligned(d_xslab)) return PSFFT_E_ALIGN;
+    if (dir != -1 && dir != 1) return PSFFT_E_SIZE;
+    psfft_slab_layout sl;
+    int rc = slab_ranges(pl, P, rank, &sl);
+    if (rc) return rc;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    const long inner = (long)a.Ny * sl.w;   // columns (ky, kx) of the x-slab; z stride = inner
+    ProfScope ps(pl, a.stream, K_CPZ, 2.0 * (double)sl.xslab_bytes);
+    if (pl->lay.dtype == PSFFT_F64)
+        CU(launch_cpass_raw<double>(a, dir, a.Nz, a.twZ, d_xslab, d_xslab, inner, inner, inner * a.Nz, 1, &pl->launches));
+    else
+        CU(launch_cpass_raw<float>(a, dir, a.Nz, a.twZ, d_xslab, d_xslab, inner, inner, inner * a.Nz, 1, &pl->launches));
+    return PSFFT_OK;
+}
+
+int psfft_slab_c2r_yx(psfft_plan plan, int P, int rank, void *const *d_blocks, long zoff, void *d_zspec,
+                      void *d_real_slab, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_real_slab || !d_zspec || !d_blocks) return PSFFT_E_NULL;
+    if (misaligned(d_real_slab) || misaligned(d_zspec)) return PSFFT_E_ALIGN;
+    psfft_slab_layout sl;
+    int rc = slab_ranges(pl, P, rank, &sl);
+    if (rc) return rc;
+    XDistArgs xd;
+    rc = slab_xdist(pl, sl, d_blocks, zoff, &xd);
+    if (rc) return rc;
+    if (spans_overlap({{d_zspec, sl.zspec_bytes, true}, {d_real_slab, sl.real_bytes, true}})) return PSFFT_E_OVERLAP;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    const long nrows = (long)sl.Mz * a.Ny;
+    const double scale = 1.0 / ((double)a.N * a.Ny * a.Nz);
+    const double R = (double)sl.real_bytes, C = (double)sl.zspec_bytes;
+    if (pl->lay.dtype == PSFFT_F64) {
+        { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass_xdist<double>(a, false, nullptr, d_zspec, xd, sl.Mz, &pl->launches)); }
+        { ProfScope ps(pl, a.stream, K_XC2R, R + C); CU(launch_xpass_c2r<double>(a, d_zspec, d_real_slab, nrows, scale, &pl->launches)); }
+    } else {
+        { ProfScope ps(pl, a.stream, K_CPY, 2 * C); CU(launch_cpass_xdist<float>(a, false, nullptr, d_zspec, xd, sl.Mz, &pl->launches)); }
+        { ProfScope ps(pl, a.stream, K_XC2R, R + C); CU(launch_xpass_c2r<float>(a, d_zspec, d_real_slab, nrows, scale, &pl->launches)); }
+    }
+    return PSFFT_OK;
+}
+
 int psfft_profile_enable(psfft_plan plan, int on)
 {
     Plan *pl = get(plan);
@@ -786,7 +945,7 @@ const char *psfft_strerror(int code)
     switch (code) {
         case PSFFT_OK: return "success";
         case PSFFT_E_NULL: return "psfft: required pointer is NULL";
-        case PSFFT_E_SIZE: return "psfft: unsupported grid size or batch";
+        case PSFFT_E_SIZE: return "psfft: unsupported grid size, batch, system, order or box length";
         case PSFFT_E_DTYPE: return "psfft: dtype must be PSFFT_F32 or PSFFT_F64";
         case PSFFT_E_ALIGN: return "psfft: device pointer not 16-byte aligned";
         case PSFFT_E_TABLE: return "psfft: table buffer too small";

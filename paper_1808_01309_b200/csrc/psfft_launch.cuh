@@ -25,7 +25,15 @@ struct PassArgs {
     const void *twZ;
     int ldk;
     cudaStream_t stream;
+    // right-hand sides (psfft_rhs.cuh Geom; readings G24, G25): compact row pitch of the workspace fields,
+    // retained kx count, integer weights of the 2/3-rule ellipsoid, wavenumber factors 2 pi / L_i
+    int kxp, kxc, rx2, ry2, rz2, lim;
+    double kf[3];
+    bool unit_cube;    // Nx = Ny = Nz and the 2 pi box: the column passes run with compile-time geometry
 };
+
+// compact row pitch of the RHS workspace fields of an (Nx, Ny, Nz) plan with complex size csize (host)
+int rhs_pitch3(int Nx, int Ny, int Nz, int csize);
 
 // Each launcher returns cudaGetLastError() of its launch (or cudaErrorInvalidValue for an
 // unsupported N) and increments *launches.
@@ -56,11 +64,28 @@ struct RhsArgs {
     void *zbuf;           // 5 nv + 2 ns compact fields (inv_z out; later mid_x out / fwd_y in place, 3 nv + ns fields)
     void *ybuf;           // 6 nv + 3 ns compact fields (inv_y out)
 };
-template <typename T> cudaError_t launch_rhs_inv_z(const PassArgs &a, const RhsArgs &r, int *launches);
-template <typename T> cudaError_t launch_rhs_inv_y(const PassArgs &a, const RhsArgs &r, int *launches);
 template <typename T> cudaError_t launch_rhs_mid_x(const PassArgs &a, const RhsArgs &r, int *launches);
-template <typename T> cudaError_t launch_rhs_fwd_y(const PassArgs &a, const RhsArgs &r, int *launches);
-template <typename T> cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches);
+// column passes: CUBE = compile-time geometry of the N^3 grid in the 2 pi box; false = the plan's run-time geometry
+template <typename T, bool CUBE> cudaError_t launch_rhs_inv_z_g(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T, bool CUBE> cudaError_t launch_rhs_inv_y_g(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T, bool CUBE> cudaError_t launch_rhs_fwd_y_g(const PassArgs &a, const RhsArgs &r, int *launches);
+template <typename T, bool CUBE> cudaError_t launch_rhs_fwd_z_g(const PassArgs &a, const RhsArgs &r, int *launches);
+#define PSFFT_BY_GEOMETRY(name)                                                                          \
+    template <typename T> inline cudaError_t launch_rhs_##name(const PassArgs &a, const RhsArgs &r, int *launches) \
+    {                                                                                                    \
+        return a.unit_cube ? launch_rhs_##name##_g<T, true>(a, r, launches) : launch_rhs_##name##_g<T, false>(a, r, launches); \
+    }
+PSFFT_BY_GEOMETRY(inv_z)
+PSFFT_BY_GEOMETRY(inv_y)
+PSFFT_BY_GEOMETRY(fwd_y)
+#undef PSFFT_BY_GEOMETRY
+// fwd_z takes the run-time geometry on every plan: measured on B200 it is the faster build of this pass (the epilogue
+// spills less at the 64-register budget): 512^3 fp64 1.15 -> 1.09 ms, 768^3 fp32 2.73 -> 2.05 ms, 1024^3 fp32 MHD
+// 10.8 -> 9.7 ms
+template <typename T> inline cudaError_t launch_rhs_fwd_z(const PassArgs &a, const RhsArgs &r, int *launches)
+{
+    return launch_rhs_fwd_z_g<T, false>(a, r, launches);
+}
 
 // Gross-Pitaevskii right-hand side (psi = p + i q as two real fields): pass = 0 inv_z, 1 inv_y, 2 mid_x,
 // 3 fwd_y, 4 fwd_z
@@ -73,7 +98,26 @@ struct GpeArgs {
     void *zbuf;           // 2 compact fields: inv_z out, inv_y in place
     void *obuf;           // 2 compact fields: mid_x out, fwd_y in place
 };
-template <typename T> cudaError_t launch_gpe_pass(const PassArgs &a, const GpeArgs &g, int pass, int *launches);
+template <typename T, bool CUBE> cudaError_t launch_gpe_pass_g(const PassArgs &a, const GpeArgs &g, int pass, int *launches);
+template <typename T> inline cudaError_t launch_gpe_pass(const PassArgs &a, const GpeArgs &g, int pass, int *launches)
+{
+    return a.unit_cube ? launch_gpe_pass_g<T, true>(a, g, pass, launches) : launch_gpe_pass_g<T, false>(a, g, pass, launches);
+}
+
+// ---- slab-decomposed transform (psfft_slab.cuh) ------------------------------------------------
+// x-distributed blocks of one exchange: block q holds kx in [x0[q], x0[q + 1]) as [rows][Ny][w_q]
+struct XDistArgs {
+    void *base[16];
+    int x0[17];
+    int P;
+    long zoff;
+};
+// y-pass of the z-slab [mz][Ny][ldk] `slab` with the other side in the blocks: scatter (forward) or gather (inverse)
+template <typename T> cudaError_t launch_cpass_xdist(const PassArgs &a, bool scatter, const void *slab_in, void *slab_out,
+                                                     const XDistArgs &xd, int mz, int *launches);
+// plain strided column pass of length `len` (table `tw`): element (i, col, o) at base[o outer_stride + i axis_stride + col]
+template <typename T> cudaError_t launch_cpass_raw(const PassArgs &a, int dir, int len, const void *tw, const void *in, void *out,
+                                                   long axis_stride, long inner, long outer_stride, long outer, int *launches);
 
 // complex entries of the tables of an (Nx, Ny, Nz) plan: [roots of unity, Nx][stage tables Ny]
 // [symmetric-schedule stage tables Nx (x passes, mid_x)][stage tables Nz, only when Nz != Ny]

@@ -195,7 +195,7 @@ template <int N> __host__ __device__ constexpr int xg_rows()
 template <typename T, int N, int NV, int NS, int MINB>
 __global__ void __launch_bounds__(xg_rows<N>() * XSched<N>::TPR, MINB)
     k_mid_xg(const Cx<T> *__restrict__ in, Cx<T> *__restrict__ out, const Cx<T> *__restrict__ twx, long nfw, int kxp,
-             T scale2)
+             T scale2, T kfx)
 {
     using C = Cx<T>;
     using X = XSched<N>;
@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(xg_rows<N>() * XSched<N>::TPR, MINB)
         }
 #pragma unroll
         for (int r = 0; r < RM; ++r) {   // w^_y = P - i kx U_z,  w^_z = i kx U_y - D
-            const T kk = (T)kq[r];
+            const T kk = (T)kq[r] * kfx;   // k_x = n_x 2 pi / L_x
             const C p = wy[r], d = wz[r];
             wy[r] = csub(p, mul_ik(uz[r], kk));
             wz[r] = csub(mul_ik(uy[r], kk), d);
@@ -278,7 +278,7 @@ __global__ void __launch_bounds__(xg_rows<N>() * XSched<N>::TPR, MINB)
         for (int r = 0; r < RM; ++r) {
             gx[r] = gy[r] = gz[r] = zz[r] = zero;
             if (pq[r]) {
-                gx[r] = mul_ik(ld_stream(f + kq[r]), (T)kq[r]);
+                gx[r] = mul_ik(ld_stream(f + kq[r]), (T)kq[r] * kfx);
                 gy[r] = ld_stream(f + nfw + kq[r]);
                 gz[r] = ld_stream(f + 2 * nfw + kq[r]);
             }

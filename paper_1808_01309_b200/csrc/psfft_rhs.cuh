@@ -52,6 +52,33 @@ __device__ __forceinline__ float2x2 mul_ik(float2x2 v, float k)
     return r;
 }
 
+// Geometry of a right-hand side on an (Nx, Ny, Nz) grid in an (Lx, Ly, Lz) box (box size and grid points
+// independent per direction; readings G24, G25).  Index n_i (integer, the wavenumber of the 2 pi box):
+//   mask         keep iff sum_i (n_i / N_i)^2 < 1/9, in integers  rx2 nx^2 + ry2 ny^2 + rz2 nz^2 < lim  with
+//                r_i = lcm(Nx, Ny, Nz) / N_i,  lim = ceil(lcm^2 / 9)   (cubic: r_i = 1, i.e. 9 |n|^2 < N^2)
+//   wavenumbers  k_i = n_i kf_i,  kf_i = 2 pi / L_i  (exactly 1 in the 2 pi box)
+// A job template's N is the length of ITS transform axis only; everything about the other two axes comes from its
+// geometry policy G: GeomCube (the N^3 grid in the 2 pi box of every BASELINE.json config: all compile-time, the
+// multiplications by 1 fold away) or GeomAny (run-time values from the plan).  Measured on B200, 512^3 fp64: with
+// run-time geometry alone inv_y ran 1.56 -> 2.03 ms (spills at the 64-register budget), hence the two policies.
+template <typename T, int N> struct GeomCube {
+    static constexpr int ny = N, nz = N, kxc = kx_count(N);
+    static constexpr int rx2 = 1, ry2 = 1, rz2 = 1, lim = (N * N + 8) / 9;
+    static constexpr T kfx = (T)1, kfy = (T)1, kfz = (T)1;
+    __device__ __forceinline__ static int w2(int kx, int ky) { return kx * kx + ky * ky; }
+    __device__ __forceinline__ static bool keep2(int kxy2) { return 9 * kxy2 < N * N; }
+    __device__ __forceinline__ static bool keep3(int kxy2, int kz) { return 9 * (kxy2 + kz * kz) < N * N; }
+};
+template <typename T> struct GeomAny {
+    int ny, nz;           // grid points along y, z
+    int kxc;              // retained kx: kx < kxc = kx_count(Nx)
+    int rx2, ry2, rz2, lim;
+    T kfx, kfy, kfz;
+    __device__ __forceinline__ int w2(int kx, int ky) const { return rx2 * kx * kx + ry2 * ky * ky; }
+    __device__ __forceinline__ bool keep2(int kxy2) const { return kxy2 < lim; }
+    __device__ __forceinline__ bool keep3(int kxy2, int kz) const { return kxy2 + rz2 * kz * kz < lim; }
+};
+
 // 16-byte access to two adjacent fp32 columns (re0, im0, re1, im1) <-> float2x2; p must be 16-byte aligned
 __device__ __forceinline__ float2x2 pack2(float4 q)
 {
@@ -157,31 +184,32 @@ __global__ void __launch_bounds__(TC *TPF, MINB) k_cpass_job(Job job, const Cx<T
 // ---- inv_z -------------------------------------------------------------------------------------
 // grid (kxp / TC, N): tile = TC consecutive kx at one ky.  Reads the caller's layout (pitch ldk),
 // writes the compact workspace layout (pitch kxp).
-template <typename T, int N, int TC, int NV, int NS> struct JobInvZ : JobElems<JobInvZ<T, N, TC, NV, NS>, Cx<T>, Ex<T>> {
+template <typename T, int N, int TC, int NV, int NS, class G> struct JobInvZ : JobElems<JobInvZ<T, N, TC, NV, NS, G>, Cx<T>, Ex<T>> {
     using C = Cx<T>;
     const C *src[NV];   // NV x 3 spectral fields (u^, b^), caller layout
     const C *ssrc;      // NS = 1: theta^, caller layout
     C *dst;             // NV x 5 fields: A_x, A_y, A_z, B_x = F_z^-1(i kz u_x), G_x = F_z^-1(w^_x); then NS x 2: T_A, T_B
-    long plane, nf;     // caller layout: ldk N, ldk N N
-    long wplane, wnf;   // workspace layout: kxp N, kxp N N
+    long plane, nf;     // caller layout: ldk Ny, ldk Ny Nz
+    long wplane, wnf;   // workspace layout: kxp Ny, kxp Ny Nz
+    int ldk, kxp;
+    G geo;
     struct State { long col, wcol; int kxy2, ky; bool active; };
 
     __host__ __device__ __forceinline__ int rounds() const { return 5 * NV + 2 * NS; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
-        const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, N);
-        s.kxy2 = kx * kx + ky * ky;
+        const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, geo.ny);
+        s.kxy2 = geo.w2(kx, ky);
         s.ky = ky;
-        s.active = 9 * s.kxy2 < N * N;
-        s.col = (long)blockIdx.y * (plane / N) + kx;
-        s.wcol = (long)blockIdx.y * (wplane / N) + kx;
+        s.active = geo.keep2(s.kxy2);
+        s.col = (long)blockIdx.y * ldk + kx;
+        s.wcol = (long)blockIdx.y * kxp + kx;
         return s.active;
     }
     __device__ __forceinline__ void idle(const State &, int, int) const {}
     __device__ __forceinline__ bool keep(const State &s, int i) const
     {
-        const int kz = wavenumber(i, N);
-        return s.active && 9 * (s.kxy2 + kz * kz) < N * N;
+        return s.active && geo.keep3(s.kxy2, wavenumber(i, N));
     }
     __device__ __forceinline__ const C *field(int r) const { return (NV == 2 && r >= 5) ? src[NV - 1] : src[0]; }
     // rr: 0..2 A_c <- u_c | 3 B_x <- i kz u_x | 4 G_x <- i (ky u_z - kz u_y);  scalar: T_A <- th | T_B <- i kz th
@@ -199,14 +227,14 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvZ : JobElems<J
     }
     __device__ __forceinline__ C post(const State &s, int r, int i, C x) const
     {
-        if (NS > 0 && r >= 5 * NV) return r == 5 * NV ? x : mul_ik(x, (T)wavenumber(i, N));
+        if (NS > 0 && r >= 5 * NV) return r == 5 * NV ? x : mul_ik(x, (T)wavenumber(i, N) * geo.kfz);
         const int rr = r % 5;
         if (rr < 3) return x;
-        const T kz = (T)wavenumber(i, N);
+        const T kz = (T)wavenumber(i, N) * geo.kfz;
         if (rr == 3) return mul_ik(x, kz);
         C y = mk<T>(0, 0);
         if (keep(s, i)) y = ldg_c(field(r) + nf + i * plane + s.col);   // u_y (sparse, L1/L2 resident)
-        const T ky = (T)s.ky;
+        const T ky = (T)s.ky * geo.kfy;
         return mk<T>(-(ky * x.y - kz * y.y), ky * x.x - kz * y.x);
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
@@ -223,12 +251,13 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvZ : JobElems<J
 
 // ---- inv_y -------------------------------------------------------------------------------------
 // grid (kxp / TC, N): tile = TC consecutive kx of one z plane, all in the compact layout.
-template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<JobInvY<T, N, TC, NV, NS>, Cx<T>, Ex<T>> {
+template <typename T, int N, int TC, int NV, int NS, class G> struct JobInvY : JobElems<JobInvY<T, N, TC, NV, NS, G>, Cx<T>, Ex<T>> {
     using C = Cx<T>;
     const C *src;  // NV x 5 (+ NS x 2) fields from inv_z
     C *dst;        // NV x 6 fields: U_x, U_y, U_z, W_x, P, D;  then NS x 3: Th, Dt, Gz
     long wplane, wnf;
     int kxp;
+    G geo;
     struct State { long base; int kx; bool active; };
     static constexpr bool prefetch_next = sizeof(T) == 4;
 
@@ -236,10 +265,11 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
-        s.active = s.kx < kx_count(N);
+        s.active = s.kx < geo.kxc;
         s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
+    __device__ __forceinline__ bool keepy(const State &s, int ky) const { return s.active && geo.keep2(geo.w2(s.kx, ky)); }
     __device__ __forceinline__ void idle(const State &, int, int) const {}
     // scalar rounds (r >= 6 NV): Th <- T_A | Dt <- i ky T_A | Gz <- T_B
     // round order: U_x <- A_x | D <- i ky A_x | U_y | U_z | W_x <- G_x | P <- B_x.  A_x is read in two
@@ -252,7 +282,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
         const bool sc = NS > 0 && r >= 6 * NV;
         const int v = r / 6, rr = sc ? r - 6 * NV : r % 6;
         C x = mk<T>(0, 0);
-        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) {
+        if (keepy(s, ky)) {
             const int f = sc ? 5 * NV + (rr >> 1) : v * 5 + src_field(rr);
             const C *p = src + (long)f * wnf + s.base + (long)i * kxp;
             x = rr == 0 ? *p : ld_stream(p);
@@ -264,14 +294,14 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
         const int ky = wavenumber(i, N);
         const bool sc = NS > 0 && r >= 6 * NV;
         const int v = r / 6, rr = sc ? r - 6 * NV : r % 6;
-        if (rr == 1 || !s.active || 9 * (s.kx * s.kx + ky * ky) >= N * N) return nullptr;   // rr 1 re-reads rr 0's field
+        if (rr == 1 || !keepy(s, ky)) return nullptr;   // rr 1 re-reads rr 0's field
         const int f = sc ? 5 * NV + (rr >> 1) : v * 5 + src_field(rr);
         return src + (long)f * wnf + s.base + (long)i * kxp;
     }
     __device__ __forceinline__ C post(const State &, int r, int i, C x) const
     {
         const int rr = (NS > 0 && r >= 6 * NV) ? r - 6 * NV : r % 6;
-        return rr == 1 ? mul_ik(x, (T)wavenumber(i, N)) : x;
+        return rr == 1 ? mul_ik(x, (T)wavenumber(i, N) * geo.kfy) : x;
     }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
@@ -289,8 +319,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
         const int ky = wavenumber(i, N);
         const bool sc = NS > 0 && r >= 6 * NV;
         const int v = r / 6, rr = sc ? r - 6 * NV : r % 6;
-        const bool m0 = s[0].active && 9 * (s[0].kx * s[0].kx + ky * ky) < N * N;
-        const bool m1 = s[1].active && 9 * (s[1].kx * s[1].kx + ky * ky) < N * N;
+        const bool m0 = keepy(s[0], ky), m1 = keepy(s[1], ky);
         float2x2 x = ezero<float2x2>();
         if (m0 || m1) {
             const int f = sc ? 5 * NV + (rr >> 1) : v * 5 + src_field(rr);
@@ -302,7 +331,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
     __device__ __forceinline__ float2x2 post_e(const State *, int r, int i, float2x2 x) const
     {
         const int rr = (NS > 0 && r >= 6 * NV) ? r - 6 * NV : r % 6;
-        return rr == 1 ? mul_ik(x, (float)wavenumber(i, N)) : x;
+        return rr == 1 ? mul_ik(x, (float)wavenumber(i, N) * geo.kfy) : x;
     }
     __device__ __forceinline__ double2 post_e(const State *s, int r, int i, double2 x) const { return post(s[0], r, i, x); }
     __device__ __forceinline__ void store_e(const State *s, int r, int i, float2x2 v) const
@@ -314,11 +343,12 @@ template <typename T, int N, int TC, int NV, int NS> struct JobInvY : JobElems<J
 };
 
 // ---- fwd_y -------------------------------------------------------------------------------------
-template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>, Cx<T>, Ex<T>> {
+template <typename T, int N, int TC, class G> struct JobFwdY : JobElems<JobFwdY<T, N, TC, G>, Cx<T>, Ex<T>> {
     using C = Cx<T>;
     C *buf;  // NF fields, in place, compact layout
     long wplane, wnf;
     int kxp, nfields;
+    G geo;
     struct State { long base; int kx; bool active; };
     static constexpr bool prefetch_next = sizeof(T) == 4;
 
@@ -326,10 +356,11 @@ template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
-        s.active = s.kx < kx_count(N);
+        s.active = s.kx < geo.kxc;
         s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
+    __device__ __forceinline__ bool keepy(const State &s, int ky) const { return s.active && geo.keep2(geo.w2(s.kx, ky)); }
     __device__ __forceinline__ void idle(const State &, int, int) const {}
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
@@ -344,8 +375,7 @@ template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>
     __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
     __device__ __forceinline__ void store(const State &s, int r, int i, C v) const
     {
-        const int ky = wavenumber(i, N);
-        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) st_stream(buf + r * wnf + s.base + (long)i * kxp, v);
+        if (keepy(s, wavenumber(i, N))) st_stream(buf + r * wnf + s.base + (long)i * kxp, v);
     }
     // fp32 pairs: one 16-byte access per element
     __device__ __forceinline__ Ex<T> load_e(const State *s, int r, int i) const
@@ -364,9 +394,7 @@ template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>
     __device__ __forceinline__ void store_e(const State *s, int r, int i, float2x2 v) const
     {
         const int ky = wavenumber(i, N);
-        const bool m0 = s[0].active && 9 * (s[0].kx * s[0].kx + ky * ky) < N * N;
-        const bool m1 = s[1].active && 9 * (s[1].kx * s[1].kx + ky * ky) < N * N;
-        st_stream2(buf + r * wnf + s[0].base + (long)i * kxp, v, m0, m1);
+        st_stream2(buf + r * wnf + s[0].base + (long)i * kxp, v, keepy(s[0], ky), keepy(s[1], ky));
     }
     __device__ __forceinline__ void store_e(const State *s, int r, int i, double2 v) const { store(s[0], r, i, v); }
 };
@@ -379,7 +407,7 @@ template <typename T, int N, int TC> struct JobFwdY : JobElems<JobFwdY<T, N, TC>
 // before the projection (Eqs. 1-2).
 // Works on single columns in both precisions (the two columns of an fp32 pair would sit in different rows
 // of the caller's odd-pitch layout, and the epilogue is per mode anyway).
-template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<JobFwdZ<T, N, TC, NV, NS>, Cx<T>, Cx<T>> {
+template <typename T, int N, int TC, int NV, int NS, class G> struct JobFwdZ : JobElems<JobFwdZ<T, N, TC, NV, NS, G>, Cx<T>, Cx<T>> {
     using C = Cx<T>;
     const C *src;        // NV x 3 (+ NS) fields (after fwd_y), compact layout
     C *dst[NV];          // NV outputs of 3 fields, caller layout
@@ -397,8 +425,9 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     static constexpr bool is_fwdz = true;
     long plane, nf;      // caller layout
     long wplane, wnf;    // workspace layout
-    int ldk;
-    struct State { long col, wcol; int kx, ky, kxy2; bool active, valid; };
+    int ldk, kxp;
+    G geo;
+    struct State { long col, wcol; int kx, ky, kxy2; bool active, valid; };   // kxy2: weighted (mask) form
 
     __host__ __device__ __forceinline__ int rounds() const { return 3 * NV + NS; }
     // grid (ceil(ldk N / TC)): tile = TC consecutive columns of the caller's (ky, kx) plane, whose
@@ -414,10 +443,10 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
         if (s.valid) {
             s.kx = (int)(s.col % ldk);
             const int q = (int)(s.col / ldk);
-            s.ky = wavenumber(q, N);
-            s.kxy2 = s.kx * s.kx + s.ky * s.ky;
-            s.active = 9 * s.kxy2 < N * N;
-            s.wcol = (long)q * (wplane / N) + s.kx;
+            s.ky = wavenumber(q, geo.ny);
+            s.kxy2 = geo.w2(s.kx, s.ky);
+            s.active = geo.keep2(s.kxy2);
+            s.wcol = (long)q * kxp + s.kx;
         }
         return s.active;
     }
@@ -445,8 +474,7 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
         if (!s.valid) return;
         const int g = r / 3, comp = r % 3;
         const int kz = wavenumber(i, N);
-        const int kx = s.kx, ky = s.ky, kxy2 = s.kxy2;
-        const bool keep = s.active && 9 * (kxy2 + kz * kz) < N * N;
+        const bool keep = s.active && geo.keep3(s.kxy2, kz);
         if (NS > 0 && r == 3 * NV) {   // Eq. 2: R_theta = -s^ + N_bv u^_z - kappa |k|^2 theta^
             C *os = sdst + i * plane + s.col;
             if (!keep) { if (!sparse) *os = mk<T>(0, 0); return; }
@@ -456,7 +484,8 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
                 rt.x += nbv * uz.x; rt.y += nbv * uz.y;
             }
             if (sdiff != (T)0) {
-                const T sc = sdiff * (T)(kxy2 + kz * kz);
+                const T qx = (T)s.kx * geo.kfx, qy = (T)s.ky * geo.kfy, qz = (T)kz * geo.kfz;
+                const T sc = sdiff * (qx * qx + qy * qy + qz * qz);
                 const C th = ldg_c(saux + i * plane + s.col);
                 rt.x -= sc * th.x; rt.y -= sc * th.y;
             }
@@ -476,9 +505,8 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
     __device__ __forceinline__ void finish(const State &s, int g, int i, C *o, C fx, C fy, C fz) const
     {
         const int kz = wavenumber(i, N);
-        const int kx = s.kx, ky = s.ky, kxy2 = s.kxy2;
-        const T qx = (T)kx, qy = (T)ky, qz = (T)kz;
-        const T k2 = (T)(kxy2 + kz * kz);
+        const T qx = (T)s.kx * geo.kfx, qy = (T)s.ky * geo.kfy, qz = (T)kz * geo.kfz;
+        const T k2 = qx * qx + qy * qy + qz * qz;
         if (g == 0) {            // a10: projection, identity at k = 0
             if (NS > 0 && nbv != (T)0) {   // Eq. 1: buoyancy -N_bv theta z^, inside the projection
                 const C th = ldg_c(saux + i * plane + s.col);
@@ -524,28 +552,29 @@ template <typename T, int N, int TC, int NV, int NS> struct JobFwdZ : JobElems<J
 // inverse z / y passes of NF fields, and the fwd_z epilogue R_p = beta a^ + alpha |k|^2 q^,
 // R_q = -beta b^ - alpha |k|^2 p^ (a = |psi|^2 q, b = |psi|^2 p from mid_x).
 // ------------------------------------------------------------------------------------------
-template <typename T, int N, int TC, int NF> struct JobPlainInvZ : JobElems<JobPlainInvZ<T, N, TC, NF>, Cx<T>, Ex<T>> {
+template <typename T, int N, int TC, int NF, class G> struct JobPlainInvZ : JobElems<JobPlainInvZ<T, N, TC, NF, G>, Cx<T>, Ex<T>> {
     using C = Cx<T>;
     const C *src;       // NF spectral fields, caller layout
     C *dst;             // NF compact fields
     long plane, nf, wplane, wnf;
+    int ldk, kxp;
+    G geo;
     struct State { long col, wcol; int kxy2; bool active; };
     __host__ __device__ __forceinline__ int rounds() const { return NF; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
-        const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, N);
-        s.kxy2 = kx * kx + ky * ky;
-        s.active = 9 * s.kxy2 < N * N;
-        s.col = (long)blockIdx.y * (plane / N) + kx;
-        s.wcol = (long)blockIdx.y * (wplane / N) + kx;
+        const int kx = (int)colidx, ky = wavenumber((int)blockIdx.y, geo.ny);
+        s.kxy2 = geo.w2(kx, ky);
+        s.active = geo.keep2(s.kxy2);
+        s.col = (long)blockIdx.y * ldk + kx;
+        s.wcol = (long)blockIdx.y * kxp + kx;
         return s.active;
     }
     __device__ __forceinline__ void idle(const State &, int, int) const {}
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
-        const int kz = wavenumber(i, N);
         C x = mk<T>(0, 0);
-        if (s.active && 9 * (s.kxy2 + kz * kz) < N * N) x = ldg_c(src + r * nf + i * plane + s.col);
+        if (s.active && geo.keep3(s.kxy2, wavenumber(i, N))) x = ldg_c(src + r * nf + i * plane + s.col);
         return x;
     }
     __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
@@ -561,26 +590,26 @@ template <typename T, int N, int TC, int NF> struct JobPlainInvZ : JobElems<JobP
 };
 
 // in place on NF compact fields; reads only the retained (ky, kx), writes every ky of the retained kx
-template <typename T, int N, int TC> struct JobPlainInvY : JobElems<JobPlainInvY<T, N, TC>, Cx<T>, Ex<T>> {
+template <typename T, int N, int TC, class G> struct JobPlainInvY : JobElems<JobPlainInvY<T, N, TC, G>, Cx<T>, Ex<T>> {
     using C = Cx<T>;
     C *buf;
     long wplane, wnf;
     int kxp, nfields;
+    G geo;
     struct State { long base; int kx; bool active; };
     __host__ __device__ __forceinline__ int rounds() const { return nfields; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
         s.kx = (int)colidx;
-        s.active = s.kx < kx_count(N);
+        s.active = s.kx < geo.kxc;
         s.base = (long)blockIdx.y * wplane + s.kx;
         return true;
     }
     __device__ __forceinline__ void idle(const State &, int, int) const {}
     __device__ __forceinline__ C load(const State &s, int r, int i) const
     {
-        const int ky = wavenumber(i, N);
         C x = mk<T>(0, 0);
-        if (s.active && 9 * (s.kx * s.kx + ky * ky) < N * N) x = ld_stream(buf + r * wnf + s.base + (long)i * kxp);
+        if (s.active && geo.keep2(geo.w2(s.kx, wavenumber(i, N)))) x = ld_stream(buf + r * wnf + s.base + (long)i * kxp);
         return x;
     }
     __device__ __forceinline__ C post(const State &, int, int, C x) const { return x; }
@@ -590,7 +619,7 @@ template <typename T, int N, int TC> struct JobPlainInvY : JobElems<JobPlainInvY
     }
 };
 
-template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, N, TC>, Cx<T>, Cx<T>> {
+template <typename T, int N, int TC, class G> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, N, TC, G>, Cx<T>, Cx<T>> {
     using C = Cx<T>;
     const C *src;        // 2 compact fields (after fwd_y): a^, b^
     C *dst;              // 2 fields, caller layout: R_p, R_q
@@ -601,8 +630,9 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
     static constexpr bool split_rounds = false;   // the idle path fills both fields
     static constexpr bool is_fwdz = true;
     long plane, nf, wplane, wnf;
-    int ldk;
-    struct State { long col, wcol; int kxy2; bool active, valid; };
+    int ldk, kxp;
+    G geo;
+    struct State { long col, wcol; int kxy2; T kr2; bool active, valid; };   // kr2 = kx^2 + ky^2 (physical)
     __host__ __device__ __forceinline__ int rounds() const { return 2; }
     __device__ __forceinline__ bool begin(State &s, long colidx) const
     {
@@ -610,12 +640,15 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
         s.valid = s.col < plane;
         s.active = false;
         s.kxy2 = 0;
+        s.kr2 = (T)0;
         s.wcol = 0;
         if (s.valid) {
-            const int kx = (int)(s.col % ldk), q = (int)(s.col / ldk), ky = wavenumber(q, N);
-            s.kxy2 = kx * kx + ky * ky;
-            s.active = 9 * s.kxy2 < N * N;
-            s.wcol = (long)q * (wplane / N) + kx;
+            const int kx = (int)(s.col % ldk), q = (int)(s.col / ldk), ky = wavenumber(q, geo.ny);
+            s.kxy2 = geo.w2(kx, ky);
+            const T qx = (T)kx * geo.kfx, qy = (T)ky * geo.kfy;
+            s.kr2 = qx * qx + qy * qy;
+            s.active = geo.keep2(s.kxy2);
+            s.wcol = (long)q * kxp + kx;
         }
         return s.active;
     }
@@ -637,11 +670,12 @@ template <typename T, int N, int TC> struct JobGpeFwdZ : JobElems<JobGpeFwdZ<T, 
         if (!s.valid) return;
         const int kz = wavenumber(i, N);
         C *o = dst + r * nf + i * plane + s.col;
-        if (!(s.active && 9 * (s.kxy2 + kz * kz) < N * N)) { if (!sparse) *o = mk<T>(0, 0); return; }
+        if (!(s.active && geo.keep3(s.kxy2, kz))) { if (!sparse) *o = mk<T>(0, 0); return; }
         // r = 0: R_p = beta a^ + alpha |k|^2 q^;   r = 1: R_q = -beta b^ - alpha |k|^2 p^
         const T sg = r == 0 ? (T)1 : (T)-1;
         const C other = ldg_c(psi + (1 - r) * nf + i * plane + s.col);
-        const T d = sg * alpha * (T)(s.kxy2 + kz * kz), b = sg * beta;
+        const T qz = (T)kz * geo.kfz;
+        const T d = sg * alpha * (s.kr2 + qz * qz), b = sg * beta;
         C res = mk<T>(b * v.x + d * other.x, b * v.y + d * other.y);
         if (base != nullptr) {
             const C y0 = ldg_c(base + r * nf + i * plane + s.col);

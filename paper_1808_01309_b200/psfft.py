@@ -18,10 +18,11 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_query3", "psfft_plan_create3", "psfft_plan_destroy",
-    "psfft_plan_layout",
+    "psfft_plan_layout", "psfft_plan_set_box",
     "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs", "psfft_gpe_rhs",
     "psfft_rk_work_bytes", "psfft_rk_step",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
+    "psfft_slab_query", "psfft_slab_r2c_xy", "psfft_slab_z", "psfft_slab_c2r_yx",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
     "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
     "psfft_kernel_name", "psfft_last_launch_count", "psfft_strerror", "psfft_version",
@@ -43,6 +44,18 @@ class Layout(ctypes.Structure):
                 ("work_bytes_gpe", ctypes.c_size_t)]
 
 
+MAX_RANKS = 16
+
+
+class SlabLayout(ctypes.Structure):
+    """Mirror of ``psfft_slab_layout``."""
+    _fields_ = [("P", ctypes.c_int), ("rank", ctypes.c_int), ("Mz", ctypes.c_int), ("z0", ctypes.c_int),
+                ("w", ctypes.c_int), ("x0", ctypes.c_int * (MAX_RANKS + 1)),
+                ("real_elems", ctypes.c_size_t), ("real_bytes", ctypes.c_size_t),
+                ("zspec_elems", ctypes.c_size_t), ("zspec_bytes", ctypes.c_size_t),
+                ("xslab_elems", ctypes.c_size_t), ("xslab_bytes", ctypes.c_size_t)]
+
+
 _lib = None
 
 
@@ -61,6 +74,7 @@ def lib() -> ctypes.CDLL:
         L.psfft_plan_create3.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, vp, sz, vp]
         L.psfft_plan_destroy.argtypes = [vp]
         L.psfft_plan_layout.argtypes = [vp, ctypes.POINTER(Layout)]
+        L.psfft_plan_set_box.argtypes = [vp, cd, cd, cd]
         L.psfft_fft3d_r2c.argtypes = [vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r.argtypes = [vp, vp, vp, vp, vp]
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
@@ -72,6 +86,11 @@ def lib() -> ctypes.CDLL:
         L.psfft_rk_step.argtypes = [vp, ci, vp, vp, ci, cd, ctypes.POINTER(cd), vp, vp]
         L.psfft_hd_rhs_unfused.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs_unfused.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
+        cl = ctypes.c_long
+        L.psfft_slab_query.argtypes = [vp, ci, ci, ctypes.POINTER(SlabLayout)]
+        L.psfft_slab_r2c_xy.argtypes = [vp, ci, ci, vp, vp, ctypes.POINTER(vp), cl, vp]
+        L.psfft_slab_z.argtypes = [vp, ci, ci, ci, vp, vp]
+        L.psfft_slab_c2r_yx.argtypes = [vp, ci, ci, ctypes.POINTER(vp), cl, vp, vp, vp]
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_hd_rhs_host.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
@@ -145,6 +164,10 @@ def plan_create3(Nx: int, Ny: int, Nz: int, dtype: int, batch: int, d_tables, ta
     return h.value
 
 
+def plan_set_box(plan: int, Lx: float, Ly: float, Lz: float) -> None:
+    _check(lib().psfft_plan_set_box(plan, float(Lx), float(Ly), float(Lz)), "psfft_plan_set_box")
+
+
 def plan_destroy(plan: int) -> None:
     _check(lib().psfft_plan_destroy(plan), "psfft_plan_destroy")
 
@@ -200,6 +223,31 @@ def hd_rhs_unfused(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> 
 def mhd_rhs_unfused(plan: int, d_uhat, d_bhat, d_rhs_u, d_rhs_b, nu: float, eta: float, d_work, stream=None) -> None:
     _check(lib().psfft_mhd_rhs_unfused(plan, _ptr(d_uhat), _ptr(d_bhat), _ptr(d_rhs_u), _ptr(d_rhs_b), float(nu),
                                        float(eta), _ptr(d_work), _stream(stream)), "psfft_mhd_rhs_unfused")
+
+
+def slab_query(plan: int, P: int, rank: int) -> SlabLayout:
+    sl = SlabLayout()
+    _check(lib().psfft_slab_query(plan, P, rank, ctypes.byref(sl)), "psfft_slab_query")
+    return sl
+
+
+def _ptr_array(blocks):
+    return (ctypes.c_void_p * len(blocks))(*[_ptr(b) for b in blocks])
+
+
+def slab_r2c_xy(plan: int, P: int, rank: int, d_real_slab, d_zspec, d_blocks, zoff: int, stream=None) -> None:
+    """d_blocks: P tensors / device pointers, the block of each rank (see psfft.h)."""
+    _check(lib().psfft_slab_r2c_xy(plan, P, rank, _ptr(d_real_slab), _ptr(d_zspec), _ptr_array(d_blocks), int(zoff),
+                                   _stream(stream)), "psfft_slab_r2c_xy")
+
+
+def slab_z(plan: int, P: int, rank: int, direction: int, d_xslab, stream=None) -> None:
+    _check(lib().psfft_slab_z(plan, P, rank, int(direction), _ptr(d_xslab), _stream(stream)), "psfft_slab_z")
+
+
+def slab_c2r_yx(plan: int, P: int, rank: int, d_blocks, zoff: int, d_zspec, d_real_slab, stream=None) -> None:
+    _check(lib().psfft_slab_c2r_yx(plan, P, rank, _ptr_array(d_blocks), int(zoff), _ptr(d_zspec), _ptr(d_real_slab),
+                                   _stream(stream)), "psfft_slab_c2r_yx")
 
 
 def fft3d_r2c_host(plan: int, h_real, h_spec, d_in, d_out, d_work=None, stream=None) -> None:
@@ -270,7 +318,7 @@ class Plan:
     >>> rhs = p.hd_rhs(uhat)        # uhat: [3, N, N, N/2+1] complex
     """
 
-    def __init__(self, N: int, dtype=torch.float64, batch: int = 1, device="cuda:0", work: str = "fft"):
+    def __init__(self, N, dtype=torch.float64, batch: int = 1, device="cuda:0", work: str = "fft", box=None):
         if not torch.cuda.is_available():
             raise PsfftError("no CUDA device: libpsfft has no CPU fallback")
         self.device = torch.device(device)
@@ -279,13 +327,15 @@ class Plan:
         self.rdtype = dtype
         self.cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
         code = F64 if dtype == torch.float64 else F32
-        # N: one size (cubic grid) or (Nx, Ny, Nz) for an anisotropic grid (transforms only)
+        # N: one size (cubic grid) or (Nx, Ny, Nz) for an anisotropic grid; box = (Lx, Ly, Lz), default 2 pi each
         Nx, Ny, Nz = (N, N, N) if isinstance(N, int) else tuple(N)
         self.layout = plan_query3(Nx, Ny, Nz, code, batch)
         self.N, self.Ny, self.Nz, self.batch, self.ldk = Nx, Ny, Nz, batch, self.layout.ldk
         with torch.cuda.device(self.device):
             self.tables = torch.empty(self.layout.table_bytes, dtype=torch.uint8, device=self.device)
             self.handle = plan_create3(Nx, Ny, Nz, code, batch, self.tables, self.layout.table_bytes)
+        if box is not None:
+            plan_set_box(self.handle, *box)
         self._work = None
         self._work_kind = None
         self.ensure_work(work)

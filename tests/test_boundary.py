@@ -97,11 +97,15 @@ def test_product_never_imports_the_oracle():
 
 
 def test_plan_query3_anisotropic_sizes(lib):
-    """Anisotropic plans (PAPER.md:370 runs 1024 x 1024 x 256): sizes per axis, no RHS workspace."""
+    """Anisotropic plans (PAPER.md:370 runs 1024 x 1024 x 256): sizes per axis; RHS workspace = 11 (HD) / 16
+    (Boussinesq) compact fields [Nz][Ny][kx pitch] whose pitch is the retained kx count of Nx rounded up to a tile."""
     lay = psfft.plan_query3(1024, 1024, 256, psfft.F32, 1)
     assert (lay.N, lay.Ny, lay.Nz, lay.ldk) == (1024, 1024, 256, 513)
     assert lay.real_elems == 1024 * 1024 * 256 and lay.spec_elems == 513 * 1024 * 256
-    assert lay.work_bytes_fft == lay.spec_bytes and lay.work_bytes_hd == 0 and lay.work_bytes_boussinesq == 0
+    assert lay.work_bytes_fft == lay.spec_bytes
+    pitch = lay.work_bytes_hd // (11 * 256 * 1024 * 8)
+    assert lay.work_bytes_hd == 11 * 256 * 1024 * pitch * 8 and 342 <= pitch <= 342 + 32 and pitch % 16 == 0
+    assert lay.work_bytes_boussinesq * 11 == lay.work_bytes_hd * 16 and lay.work_bytes_mhd == 2 * lay.work_bytes_hd
     cub = psfft.plan_query3(512, 512, 512, psfft.F64, 3)
     ref = psfft.plan_query(512, psfft.F64, 3)
     assert (cub.table_bytes, cub.work_bytes_hd, cub.Ny, cub.Nz) == (ref.table_bytes, ref.work_bytes_hd, 512, 512)

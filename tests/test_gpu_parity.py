@@ -114,12 +114,13 @@ def test_anisotropic_r2c_c2r_match_oracle(shape, dtype):
     assert rel(y, oracle.c2r3d(Y.astype(np.complex128), Nx)) < TOL[dtype]
 
 
-def test_anisotropic_plan_rejects_the_right_hand_sides():
-    p = psfft.Plan((32, 32, 16), torch.float64, 1)
-    assert p.layout.work_bytes_hd == 0 and psfft.rk_work_bytes(p.handle, psfft.SYS_HD) == 0
+def test_unfused_cross_check_path_needs_a_cubic_plan():
+    """Only the *_unfused variants are cubic-only; the fused right-hand sides take any plan (tests/test_gpu_aniso.py)."""
+    p = psfft.Plan((32, 32, 16), torch.float64, 1, work="hd")
+    assert p.layout.work_bytes_hd > 0 and psfft.rk_work_bytes(p.handle, psfft.SYS_HD) > 0
     u = torch.zeros((3, 16, 32, 17), dtype=torch.complex128, device="cuda")
     with pytest.raises(psfft.PsfftError):
-        psfft.hd_rhs(p.handle, u, torch.empty_like(u), 0.0, torch.empty_like(u))
+        psfft.hd_rhs_unfused(p.handle, u, torch.empty_like(u), 0.0, p.ensure_work("hd"))
 
 
 def test_degenerate_inputs():

@@ -1,0 +1,73 @@
+"""Slab-decomposed transform on ONE GPU: P virtual ranks in direct
+mode -- each rank's y-pass stores straight into the x-slabs of all ranks -- must reproduce the single-GPU transform
+BIT FOR BIT (same kernels, same butterfly order per column), and the oracle within tolerance.  -m gpu."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from paper_1808_01309_b200 import psfft, slab, synth  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float64: 1e-12, torch.float32: 2e-5}
+RDT = {torch.float64: np.float64, torch.float32: np.float32}
+
+
+def field(shape, dtype, seed=31):
+    Nx, Ny, Nz = shape
+    x = synth.uniform01(seed, np.arange(Nz * Ny * Nx, dtype=np.uint64)).reshape(Nz, Ny, Nx) * 2 - 1
+    return x.astype(RDT[dtype])
+
+
+def rel(a, b):
+    a = np.asarray(a).astype(np.complex128)
+    b = np.asarray(b).astype(np.complex128)
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("shape,P", [((32, 32, 32), 2), ((32, 32, 32), 8), ((64, 48, 16), 4), ((128, 128, 128), 8),
+                                     ((24, 16, 48), 3), ((64, 8, 16), 16), ((256, 64, 32), 2), ((32, 32, 32), 1)])
+def test_virtual_ranks_equal_the_single_gpu_transform_bit_for_bit(shape, P, dtype):
+    Nx, Ny, Nz = shape
+    x = field(shape, dtype)
+    plan = psfft.Plan(shape, dtype, 1)
+    xd = torch.from_numpy(x).cuda()
+    single = plan.r2c(xd[None])[0]
+    vs = slab.VirtualSlabs(plan, P)
+    got = vs.r2c(xd)
+    assert torch.equal(got, single)                              # bit for bit
+    assert rel(got.cpu().numpy(), oracle.r2c3d(x.astype(np.float64))) < TOL[dtype]
+    # the kx ranges partition [0, ldk) as evenly as possible
+    x0 = list(vs.lays[0].x0[:P + 1])
+    assert x0[0] == 0 and x0[-1] == Nx // 2 + 1 and max(np.diff(x0)) - min(np.diff(x0)) <= 1
+    # inverse through the virtual ranks: bit for bit the single-GPU c2r, and the round trip
+    back = vs.c2r(single)
+    assert torch.equal(back, plan.c2r(single[None])[0])
+    assert rel(back.cpu().numpy(), x) < TOL[dtype]
+
+
+def test_packed_mode_blocks_and_argument_checks():
+    """Packed mode on one rank-0-of-2 call: the send buffer holds the slices [q][Mz][Ny][w_q] of the y-transformed
+    slab; bad (P, rank) are refused."""
+    shape, P = (32, 16, 8), 2
+    Nx, Ny, Nz = shape
+    plan = psfft.Plan(shape, torch.float64, 1)
+    lay = psfft.slab_query(plan.handle, P, 0)
+    assert (lay.Mz, lay.z0, lay.w) == (4, 0, 8) and list(lay.x0[:3]) == [0, 8, 17]
+    x = field(shape, torch.float64)
+    xd = torch.from_numpy(x).cuda()
+    send = torch.zeros(lay.zspec_elems, dtype=torch.complex128, device="cuda")
+    zs = torch.empty_like(send)
+    counts, _ = slab.forward_splits(Nz, Ny, Nx // 2 + 1, P, 0)
+    psfft.slab_r2c_xy(plan.handle, P, 0, xd[:4], zs, slab._slice_ptrs(send, counts), 0)
+    want = np.fft.fft(np.fft.rfft(x[:4].astype(np.float64), axis=2), axis=1)       # x then y of the slab (check only)
+    s = send.cpu().numpy()
+    b0 = s[:counts[0]].reshape(4, Ny, 8)
+    b1 = s[counts[0]:].reshape(4, Ny, 9)
+    assert rel(b0, want[:, :, :8]) < 1e-13 and rel(b1, want[:, :, 8:]) < 1e-13
+    for bad in [(3, 0), (2, 2), (0, 0), (17, 0)]:
+        with pytest.raises(psfft.PsfftError):
+            psfft.slab_query(plan.handle, *bad)
