@@ -329,6 +329,61 @@ def device_spectrum(torch, synth, N, k0, kcut, seed, tag, cdtype, dev):
     return u
 
 
+WORKLOADS = {   # --workload: one right-hand side alone (the command lines of the ncu captures under profiles/)
+    "hd512": (512, "float64", "hd", 4.0, 32, 42, "512^3 fp64 HD RHS (the metric's workload)"),
+    "hd512f32": (512, "float32", "hd", 4.0, 32, 42, "512^3 fp32 HD RHS"),
+    "hd768f32": (768, "float32", "hd", 4.0, 32, 42, "768^3 fp32 HD RHS (BASELINE.json configs[3])"),
+    "mhd1024f32": (1024, "float32", "mhd", 3.0, 24, 84, "1024^3 fp32 MHD RHS (BASELINE.json configs[4])"),
+}
+
+
+def rhs_workload(torch, psfft, synth, dev, stream, peak, K, N, rdtype, system, k0, kcut, workload, dense_units, note) -> dict:
+    """One right-hand-side workload: plan outside the timed region, 3 warm-up calls, K (<= 10) timed calls between CUDA
+    events on device-resident input, then the same calls again with the per-launch events on for the bytes moved."""
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    cdt = torch.complex128 if rdtype == torch.float64 else torch.complex64
+    code = psfft.F64 if rdtype == torch.float64 else psfft.F32
+    lay = psfft.plan_query(N, code, 1)
+    nvec = 2 if system == "mhd" else 1
+    need = (lay.work_bytes_mhd if system == "mhd" else lay.work_bytes_hd) + 6 * nvec * lay.spec_bytes
+    free = torch.cuda.mem_get_info(dev)[0]
+    if free < need + (1 << 30):
+        return {"workload": workload, "skipped": f"needs {need / 2**30:.0f} GiB, {free / 2**30:.0f} GiB free"}
+    p = psfft.Plan(N, rdtype, 1, device=dev, work=system)
+    u = device_spectrum(torch, synth, N, k0, kcut, 1234, 0, cdt, dev)
+    ru = torch.empty_like(u)
+    wk = p.ensure_work(system)
+    if system == "mhd":
+        b = device_spectrum(torch, synth, N, k0, kcut, 1234, 1, cdt, dev)
+        rb = torch.empty_like(b)
+        fn = lambda: psfft.mhd_rhs(p.handle, u, b, ru, rb, 0.0, 0.0, wk)
+    else:
+        fn = lambda: psfft.hd_rhs(p.handle, u, ru, 0.0, wk)
+    n = max(3, min(K, 10))
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    ms = time_loop(fn, n, stream)
+    psfft.profile_reset(p.handle)
+    psfft.profile_enable(p.handle, True)
+    time_loop(fn, n, stream)
+    torch.cuda.synchronize()
+    psfft.profile_enable(p.handle, False)
+    dt = "fp64" if rdtype == torch.float64 else "fp32"
+    rl = roofline_of(psfft.profile_records(p.handle), n, ms, dense_units * lay.spec_bytes,
+                     f"fused 3-pass dense count = {dense_units} C (SURVEY.md §8(a))", peak, f"{N}^3 {dt}")
+    out = {"workload": workload, "ms": ms, "evals_per_s": 1e3 / ms, "steps": n,
+           "frac_bytes_moved": rl["step_bytes_moved"]["frac"],
+           "dense_model_equivalent_frac": rl["step_dense_model"]["equivalent_frac"],
+           "dominant_kernel": rl["kernel"], "dominant_kernel_frac": rl["frac"],
+           "dominant_kernel_traffic": rl["traffic"], "traffic_source": rl["traffic_source"],
+           "per_kernel": rl["per_kernel"], "launches_per_eval": psfft.last_launch_count(p.handle), "note": note}
+    p.close()
+    return out
+
+
 def other_configs(torch, psfft, synth, dev, stream, peak, K: int) -> dict:
     """BASELINE.json configs 1, 2, 4, 5 (the metric's config 3 / 3b is the headline), same protocol: plan outside
     the timed region, 3 warm-up calls, K timed calls between CUDA events, device-resident inputs; then K more
@@ -360,43 +415,8 @@ def other_configs(torch, psfft, synth, dev, stream, peak, K: int) -> dict:
     del p, x, X, y, w
 
     def rhs_config(key, N, rdtype, system, k0, kcut, workload, dense_units, note):
-        gc.collect()
-        torch.cuda.empty_cache()
-        cdt = torch.complex128 if rdtype == torch.float64 else torch.complex64
-        code = psfft.F64 if rdtype == torch.float64 else psfft.F32
-        lay = psfft.plan_query(N, code, 1)
-        nvec = 2 if system == "mhd" else 1
-        need = (lay.work_bytes_mhd if system == "mhd" else lay.work_bytes_hd) + 6 * nvec * lay.spec_bytes
-        free = torch.cuda.mem_get_info(dev)[0]
-        if free < need + (1 << 30):
-            out[key] = {"workload": workload, "skipped": f"needs {need / 2**30:.0f} GiB, {free / 2**30:.0f} GiB free"}
-            return
-        p = psfft.Plan(N, rdtype, 1, device=dev, work=system)
-        u = device_spectrum(torch, synth, N, k0, kcut, 1234, 0, cdt, dev)
-        ru = torch.empty_like(u)
-        wk = p.ensure_work(system)
-        if system == "mhd":
-            b = device_spectrum(torch, synth, N, k0, kcut, 1234, 1, cdt, dev)
-            rb = torch.empty_like(b)
-            fn = lambda: psfft.mhd_rhs(p.handle, u, b, ru, rb, 0.0, 0.0, wk)
-        else:
-            fn = lambda: psfft.hd_rhs(p.handle, u, ru, 0.0, wk)
-        n = max(3, min(K, 10))
-        ms = timed(fn, n)
-        psfft.profile_reset(p.handle)
-        psfft.profile_enable(p.handle, True)
-        time_loop(fn, n, stream)
-        torch.cuda.synchronize()
-        psfft.profile_enable(p.handle, False)
-        dt = "fp64" if rdtype == torch.float64 else "fp32"
-        rl = roofline_of(psfft.profile_records(p.handle), n, ms, dense_units * lay.spec_bytes,
-                         f"fused 3-pass dense count = {dense_units} C (SURVEY.md §8(a))", peak, f"{N}^3 {dt}")
-        out[key] = {"workload": workload, "ms": ms, "evals_per_s": 1e3 / ms, "steps": n,
-                    "frac_bytes_moved": rl["step_bytes_moved"]["frac"],
-                    "dense_model_equivalent_frac": rl["step_dense_model"]["equivalent_frac"],
-                    "dominant_kernel": rl["kernel"], "dominant_kernel_frac": rl["frac"],
-                    "per_kernel": rl["per_kernel"], "launches_per_eval": psfft.last_launch_count(p.handle), "note": note}
-        p.close()
+        out[key] = rhs_workload(torch, psfft, synth, dev, stream, peak, K, N, rdtype, system, k0, kcut, workload,
+                                dense_units, note)
 
     rhs_config("configs[1]", 128, torch.float64, "hd", 4.0, 32,
                "128^3 fp64 HD RHS, E(k) ~ k^4 exp(-2(k/4)^2), unit energy, seed 1234", 42,
@@ -408,7 +428,72 @@ def other_configs(torch, psfft, synth, dev, stream, peak, K: int) -> dict:
                "155 GB resident; inputs far larger than L2")
     gc.collect()
     torch.cuda.empty_cache()
+    out["flat_box"] = flat_box_rows(torch, psfft, synth, dev, stream, peak, K, timed)
+    gc.collect()
+    torch.cuda.empty_cache()
+    out["slab"] = slab_rows(torch, psfft, dev, stream, K, timed)
+    gc.collect()
+    torch.cuda.empty_cache()
     return out
+
+
+def flat_box_rows(torch, psfft, synth, dev, stream, peak, K, timed) -> dict:
+    """SURVEY.md §8(f) NEXT-2 at the paper's flat-box size: Boussinesq right-hand side and one RK2
+    step on 1024 x 1024 x 256 in the box (2 pi, 2 pi, 2 pi / 4), fp64, device-resident broadband input."""
+    import math
+    shape, box = (1024, 1024, 256), (2 * math.pi, 2 * math.pi, 2 * math.pi / 4)
+    p = psfft.Plan(shape, torch.float64, 1, device=dev, work="rk_boussinesq", box=box)
+    y = torch.empty(p.spec_shape(4), dtype=torch.complex128, device=dev)
+    y[:3].copy_(torch.from_numpy(synth.aniso_spectrum(shape, box, seed=1234, fill=0.2)))
+    y[3].copy_(torch.from_numpy(synth.aniso_spectrum(shape, box, seed=1234, tag=7, ncomp=1, fill=0.2)))
+    out = torch.empty_like(y)
+    wk = p.ensure_work("rk_boussinesq")
+    n = max(3, min(K, 10))
+    f_rhs = lambda: psfft.boussinesq_rhs(p.handle, y[:3], y[3], out[:3], out[3], 1e-3, 1e-3, 2.0, wk)
+    f_rk = lambda: psfft.rk_step(p.handle, psfft.SYS_BOUSSINESQ, y, out, 2, 1e-3, (1e-3, 1e-3, 2.0), wk)
+    t_rhs = timed(f_rhs, n)
+    psfft.profile_reset(p.handle)
+    psfft.profile_enable(p.handle, True)
+    time_loop(f_rhs, n, stream)
+    torch.cuda.synchronize()
+    psfft.profile_enable(p.handle, False)
+    rl = roofline_of(psfft.profile_records(p.handle), n, t_rhs, 56.0 * p.layout.spec_bytes,
+                     "fused 3-pass dense count = 56 C (9 + 4 transforms + 4 C epilogue reads)", peak, "1024x1024x256 fp64")
+    t_rk = timed(f_rk, n)
+    res = {"workload": "1024 x 1024 x 256 fp64 Boussinesq in the box (2 pi, 2 pi, 2 pi/4), broadband solenoidal u + theta "
+                       "(synth.aniso_spectrum, fill 0.2), nu = kappa = 1e-3, N_bv = 2",
+           "boussinesq_rhs": {"ms": t_rhs, "evals_per_s": 1e3 / t_rhs, "frac_bytes_moved": rl["step_bytes_moved"]["frac"],
+                              "per_kernel": rl["per_kernel"]},
+           "boussinesq_rk2_step": {"ms": t_rk, "steps_per_s": 1e3 / t_rk}, "steps": n}
+    p.close()
+    return res
+
+
+def slab_rows(torch, psfft, dev, stream, K, timed) -> dict:
+    """what ONE rank of a P = 8 slab decomposition of the 512^3 fp64 transform does
+    locally (phase 1: x-pass + y-pass with the all-to-all fused into its stores, packed mode; phase 2: z-pass of its
+    x-slab).  The exchange itself needs P GPUs: unmeasured on this box."""
+    from paper_1808_01309_b200 import slab
+    N, P = 512, 8
+    p = psfft.Plan(N, torch.float64, 1, device=dev)
+    lay = psfft.slab_query(p.handle, P, 0)
+    real = torch.rand((lay.Mz, N, N), dtype=torch.float64, device=dev) * 2 - 1
+    zs = torch.empty(lay.zspec_elems, dtype=torch.complex128, device=dev)
+    send = torch.empty(lay.zspec_elems, dtype=torch.complex128, device=dev)
+    xs = torch.empty(lay.xslab_elems, dtype=torch.complex128, device=dev)
+    counts, _ = slab.forward_splits(N, N, p.ldk, P, 0)
+    blocks = slab._slice_ptrs(send, counts)
+    n = max(3, min(K, 20))
+    t1 = timed(lambda: psfft.slab_r2c_xy(p.handle, P, 0, real, zs, blocks, 0), n)
+    t2 = timed(lambda: psfft.slab_z(p.handle, P, 0, -1, xs), n)
+    res = {"workload": f"rank 0 of P = {P}, {N}^3 fp64, one field: z-slab of {lay.Mz} planes, x-slab of {lay.w} kx columns",
+           "ms_phase1_xy_scatter": t1, "ms_phase2_z": t2,
+           "bytes_sent_per_rank": (P - 1) * lay.zspec_bytes // P,
+           "exchange": "unmeasured on hardware (one GPU per box); at the guide's 770 GB/s per direction the "
+                       f"{(P - 1) * lay.zspec_bytes // P / 1e6:.0f} MB take {(P - 1) * lay.zspec_bytes / P / 770e9 * 1e3:.3f} ms",
+           "single_gpu_equivalent": "8 virtual ranks reproduce psfft_fft3d_r2c bit for bit (tests/test_gpu_slab.py)"}
+    p.close()
+    return res
 
 
 def run_ours(args) -> int:
@@ -427,6 +512,12 @@ def run_ours(args) -> int:
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream()
     peak, peak_src = hbm_peak()
+    if args.workload != "metric":   # one right-hand side alone: the command line of an ncu capture under profiles/
+        Nw, dtw, system, k0, kcut, dense, what = WORKLOADS[args.workload]
+        res = rhs_workload(torch, psfft, synth, dev, stream, peak, K, Nw, getattr(torch, dtw), system, k0, kcut, what,
+                           dense, "single-workload run (--workload)")
+        print(json.dumps({"workload_run": args.workload, **res}), flush=True)
+        return 0
     m = metric_parts(torch, psfft, synth, N, K, W, rank, local, world, dev, stream, peak, peak_src)   # its buffers die here
 
     # ---- the other BASELINE.json configs, after the metric (they need the memory the 512^3 buffers held) ----
@@ -579,6 +670,8 @@ def main() -> int:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--N", type=int, default=512, help="grid size (the metric is quoted at 512)")
+    ap.add_argument("--workload", default="metric", choices=["metric"] + sorted(WORKLOADS),
+                    help="metric: the full bench line (default); otherwise time ONE right-hand-side workload alone")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE.json configs (768^3, 1024^3 ...)")
     ap.add_argument("--reference-budget-s", type=float, default=150.0,

@@ -92,3 +92,33 @@ def assert_shells_device(got, want, N, tol, min_shells=8):
     bad = {int(s): float(e) for s, e in zip(shells, err) if not e < tol}
     assert not bad, f"per-shell relative error above {tol}: {bad}"
     return float(err.max())
+
+
+def ellipsoid_shell_index(shape, nshell=8):
+    """Shell number floor(nshell * 3 * sqrt(sum (n_i / N_i)^2)) of every half-spectrum mode of an (Nx, Ny, Nz) grid:
+    shells 0 .. nshell-1 tile the 2/3-rule ellipsoid sum (n_i / N_i)^2 < 1/9 (reading G25)."""
+    Nx, Ny, Nz = shape
+    fy = np.fft.fftfreq(Ny)          # n / N
+    fz = np.fft.fftfreq(Nz)
+    fx = np.arange(Nx // 2 + 1) / Nx
+    rho = np.sqrt(fz[:, None, None] ** 2 + fy[None, :, None] ** 2 + fx[None, None, :] ** 2)
+    return (rho * (3 * nshell)).astype(np.int32)
+
+
+def assert_ellipsoid_shells(got, want, shape, tol, nshell=8):
+    """Per-shell relative L2 error on an anisotropic grid: every populated shell within tol and the reference reaches
+    the outermost retained shell."""
+    sh = ellipsoid_shell_index(shape, nshell)
+    nb = int(sh.max()) + 1
+    num = np.zeros(nb)
+    den = np.zeros(nb)
+    for g, w in zip(got, want):
+        w = w.astype(np.complex128)
+        num += np.bincount(sh.ravel(), weights=(np.abs(g.astype(np.complex128) - w) ** 2).ravel(), minlength=nb)
+        den += np.bincount(sh.ravel(), weights=(np.abs(w) ** 2).ravel(), minlength=nb)
+    live = den > 0
+    shells, err = np.nonzero(live)[0], np.sqrt(num[live] / den[live])
+    assert len(shells) >= nshell and shells.max() >= nshell - 1, f"reference populates shells {shells}"
+    bad = {int(s): float(e) for s, e in zip(shells, err) if not e < tol}
+    assert not bad, f"per-shell relative error above {tol}: {bad}"
+    return float(err.max())

@@ -15,6 +15,9 @@
   against unfused after the unfused path's transforms have been oracle-checked at that size; (b) the Taylor-Green
   closed form at a wavenumber m whose output lands in the LAST retained shell (9 * 8 m^2 < N^2); (c) the plain
   transforms against the oracle at 768^3, 1024^3 and on the paper's 1024 x 1024 x 256 box.
+* The paper's flat box, 1024 x 1024 x 256 in (2 pi, 2 pi, 2 pi / 4) (last part of this file): HD fp64
+  and the Boussinesq system fp32 on a broadband field filling the whole ellipsoid, element by element against the
+  full-size oracle with per-shell bounds; Boussinesq RK2 against the 256 x 256 x 64 oracle (P12).
 """
 import numpy as np
 import pytest
@@ -23,7 +26,7 @@ torch = pytest.importorskip("torch")
 
 import oracle  # noqa: E402
 from paper_1808_01309_b200 import psfft, synth  # noqa: E402
-from parity_util import assert_shells, assert_shells_device  # noqa: E402
+from parity_util import assert_ellipsoid_shells, assert_shells, assert_shells_device  # noqa: E402
 
 pytestmark = pytest.mark.gpu
 
@@ -412,3 +415,79 @@ def test_hd_and_mhd_rhs_1024_fp32_full_sphere():
     s = np.sqrt(dot(ud, ud) * dot(ru, ru)) + np.sqrt(dot(bd, bd) * dot(rb, rb))
     assert abs(dot(ud, ru) + dot(bd, rb)) / s < 1e-5
     assert abs(dot(bd, ru) + dot(ud, rb)) / s < 1e-5
+
+
+# ---- the paper's flat box: 1024 x 1024 x 256 (PAPER.md:344 Fig. 5, :370 Fig. 7) -----------------
+
+FLAT = (1024, 1024, 256)
+FLATBOX = (2 * np.pi, 2 * np.pi, 2 * np.pi / 4)     # isotropic resolution: dx = dy = dz
+
+
+def test_hd_rhs_1024x1024x256_fp64_full_ellipsoid():
+    """Every retained mode of the ellipsoid carries data (and so do the modes the input mask has to remove); the
+    oracle runs at full size on the host (about 45 GB)."""
+    uh = synth.aniso_spectrum(FLAT, FLATBOX, seed=1234)
+    p = psfft.Plan(FLAT, torch.float64, 1, work="hd", box=FLATBOX)
+    got = p.hd_rhs(torch.from_numpy(uh).cuda(), 1e-3).cpu().numpy()
+    p.close()
+    del p
+    torch.cuda.empty_cache()
+    want = oracle.hd_rhs(uh, 1e-3, box=FLATBOX)
+    assert rel(got, want) < 1e-12
+    assert_ellipsoid_shells(got, want, FLAT, 1e-12)
+    M = oracle.dealias_mask(*FLAT)
+    assert np.all(got[:, ~M] == 0)
+
+
+def test_boussinesq_rhs_1024x1024x256_fp32_full_ellipsoid():
+    """The paper's reference equations on its flat-box geometry (Boussinesq, 1024 x 1024 x 256), fp32,
+    all terms on, against the full-size fp64 oracle."""
+    uh = synth.aniso_spectrum(FLAT, FLATBOX, seed=1234, dtype=np.complex64)
+    th = synth.aniso_spectrum(FLAT, FLATBOX, seed=1234, tag=7, ncomp=1, dtype=np.complex64)
+    p = psfft.Plan(FLAT, torch.float32, 1, work="boussinesq", box=FLATBOX)
+    ru, rt = p.boussinesq_rhs(torch.from_numpy(uh).cuda(), torch.from_numpy(th).cuda(), 1e-3, 2e-3, 2.0)
+    ru, rt = ru.cpu().numpy(), rt.cpu().numpy()
+    p.close()
+    del p
+    torch.cuda.empty_cache()
+    wu, wt = oracle.boussinesq_rhs(uh.astype(np.complex128), th.astype(np.complex128), 1e-3, 2e-3, 2.0, box=FLATBOX)
+    assert rel(ru, wu) < 2e-5 and rel(rt, wt) < 2e-5
+    assert_ellipsoid_shells(ru, wu, FLAT, 2e-5)
+    assert_ellipsoid_shells(rt[None], wt[None], FLAT, 2e-5)
+    M = oracle.dealias_mask(*FLAT)
+    assert np.all(ru[:, ~M] == 0) and np.all(rt[~M] == 0)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_boussinesq_rk2_1024x1024x256_against_the_256x256x64_oracle(dtype):
+    """P12 on the flat box: the same band-limited coefficients (keyed on the index vector, fill 0.16 of the small grid
+    so that both RK2 stages stay inside its mask) on 256 x 256 x 64 give the same step on every mode the small grid retains; beyond
+    the reach of two quadratic stages the big grid's result must be roundoff."""
+    small = (256, 256, 64)
+    cdt = np.complex128 if dtype == torch.float64 else np.complex64
+    tol = 1e-12 if dtype == torch.float64 else 2e-5
+    f = 0.16
+    ys = np.concatenate([synth.aniso_spectrum(small, FLATBOX, seed=77, fill=f),
+                         synth.aniso_spectrum(small, FLATBOX, seed=77, tag=7, ncomp=1, fill=f)[None]])
+    yb = np.concatenate([synth.aniso_spectrum(FLAT, FLATBOX, seed=77, fill=f / 4, dtype=cdt),
+                         synth.aniso_spectrum(FLAT, FLATBOX, seed=77, tag=7, ncomp=1, fill=f / 4, dtype=cdt)[None]])
+    dt, nu, kappa, nbv = 5e-3, 1e-3, 2e-3, 2.0
+    p = psfft.Plan(FLAT, dtype, 1, work="fft", box=FLATBOX)
+    got = p.rk_step(psfft.SYS_BOUSSINESQ, torch.from_numpy(np.ascontiguousarray(yb)).cuda(), 2, dt, nu, kappa, nbv).cpu().numpy()
+    want = oracle.rk_step(2, ys, 2, dt, nu, kappa, nbv, box=FLATBOX)
+    nbig, nsmall = float(np.prod(FLAT)), float(np.prod(small))
+    # index box of the small grid inside the big one
+    iz = np.r_[0:32, FLAT[2] - 32:FLAT[2]]
+    iy = np.r_[0:128, FLAT[1] - 128:FLAT[1]]
+    jz = np.r_[0:32, small[2] - 32:small[2]]
+    jy = np.r_[0:128, small[1] - 128:small[1]]
+    big = got[:, iz][:, :, iy][:, :, :, :128].astype(np.complex128) / nbig
+    sm = want[:, jz][:, :, jy][:, :, :, :128] / nsmall
+    Ms = oracle.dealias_mask(*small)[jz][:, jy][:, :, :128]          # compare where the SMALL grid retains the mode
+    assert Ms.sum() > 1e5 and np.all(sm[:, ~Ms] == 0)
+    assert np.linalg.norm((big - sm)[:, Ms].ravel()) / np.linalg.norm(sm.ravel()) < tol
+    # two quadratic stages of a field band-limited to 0.16 reach 0.64 of the small grid's indices: beyond that the big
+    # grid's result must be roundoff
+    fz, fy, fx = np.fft.fftfreq(FLAT[2]) * 4, np.fft.fftfreq(FLAT[1]) * 4, np.arange(FLAT[0] // 2 + 1) / FLAT[0] * 4
+    far = (fz[:, None, None] ** 2 + fy[None, :, None] ** 2 + fx[None, None, :] ** 2) > 0.66**2
+    assert np.linalg.norm(got[:, far].astype(np.complex128).ravel()) / nbig / np.linalg.norm(sm.ravel()) < tol
