@@ -80,6 +80,11 @@ template <int N> struct XSched {
 // Shared-memory slot of element i of one transform buffer: i + X (i >> A) + Y (i >> B) + Z (i >> C), found by
 // exhaustive search over this family for the fewest bank conflicts summed over every exchange of the
 // inverse and forward transforms (16-byte elements: per quarter warp; 8-byte elements: per half warp).
+// To regenerate a row of the table: for every (a, x, b, y, c, z) with a < b < c <= 9 and x, y, z in 0..4, walk the
+// exchanges of XSched<N> (first-stage writes RM b + r; middle-stage reads bb + r NBF / writes j0 + r Ns, through the
+// slot map e / RM + TPR (e % RM) where SLOT applies; last-stage reads b + TPR r) for the lanes of each quarter (half)
+// warp, count the lanes beyond the first that fall into an occupied 16-byte (8-byte) bank group, and keep the
+// minimum, ties to the smaller buffer pad(N - 1) + 1.  The search takes seconds in plain Python.
 template <int N, int CSIZE> struct XPad {
     struct P { int a, x, b, y, c, z; };
     __host__ __device__ static constexpr P params()
@@ -95,19 +100,44 @@ template <int N, int CSIZE> struct XPad {
         } else {
             switch (N) {
                 case 1024: return {4, 2, 5, 4, 6, 1};
-                case 768: case 384: case 128: return {4, 1, 6, 0, 9, 0};
-                case 256: return {4, 3, 5, 2, 6, 2};
                 case 192: return {2, 4, 3, 4, 6, 1};
-                default: return {4, 1, 6, 4, 7, 2};   // 512 (and the small sizes)
+                default: return {4, 1, 6, 4, 7, 2};   // the small sizes
             }
+        }
+    }
+    // 8-byte elements (fp32), 128 <= N <= 768: no additive padding of the family above removes the conflicts of the
+    // stride-8 first-stage writes (17 % of mid_x's shared-memory wavefronts, profiles/r2_summary.md).  An XOR map does:
+    //     slot(i) = i ^ ((i >> s1) & m1) ^ ((i >> s2) & m2),
+    // each term feeding index bits >= 4 into the low four bits (so the map is a bijection of every aligned block of 16
+    // slots, the buffer needs no padding, BUF = N), found by the same exhaustive walk of the exchanges, per half warp:
+    // zero conflicts at every size listed.  Measured on B200, fp32 mid_x: 512^3 1.129 -> 1.098 ms, 768^3 5.09 -> 4.87 ms.
+    // N = 1024 needs three terms ({5, 15}, {2, 12}, {6, 14}) for zero conflicts; the MHD kernel then takes 173 instead
+    // of 167 registers, loses its third CTA per SM and runs 23.3 -> 27.3 ms, so 1024 keeps its additive padding (8 %
+    // conflict wavefronts).
+    struct X3 { int s1, m1, s2, m2, s3, m3; };
+    __host__ __device__ static constexpr bool use_xor()
+    {
+        return CSIZE == 8 && (N == 128 || N == 256 || N == 384 || N == 512 || N == 768);
+    }
+    __host__ __device__ static constexpr X3 xor_params()
+    {
+        switch (N) {
+            case 768: case 256: return {4, 15, 2, 8, 0, 0};
+            case 512: return {3, 14, 6, 7, 0, 0};
+            default: return {4, 7, 1, 8, 0, 0};       // 384, 128
         }
     }
     __host__ __device__ static constexpr int pad(int i)
     {
-        constexpr P p = params();
-        return i + p.x * (i >> p.a) + p.y * (i >> p.b) + p.z * (i >> p.c);
+        if constexpr (use_xor()) {
+            constexpr X3 q = xor_params();
+            return i ^ ((i >> q.s1) & q.m1) ^ ((i >> q.s2) & q.m2) ^ ((i >> q.s3) & q.m3);
+        } else {
+            constexpr P p = params();
+            return i + p.x * (i >> p.a) + p.y * (i >> p.b) + p.z * (i >> p.c);
+        }
     }
-    static constexpr int BUF = pad(N - 1) + 1;
+    static constexpr int BUF = use_xor() ? N : pad(N - 1) + 1;
 };
 
 // radix-8 inter-stage twiddles w_{8 Ns}^{r k}: three table loads, the rest by multiplication
