@@ -159,3 +159,25 @@ def test_box_on_a_cubic_plan_and_bad_boxes():
     for bad in [(0.0, 1.0, 1.0), (1.0, -2.0, 1.0), (1.0, 1.0, float("inf")), (float("nan"), 1.0, 1.0)]:
         with pytest.raises(psfft.PsfftError):
             psfft.plan_set_box(p.handle, *bad)
+
+
+def test_anisotropic_rk_step_is_graph_capturable_and_replays_bit_for_bit():
+    """A Boussinesq RK2 step on the flat-box aspect ratio captured as one CUDA graph (the execute calls only enqueue)."""
+    shape, box = (128, 128, 32), (TWO_PI, TWO_PI, TWO_PI / 4)
+    y = np.concatenate([synth.aniso_spectrum(shape, box, seed=5), synth.aniso_spectrum(shape, box, seed=5, tag=7, ncomp=1)[None]])
+    p = psfft.Plan(shape, torch.float64, 1, work="rk_boussinesq", box=box)
+    yd = dev(y)
+    out = torch.empty_like(yd)
+    work = p.ensure_work("rk_boussinesq")
+    eager = p.rk_step(psfft.SYS_BOUSSINESQ, yd, 2, 1e-3, 0.01, 0.02, 1.5).clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        psfft.rk_step(p.handle, psfft.SYS_BOUSSINESQ, yd, out, 2, 1e-3, (0.01, 0.02, 1.5), work, stream=s)   # warm-up
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            psfft.rk_step(p.handle, psfft.SYS_BOUSSINESQ, yd, out, 2, 1e-3, (0.01, 0.02, 1.5), work, stream=s)
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, eager)

@@ -71,3 +71,49 @@ def test_packed_mode_blocks_and_argument_checks():
     for bad in [(3, 0), (2, 2), (0, 0), (17, 0)]:
         with pytest.raises(psfft.PsfftError):
             psfft.slab_query(plan.handle, *bad)
+
+
+def test_slab_argument_checks_and_guard_bands():
+    """Bad pointers are refused before anything is enqueued; a phase-1 call writes its work buffer and the blocks it was
+    given and nothing around them (buffers carved from one arena with NaN guard bands)."""
+    import ctypes
+    shape, P = (32, 16, 16), 4
+    Nx, Ny, Nz = shape
+    plan = psfft.Plan(shape, torch.float64, 1)
+    lay = psfft.slab_query(plan.handle, P, 1)
+    L = psfft.lib()
+    real = torch.rand((lay.Mz, Ny, Nx), dtype=torch.float64, device="cuda")
+    zs = torch.empty(lay.zspec_elems, dtype=torch.complex128, device="cuda")
+    blocks = [torch.empty(psfft.slab_query(plan.handle, P, q).xslab_elems, dtype=torch.complex128, device="cuda") for q in range(P)]
+    st = torch.cuda.current_stream().cuda_stream
+    arr = (ctypes.c_void_p * P)(*[b.data_ptr() for b in blocks])
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), None, 0, st) == -1          # NULL
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr() + 8, zs.data_ptr(), arr, 0, st) == -4       # alignment
+    bad = (ctypes.c_void_p * P)(blocks[0].data_ptr(), None, blocks[2].data_ptr(), blocks[3].data_ptr())
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), bad, 0, st) == -1
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), arr, -1, st) == -2          # zoff < 0
+    assert L.psfft_slab_z(plan.handle, P, 1, 0, blocks[1].data_ptr(), st) == -2                               # dir
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, zs.data_ptr(), zs.data_ptr(), arr, 0, st) == -8             # overlap
+    # guard bands: arena = [guard | zspec | guard | block 0 | guard | ... ]
+    G = 512
+    sizes = [lay.zspec_elems] + [psfft.slab_query(plan.handle, P, q).xslab_elems for q in range(P)]
+    arena = torch.full((sum(sizes) + G * (len(sizes) + 1),), complex(float("nan"), float("nan")), dtype=torch.complex128,
+                       device="cuda")
+    offs, o = [], G
+    for n in sizes:
+        offs.append(o)
+        o += n + G
+    views = [arena[a:a + n] for a, n in zip(offs, sizes)]
+    for v in views[1:]:
+        v.zero_()
+    psfft.slab_r2c_xy(plan.handle, P, 1, real, views[0], views[1:], lay.z0)
+    torch.cuda.synchronize()
+    mask = torch.ones_like(arena, dtype=torch.bool)
+    for a, n in zip(offs, sizes):
+        mask[a:a + n] = False
+    assert bool(torch.isnan(arena[mask].real).all())                     # every guard element untouched
+    assert not bool(torch.isnan(views[0].real).any())                   # the work buffer was written
+    for q, v in enumerate(views[1:]):                                    # each block got exactly this rank's planes
+        w = psfft.slab_query(plan.handle, P, q).w
+        blk = v.view(Nz, Ny, w)
+        assert bool((blk[lay.z0:lay.z0 + lay.Mz] != 0).any()) and bool((blk[:lay.z0] == 0).all()) and bool((blk[lay.z0 + lay.Mz:] == 0).all())
