@@ -441,6 +441,7 @@ def flat_box_rows(torch, psfft, synth, dev, stream, peak, K, timed) -> dict:
     """SURVEY.md §8(f) NEXT-2 at the paper's flat-box size: Boussinesq right-hand side and one RK2
     step on 1024 x 1024 x 256 in the box (2 pi, 2 pi, 2 pi / 4), fp64, device-resident broadband input."""
     import math
+    import numpy as np
     shape, box = (1024, 1024, 256), (2 * math.pi, 2 * math.pi, 2 * math.pi / 4)
     p = psfft.Plan(shape, torch.float64, 1, device=dev, work="rk_boussinesq", box=box)
     y = torch.empty(p.spec_shape(4), dtype=torch.complex128, device=dev)
@@ -460,12 +461,33 @@ def flat_box_rows(torch, psfft, synth, dev, stream, peak, K, timed) -> dict:
     rl = roofline_of(psfft.profile_records(p.handle), n, t_rhs, 56.0 * p.layout.spec_bytes,
                      "fused 3-pass dense count = 56 C (9 + 4 transforms + 4 C epilogue reads)", peak, "1024x1024x256 fp64")
     t_rk = timed(f_rk, n)
+    p.close()
+    del p, y, out, wk
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    big = None
+    if torch.cuda.mem_get_info(dev)[0] > 125 * 2**30:   # the paper's largest grid, fp32: 115 GB resident
+        shape2 = (2048, 2048, 512)
+        p2 = psfft.Plan(shape2, torch.float32, 1, device=dev, work="hd", box=box)
+        u2 = torch.zeros(p2.spec_shape(3), dtype=torch.complex64, device=dev)
+        small = synth.aniso_spectrum((256, 256, 64), box, seed=1234, fill=0.4, dtype="complex64")   # modes of the low shells
+        idx = lambda n_small, n_big: torch.from_numpy((np.fft.fftfreq(n_small, 1.0 / n_small).astype("int64")) % n_big).to(dev)
+        iz, iy = idx(64, 512), idx(256, 2048)
+        u2[:, iz[:, None], iy[None, :], :129] = torch.from_numpy(small).to(dev) * (float(np.prod(shape2)) / (256 * 256 * 64))
+        r2 = torch.empty_like(u2)
+        w2 = p2.ensure_work("hd")
+        t2 = timed(lambda: psfft.hd_rhs(p2.handle, u2, r2, 1e-3, w2), max(3, min(K, 5)))
+        big = {"workload": "2048 x 2048 x 512 fp32 HD RHS in the box (2 pi, 2 pi, 2 pi/4): the paper's largest grid "
+                           "(PAPER.md:370) on ONE GPU, 115 GB resident; band-limited random solenoidal field",
+               "ms": t2, "evals_per_s": 1e3 / t2}
+        p2.close()
+        del p2, u2, r2, w2
     res = {"workload": "1024 x 1024 x 256 fp64 Boussinesq in the box (2 pi, 2 pi, 2 pi/4), broadband solenoidal u + theta "
                        "(synth.aniso_spectrum, fill 0.2), nu = kappa = 1e-3, N_bv = 2",
            "boussinesq_rhs": {"ms": t_rhs, "evals_per_s": 1e3 / t_rhs, "frac_bytes_moved": rl["step_bytes_moved"]["frac"],
                               "per_kernel": rl["per_kernel"]},
-           "boussinesq_rk2_step": {"ms": t_rk, "steps_per_s": 1e3 / t_rk}, "steps": n}
-    p.close()
+           "boussinesq_rk2_step": {"ms": t_rk, "steps_per_s": 1e3 / t_rk}, "steps": n, "largest_grid": big}
     return res
 
 

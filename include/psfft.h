@@ -82,7 +82,8 @@ typedef struct psfft_layout {
 } psfft_layout;
 
 /* Sizes for a prospective plan.  Supported N: 2^a * 3^b with b <= 1 and 8 <= N <= 1024
- * (8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024).  Host-only. */
+ * (8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024), and 2048 (the paper's largest grid is
+ * 2048 x 2048 x 512; a cubic 2048^3 field does not fit one GPU).  Host-only. */
 int psfft_plan_query(int N, int dtype, int batch, psfft_layout *out);
 
 /* Create a plan ("create plan": sizes from the input size and datatype).

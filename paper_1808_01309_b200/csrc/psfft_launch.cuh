@@ -6,13 +6,13 @@
 
 namespace psfft {
 
-// every supported grid size, in one place (psfft.h: 2^a 3^b, b <= 1, 8 <= N <= 1024)
+// every supported grid size, in one place (psfft.h: 2^a 3^b, b <= 1, 8 <= N <= 1024, and 2048)
 // (-D"PSFFT_SIZES(X)=X(32) X(512)" restricts the list for quick experimental builds)
 #ifdef PSFFT_SIZES
 #define PSFFT_FOR_EACH_N(X) PSFFT_SIZES(X)
 #else
 #define PSFFT_FOR_EACH_N(X) \
-    X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024)
+    X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024) X(2048)
 #endif
 
 struct PassArgs {

@@ -96,12 +96,15 @@ __host__ __device__ constexpr int job_tpf(int N, int TC, int esize)
     return (N >= 64 && N % 8 == 0 && max_radix(N) == 8 && TC * (N / 8) <= cap) ? N / 8 : cpass_tpf(N);
 }
 
+// plain passes: 64 KB tiles; at N = 2048 a 64 KB tile would have 32-byte rows, so one 128 KB tile with 64-byte rows
+__host__ __device__ constexpr long plain_tile_cap(int N) { return N >= 2048 ? 131072 : 65536; }
+
 template <typename T, int N, int DIR>
 static cudaError_t cpass_n(const PassArgs &a, int axis, const void *in, void *out, int fields)
 {
     // 16-byte elements in both precisions; the plain passes keep 64 KB tiles at every N (measured: 1024 x 1024 x 256
     // r2c + c2r 5.77 ms with 64 KB tiles, 5.96 ms with 128 KB ones)
-    constexpr int TC = cpass_cols_cap(N, (int)sizeof(Ex<T>), 65536);
+    constexpr int TC = cpass_cols_cap(N, (int)sizeof(Ex<T>), plain_tile_cap(N));
     constexpr int TPF = job_tpf(N, TC, 16);
     constexpr int MINB = ((long)N * TC * 16 * 2 <= 220 * 1024 && 2 * TC * TPF <= 1024) ? 2 : 1;
     return cpass_v<T, N, DIR, TC, TPF, MINB>(a, axis, in, out, fields);
@@ -112,7 +115,7 @@ template <typename T, int N, int DIR>
 static cudaError_t cpass_raw_n(const PassArgs &a, const void *tw, const void *in, void *out, long axis_stride, long inner,
                                long outer_stride, long outer)
 {
-    constexpr int TC = cpass_cols_cap(N, (int)sizeof(Ex<T>), 65536);
+    constexpr int TC = cpass_cols_cap(N, (int)sizeof(Ex<T>), plain_tile_cap(N));
     constexpr int TPF = job_tpf(N, TC, 16);
     constexpr int MINB = ((long)N * TC * 16 * 2 <= 220 * 1024 && 2 * TC * TPF <= 1024) ? 2 : 1;
     return cpass_strided<T, N, DIR, TC, TPF, MINB>(a, tw, in, out, axis_stride, inner, outer_stride, outer);
@@ -139,7 +142,7 @@ static cudaError_t cpass_xdist_n(const PassArgs &a, const void *slab_in, void *s
     using C = Cx<T>;
     using E = Ex<T>;
     constexpr int EW = ElemWidth<E>::value;
-    constexpr int TC = cpass_cols_cap(N, (int)sizeof(E), 65536);
+    constexpr int TC = cpass_cols_cap(N, (int)sizeof(E), plain_tile_cap(N));
     constexpr int TPF = job_tpf(N, TC, 16);
     constexpr int MINB = ((long)N * TC * 16 * 2 <= 220 * 1024 && 2 * TC * TPF <= 1024) ? 2 : 1;
     constexpr bool PAD = (TC * sizeof(E) < 128);

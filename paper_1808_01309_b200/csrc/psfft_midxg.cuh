@@ -30,7 +30,7 @@
 // RM = 8 if 64 | N, 4 if 16 | N, else 2:
 //     8: 2 2 2    12: 2 3 2    16: 4 4      24: 2 2 3 2   32: 4 2 4     48: 4 3 4     64: 8 8
 //    96: 4 2 3 4 128: 8 2 8   192: 8 3 8   256: 8 4 8    384: 8 2 3 8  512: 8 8 8    768: 8 4 3 8
-//  1024: 8 4 4 8
+//  1024: 8 4 4 8   2048: 8 8 4 8
 // N / RM threads own one row; a thread does one radix-RM butterfly in the outer stages and RM / R (rounded
 // up, predicated) radix-R butterflies in a middle stage.  The twiddle tables of this schedule are a third
 // table of the plan (PassArgs::twX), laid out per stage as [r - 1][k] like the others.
@@ -91,6 +91,7 @@ template <int N, int CSIZE> struct XPad {
     {
         if (CSIZE == 16) {
             switch (N) {
+                case 2048: return {3, 1, 8, 1, 11, 0};
                 case 1024: return {3, 1, 7, 1, 9, 0};
                 case 768: return {3, 1, 6, 1, 8, 4};
                 case 384: return {3, 1, 6, 3, 7, 2};

@@ -43,7 +43,9 @@ def test_plan_query_sizes(lib):
 def test_error_codes(lib):
     lay = psfft.Layout()
     assert lib.psfft_plan_query(500, psfft.F64, 1, ctypes.byref(lay)) == -2     # unsupported N
-    assert lib.psfft_plan_query(2048, psfft.F64, 1, ctypes.byref(lay)) == -2
+    assert lib.psfft_plan_query(4096, psfft.F64, 1, ctypes.byref(lay)) == -2
+    assert lib.psfft_plan_query(1536, psfft.F64, 1, ctypes.byref(lay)) == -2
+    assert lib.psfft_plan_query3(2048, 2048, 512, psfft.F32, 1, ctypes.byref(lay)) == 0 and lay.ldk == 1025
     assert lib.psfft_plan_query(512, 7, 1, ctypes.byref(lay)) == -3
     assert lib.psfft_plan_query(512, psfft.F64, 0, ctypes.byref(lay)) == -2
     assert lib.psfft_plan_query(512, psfft.F64, 1, None) == -1

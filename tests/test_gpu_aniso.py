@@ -181,3 +181,26 @@ def test_anisotropic_rk_step_is_graph_capturable_and_replays_bit_for_bit():
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(out, eager)
+
+
+# ---- N = 2048 (the paper's largest grid is 2048 x 2048 x 512) on every axis ------------------------------
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("shape", [(2048, 16, 8), (16, 2048, 8), (8, 16, 2048)])
+def test_length_2048_transforms_and_rhs_on_each_axis(shape, dtype):
+    """The 8 8 8 4 column schedule / 8 8 4 8 row schedule of length 2048 in the x-, y- and z-pass: plain transforms
+    and the Boussinesq right-hand side against the oracle."""
+    Nx, Ny, Nz = shape
+    box = (TWO_PI, 3.0, 5.0)
+    x = synth.uniform01(3, np.arange(Nz * Ny * Nx, dtype=np.uint64)).reshape(1, Nz, Ny, Nx) * 2 - 1
+    x = x.astype(np.float64 if dtype == torch.float64 else np.float32)
+    p = psfft.Plan(shape, dtype, 1, work="boussinesq", box=box)
+    X = p.r2c(dev(x))
+    assert rel(X.cpu().numpy()[0], oracle.r2c3d(x[0].astype(np.float64))) < TOL[dtype]
+    assert rel(p.c2r(X).cpu().numpy(), x) < TOL[dtype]
+    uh = synth.aniso_spectrum(shape, box, seed=31).astype(CDT[dtype])
+    th = synth.aniso_spectrum(shape, box, seed=31, tag=7, ncomp=1).astype(CDT[dtype])
+    ru, rt = p.boussinesq_rhs(dev(uh), dev(th), 0.01, 0.02, 1.5)
+    wu, wt = oracle.boussinesq_rhs(uh.astype(np.complex128), th.astype(np.complex128), 0.01, 0.02, 1.5, box=box)
+    assert rel(ru.cpu().numpy(), wu) < TOL[dtype] and rel(rt.cpu().numpy(), wt) < TOL[dtype]
+    check_mask(ru.cpu().numpy(), shape)

@@ -491,3 +491,88 @@ def test_boussinesq_rk2_1024x1024x256_against_the_256x256x64_oracle(dtype):
     fz, fy, fx = np.fft.fftfreq(FLAT[2]) * 4, np.fft.fftfreq(FLAT[1]) * 4, np.arange(FLAT[0] // 2 + 1) / FLAT[0] * 4
     far = (fz[:, None, None] ** 2 + fy[None, :, None] ** 2 + fx[None, None, :] ** 2) > 0.66**2
     assert np.linalg.norm(got[:, far].astype(np.complex128).ravel()) / nbig / np.linalg.norm(sm.ravel()) < tol
+
+
+# ---- the paper's largest grid: 2048 x 2048 x 512 (Fig. 7), fp32 (a field is 8.6 GB; HD needs 115 GB) ---------
+
+def test_hd_rhs_2048x2048x512_fp32_against_the_512x512x128_oracle():
+    """P12 on the largest grid of the paper: the same band-limited coefficients (index fill 0.3 of the small grid) on
+    512 x 512 x 128 give the same right-hand side on every mode the small grid retains; beyond twice the band limit the
+    big grid's result is roundoff; the masked region is exactly zero (sampled planes)."""
+    big, small = (2048, 2048, 512), (512, 512, 128)
+    box = (2 * np.pi, 2 * np.pi, 2 * np.pi / 4)
+    free = torch.cuda.mem_get_info()[0]
+    if free < 125 * 2**30:
+        pytest.skip(f"needs 115 GB of device memory, {free / 2**30:.0f} GiB free")
+    f = 0.3
+    us = synth.aniso_spectrum(small, box, seed=55, fill=f)
+    ub = synth.aniso_spectrum(big, box, seed=55, fill=f / 4, dtype=np.complex64)
+    p = psfft.Plan(big, torch.float32, 1, work="hd", box=box)
+    got_d = p.hd_rhs(torch.from_numpy(ub).cuda(), 1e-3)
+    del ub
+    want = oracle.hd_rhs(us, 1e-3, box=box)
+    nb, ns = float(np.prod(big)), float(np.prod(small))
+    iz = np.r_[0:64, big[2] - 64:big[2]]
+    iy = np.r_[0:256, big[1] - 256:big[1]]
+    jz = np.r_[0:64, small[2] - 64:small[2]]
+    jy = np.r_[0:256, small[1] - 256:small[1]]
+    izt, iyt = torch.from_numpy(iz).cuda(), torch.from_numpy(iy).cuda()
+    sub = got_d[:, izt][:, :, iyt][:, :, :, :256].cpu().numpy().astype(np.complex128) / nb
+    sm = want[:, jz][:, :, jy][:, :, :, :256] / ns
+    Ms = oracle.dealias_mask(*small)[jz][:, jy][:, :, :256]
+    assert Ms.sum() > 5e5 and np.all(sm[:, ~Ms] == 0)
+    assert np.linalg.norm((sub - sm)[:, Ms].ravel()) / np.linalg.norm(sm.ravel()) < 2e-5
+    # everything beyond 0.62 of the small grid's index range (2 x the band limit) is roundoff: energy summed on the device
+    fz = torch.fft.fftfreq(big[2], device="cuda", dtype=torch.float64) * 4
+    fy = torch.fft.fftfreq(big[1], device="cuda", dtype=torch.float64) * 4
+    fx = torch.arange(big[0] // 2 + 1, device="cuda", dtype=torch.float64) / big[0] * 4
+    far_e = 0.0
+    for z in range(big[2]):
+        far = (fz[z] ** 2 + fy[:, None] ** 2 + fx[None, :] ** 2) > 0.62**2
+        far_e += float((got_d[:, z].abs().to(torch.float64) ** 2 * far).sum())
+    assert np.sqrt(far_e) / nb / np.linalg.norm(sm.ravel()) < 2e-5
+    # exact zeros outside the big grid's own mask on sampled planes
+    for z in (0, 1, 170, 171, 256, 341, 511):
+        nz = z if z < 256 else z - 512
+        keep = torch.from_numpy(9 * ((np.fft.fftfreq(2048)[:, None]) ** 2 + (np.arange(1025)[None, :] / 2048) ** 2 + (nz / 512) ** 2) < 1).cuda()
+        assert float(got_d[:, z][:, ~keep].abs().max()) == 0.0
+
+
+def test_hd_rhs_2048x2048x512_fp32_broadband_invariants():
+    """Every shell of the ellipsoid populated (and the modes the input mask removes): no oracle fits this size, so what
+    holds at any size is checked on the device -- the nonlinear term conserves energy, Re sum w conj(M u^) . R = 0,
+    R is solenoidal with the box's wavenumbers, R vanishes exactly outside the mask and is O(1) inside its last shell."""
+    big = (2048, 2048, 512)
+    box = (2 * np.pi, 2 * np.pi, 2 * np.pi / 4)
+    free = torch.cuda.mem_get_info()[0]
+    if free < 150 * 2**30:
+        pytest.skip(f"needs 141 GB of device memory, {free / 2**30:.0f} GiB free")
+    p = psfft.Plan(big, torch.float32, 1, work="hd", box=box)
+    u = torch.from_numpy(synth.aniso_spectrum(big, box, seed=66, dtype=np.complex64)).cuda()
+    R = p.hd_rhs(u)
+    Nx, Ny, Nz = big
+    fy = torch.fft.fftfreq(Ny, device="cuda", dtype=torch.float64)
+    fx = torch.arange(Nx // 2 + 1, device="cuda", dtype=torch.float64) / Nx
+    ky = (fy * Ny * (2 * np.pi / box[1]))[:, None]
+    kx = (fx * Nx * (2 * np.pi / box[0]))[None, :]
+    w = torch.full((Nx // 2 + 1,), 2.0, device="cuda", dtype=torch.float64)
+    w[0] = w[-1] = 1.0
+    dE = uu = rr = div = 0.0
+    outer = 0.0
+    for z in range(Nz):
+        nz = z if z < Nz // 2 else z - Nz
+        rho2 = (nz / Nz) ** 2 + fy[:, None] ** 2 + fx[None, :] ** 2
+        keep = 9 * rho2 < 1
+        uz, rz = u[:, z].to(torch.complex128), R[:, z].to(torch.complex128)
+        assert float(rz[:, ~keep].abs().max()) == 0.0
+        um = uz * keep
+        dE += float((w * (um.conj() * rz).real.sum(0)).sum())
+        uu += float((w * (um.abs() ** 2).sum(0)).sum())
+        rr += float((w * (rz.abs() ** 2).sum(0)).sum())
+        kz = nz * (2 * np.pi / box[2])
+        div += float((w * (kx * rz[0] + ky * rz[1] + kz * rz[2]).abs() ** 2).sum())
+        outer += float((rz.abs() ** 2).sum(0)[keep & (9 * rho2 > 0.875**2)].sum())
+    assert abs(dE) / np.sqrt(uu * rr) < 2e-6                      # energy conservation (fp32 accumulation of 6e8 modes)
+    kmax2 = (Nx / 3) ** 2 * 3
+    assert np.sqrt(div / (rr * kmax2)) < 2e-6                     # k . R = 0
+    assert outer / rr > 1e-3                                      # the last eighth of the ellipsoid's radius carries the cascade

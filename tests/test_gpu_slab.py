@@ -29,7 +29,7 @@ def rel(a, b):
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("shape,P", [((32, 32, 32), 2), ((32, 32, 32), 8), ((64, 48, 16), 4), ((128, 128, 128), 8),
-                                     ((24, 16, 48), 3), ((64, 8, 16), 16), ((256, 64, 32), 2), ((32, 32, 32), 1)])
+                                     ((24, 16, 48), 3), ((64, 8, 16), 16), ((256, 64, 32), 2), ((32, 32, 32), 1), ((16, 2048, 16), 4)])
 def test_virtual_ranks_equal_the_single_gpu_transform_bit_for_bit(shape, P, dtype):
     Nx, Ny, Nz = shape
     x = field(shape, dtype)
