@@ -117,3 +117,34 @@ def test_slab_argument_checks_and_guard_bands():
         w = psfft.slab_query(plan.handle, P, q).w
         blk = v.view(Nz, Ny, w)
         assert bool((blk[lay.z0:lay.z0 + lay.Mz] != 0).any()) and bool((blk[:lay.z0] == 0).all()) and bool((blk[lay.z0 + lay.Mz:] == 0).all())
+
+
+def test_packed_mode_class_under_torch_distributed_world_size_1():
+    """slab.SlabFFT (the torch.distributed / NCCL path: send buffer of contiguous slices, one all_to_all_single, x-slab
+    z-pass) on the one GPU this box has: a world of one rank must reproduce the single-GPU transform bit for bit.  (The
+    exchange schedule for P > 1 is covered on CPU tensors by tests/test_slab_dist.py.)"""
+    import os
+    import socket
+    import torch.distributed as dist
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        shape = (64, 48, 32)
+        x = field(shape, torch.float64)
+        plan = psfft.Plan(shape, torch.float64, 1)
+        xd = torch.from_numpy(x).cuda()
+        single = plan.r2c(xd[None])[0]
+        sf = slab.SlabFFT(plan)
+        X = sf.r2c(xd)
+        assert torch.equal(X, single)
+        back = sf.c2r(X.clone())
+        assert torch.equal(back, plan.c2r(single[None])[0])
+    finally:
+        dist.destroy_process_group()
