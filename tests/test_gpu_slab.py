@@ -148,3 +148,28 @@ def test_packed_mode_class_under_torch_distributed_world_size_1():
         assert torch.equal(back, plan.c2r(single[None])[0])
     finally:
         dist.destroy_process_group()
+
+
+def test_bench_multi_gpu_slab_row_in_a_world_of_one():
+    """bench.py's slab_multi (what `--gpus N` adds to the line for N > 1) runs end to end under NCCL with one rank."""
+    import os
+    import socket
+    import sys
+    import torch.distributed as dist
+    if dist.is_initialized():
+        pytest.skip("a process group already exists in this process")
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        res = bench.slab_multi(torch, psfft, torch.device("cuda", 0), torch.cuda.current_stream(), 3, N=128)
+        assert "failed" not in res, res
+        assert res["roundtrip_max_abs_err"] < 1e-13 and res["ms_r2c"] > 0 and res["ms_c2r"] > 0
+    finally:
+        dist.destroy_process_group()
