@@ -173,3 +173,47 @@ def test_bench_multi_gpu_slab_row_in_a_world_of_one():
         assert res["roundtrip_max_abs_err"] < 1e-13 and res["ms_r2c"] > 0 and res["ms_c2r"] > 0
     finally:
         dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("shape,P", [((64, 32, 32), 4), ((32, 48, 24), 3), ((128, 64, 64), 8)])
+def test_packed_mode_for_P_ranks_emulated_on_one_gpu(shape, P):
+    """The packed (NCCL) mode for P > 1 without a process group: every rank's phase 1 fills its send buffer, the
+    all_to_all_single is replayed as tensor copies with slab.forward_splits' counts (slice q of rank p's send buffer
+    becomes slice p of rank q's receive buffer -- the semantics of the collective), phase 2 runs on the receive
+    buffers, and the assembled x-slabs equal the single-GPU transform bit for bit; then the inverse the same way."""
+    Nx, Ny, Nz = shape
+    ldk = Nx // 2 + 1
+    x = field(shape, torch.float64)
+    plan = psfft.Plan(shape, torch.float64, 1)
+    xd = torch.from_numpy(x).cuda()
+    single = plan.r2c(xd[None])[0]
+    lays = [psfft.slab_query(plan.handle, P, r) for r in range(P)]
+    Mz = lays[0].Mz
+    cd = torch.complex128
+    sends = [torch.empty(l.zspec_elems, dtype=cd, device="cuda") for l in lays]
+    zs = torch.empty(lays[0].zspec_elems, dtype=cd, device="cuda")
+    splits = [slab.forward_splits(Nz, Ny, ldk, P, r) for r in range(P)]
+    for r in range(P):
+        psfft.slab_r2c_xy(plan.handle, P, r, xd[r * Mz:(r + 1) * Mz], zs, slab._slice_ptrs(sends[r], splits[r][0]), 0)
+    recvs = []
+    for q in range(P):                                   # all_to_all_single, replayed
+        parts = []
+        for p_ in range(P):
+            off = sum(splits[p_][0][:q])
+            parts.append(sends[p_][off:off + splits[p_][0][q]])
+            assert splits[p_][0][q] == splits[q][1][p_]  # what p sends to q is what q expects from p
+        recvs.append(torch.cat(parts))
+        assert recvs[q].numel() == lays[q].xslab_elems
+    for q in range(P):
+        psfft.slab_z(plan.handle, P, q, -1, recvs[q])
+    got = torch.cat([recvs[q].view(Nz, Ny, lays[q].w) for q in range(P)], dim=2)
+    assert torch.equal(got, single)
+    # inverse: z-pass on the x-slabs, exchange of contiguous z-ranges, gather-load y-pass + c2r
+    for q in range(P):
+        psfft.slab_z(plan.handle, P, q, +1, recvs[q])
+    back = torch.empty((Nz, Ny, Nx), dtype=torch.float64, device="cuda")
+    for r in range(P):
+        parts = [recvs[q].view(Nz, Ny, lays[q].w)[r * Mz:(r + 1) * Mz].reshape(-1) for q in range(P)]   # what q sends to r
+        rbuf = torch.cat(parts)
+        psfft.slab_c2r_yx(plan.handle, P, r, slab._slice_ptrs(rbuf, splits[r][0]), 0, zs, back[r * Mz:(r + 1) * Mz])
+    assert torch.equal(back, plan.c2r(single[None])[0])
