@@ -59,6 +59,7 @@ extern "C" {
 #define PSFFT_E_PLAN (-6)        /* invalid or destroyed plan handle */
 #define PSFFT_E_BATCH (-7)       /* batch * Nz exceeds 65535 (grid limit of the y-pass) */
 #define PSFFT_E_OVERLAP (-8)     /* an output or workspace range of the call overlaps another range of the call */
+#define PSFFT_E_SCRATCH (-9)     /* psfft_fft3d_c2r_static: the plan needs more workspace than PSFFT_STATIC_SCRATCH_BYTES */
 
 typedef struct psfft_plan_s *psfft_plan;
 
@@ -137,6 +138,45 @@ int psfft_fft3d_r2c(psfft_plan plan, const void *d_real, void *d_spec, void *d_w
  *   d_real  out  batch * N^3 reals
  *   d_work       >= work_bytes_fft */
 int psfft_fft3d_c2r(psfft_plan plan, const void *d_spec, void *d_real, void *d_work, void *stream);
+
+/* Inverse transform for callers that have no device memory to give as workspace and cannot get any.
+ *
+ * psfft_fft3d_c2r needs a workspace of work_bytes_fft next to its input and output, because it must leave the
+ * input spectrum untouched.  Normally the caller allocates that once.  Some callers cannot: a solver whose
+ * host application handed it a fixed set of field buffers and forbids further device allocation (every byte of
+ * HBM is already spoken for by the application's own arena, so a cudaMalloc would fail, or the time loop is not
+ * allowed to stall on the device-wide synchronisation that cudaMalloc / cudaFree imply), or a plug-in that runs
+ * inside someone else's process where it does not own the allocator at all.  For them this call takes the
+ * workspace from an array that is part of the library image itself:
+ *
+ *     static __device__ __align__(256) unsigned char [PSFFT_STATIC_SCRATCH_BYTES]     (32 MiB)
+ *
+ * The CUDA runtime places that array on every GPU on which this library's device code gets loaded, and it stays
+ * there until the process exits -- that is the price, and the reason the limit is modest.  The call itself
+ * allocates nothing: no cudaMalloc / cudaFree, no event or stream creation, no allocating library routine; it
+ * only enqueues the same three kernels as psfft_fft3d_c2r (z-pass, y-pass, c2r x-pass) with the array as d_work,
+ * so the result is bit for bit that of psfft_fft3d_c2r.
+ *
+ *   d_spec  in   batch * ldk*Ny*Nz complex (not modified)
+ *   d_real  out  batch * Nx*Ny*Nz reals
+ *
+ * Limit     the plan's layout.work_bytes_fft (= batch * spec_bytes) must not exceed PSFFT_STATIC_SCRATCH_BYTES:
+ *           e.g. 128^3 fp64 batch 1 (17.0 MB), 128^3 fp32 batch 3 (25.6 MB), 192^3 fp32 batch 1 (28.6 MB).  A
+ *           larger plan gets PSFFT_E_SCRATCH and nothing is enqueued; use psfft_fft3d_c2r with your own workspace.
+ * Set-up    the first call on each device looks up where the array lives on that device (cudaGetSymbolAddress,
+ *           with the caller's current device -- the one that holds d_spec and d_real -- and its return code
+ *           checked) and remembers it; later calls on that device skip this.  Make that first call outside any
+ *           stream capture.
+ * Sharing   there is ONE array per device, shared by every plan and every call.  Two calls that can run on the
+ *           GPU at the same time (different streams, different host threads) race on it and both produce
+ *           garbage: serialise them on one stream, or order them with events.  The array keeps whatever the last
+ *           call left in it; this call does not depend on that, because its first pass overwrites every element
+ *           the later passes read, so nothing has to be cleared.
+ * Profiling the per-launch event hooks below (psfft_profile_*) are not fed by this call, because creating events
+ *           allocates.  psfft_last_launch_count works.
+ * Errors    as psfft_fft3d_c2r, plus PSFFT_E_SCRATCH. */
+#define PSFFT_STATIC_SCRATCH_BYTES (32u << 20)
+int psfft_fft3d_c2r_static(psfft_plan plan, const void *d_spec, void *d_real, void *stream);
 
 /* One Navier-Stokes right-hand side (Eq. 1 with theta = 0, Eq. 3):
  *     rhs = M P F[ F^-1(M u^) x F^-1(i k x M u^) ] - nu |k|^2 M u^

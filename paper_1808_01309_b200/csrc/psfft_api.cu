@@ -952,6 +952,9 @@ const char *psfft_strerror(int code)
         case PSFFT_E_PLAN: return "psfft: invalid plan handle";
         case PSFFT_E_BATCH: return "psfft: batch too large (batch * Nz must not exceed 65535)";
         case PSFFT_E_OVERLAP: return "psfft: input, output and workspace ranges of a call must not overlap";
+        case PSFFT_E_SCRATCH:
+            return "psfft: plan too large for the built-in workspace (work_bytes_fft > PSFFT_STATIC_SCRATCH_BYTES = 32 MiB); "
+                   "call psfft_fft3d_c2r with a workspace of your own";
     }
     if (code > 0) return cudaGetErrorString((cudaError_t)code);
     return "psfft: unknown error code";
@@ -960,3 +963,77 @@ const char *psfft_strerror(int code)
 const char *psfft_version(void) { return "0.1"; }
 
 }  // extern "C"
+
+// ================================================================================================
+// psfft_fft3d_c2r_static: the inverse transform for callers that cannot allocate device memory (psfft.h).
+//
+// Its workspace is this array.  It is part of the library image: the CUDA runtime gives it a home on every GPU
+// that loads this file's device code and keeps it there until the process exits, so no call ever has to ask the
+// driver for memory.  Everything that concerns it sits in this one file on purpose:
+//   * In HOST code the name `g_static_scratch` is only a stand-in the runtime uses to find the symbol.  It is not
+//     a device address.  Handing `g_static_scratch` (or `&g_static_scratch[0]`) to a kernel would make the kernel
+//     fault, or -- on a system where the GPU can read host memory -- quietly work on the wrong bytes.  The device
+//     address has to be asked for, per device, with cudaGetSymbolAddress; static_scratch_address() below does that
+//     once per device, with that device current, and checks the return code.
+//   * The array is shared by all plans and calls on a device and is never cleared.  The z-pass of the inverse
+//     transform writes all batch * ldk * Ny * Nz elements before the y- and x-passes read any of them, so stale
+//     contents of an earlier (possibly larger) call cannot leak into a result.  Calls that overlap on the GPU race.
+static __device__ __align__(256) unsigned char g_static_scratch[PSFFT_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+const int STATIC_SCRATCH_MAX_DEVICES = 64;
+std::mutex g_static_scratch_mu;
+void *g_static_scratch_addr[STATIC_SCRATCH_MAX_DEVICES];   // device address of the array per device; NULL = not asked yet
+
+// Device address of g_static_scratch on the caller's current device.  The first call on a device asks the runtime
+// (this is also what makes the runtime load this file's device image, and with it the array, on that device); the
+// answer is kept, so later calls make no CUDA call here besides cudaGetDevice.
+int static_scratch_address(void **out)
+{
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_SCRATCH_MAX_DEVICES) return (int)cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_scratch_mu);
+    if (!g_static_scratch_addr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return (int)cudaErrorInvalidSymbol;
+        g_static_scratch_addr[dev] = p;
+    }
+    *out = g_static_scratch_addr[dev];
+    return PSFFT_OK;
+}
+
+// The three passes of c2r_fields_inplace without its per-launch event hooks (creating an event allocates).
+template <typename T> int c2r_fields_static(Plan *pl, const PassArgs &a, const void *d_spec, void *scratch, void *d_real)
+{
+    const int fields = pl->lay.batch;
+    const long nrows = (long)fields * a.Ny * a.Nz;
+    const double scale = 1.0 / ((double)a.N * a.Ny * a.Nz);
+    CU(launch_cpass<T>(a, +1, 2, d_spec, scratch, fields, &pl->launches));    // z: input -> scratch (every element written)
+    CU(launch_cpass<T>(a, +1, 1, scratch, scratch, fields, &pl->launches));   // y: in place
+    CU(launch_xpass_c2r<T>(a, scratch, d_real, nrows, scale, &pl->launches)); // x: scratch -> output, scaled
+    return PSFFT_OK;
+}
+
+}  // namespace
+
+extern "C" int psfft_fft3d_c2r_static(psfft_plan plan, const void *d_spec, void *d_real, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!d_real || !d_spec) return PSFFT_E_NULL;
+    if (misaligned(d_real) || misaligned(d_spec)) return PSFFT_E_ALIGN;
+    if (pl->lay.work_bytes_fft > (size_t)PSFFT_STATIC_SCRATCH_BYTES) return PSFFT_E_SCRATCH;   // nothing enqueued
+    void *scratch = nullptr;
+    const int rc = static_scratch_address(&scratch);
+    if (rc) return rc;
+    if (spans_overlap({{d_spec, pl->lay.batch * pl->lay.spec_bytes, false}, {d_real, pl->lay.batch * pl->lay.real_bytes, true},
+                       {scratch, pl->lay.work_bytes_fft, true}}))
+        return PSFFT_E_OVERLAP;
+    pl->launches = 0;
+    PassArgs a = args_of(pl, stream);
+    return pl->lay.dtype == PSFFT_F64 ? c2r_fields_static<double>(pl, a, d_spec, scratch, d_real)
+                                      : c2r_fields_static<float>(pl, a, d_spec, scratch, d_real);
+}

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpsfft.so")
 EXPORTS = [
     "psfft_plan_query", "psfft_plan_create", "psfft_plan_query3", "psfft_plan_create3", "psfft_plan_destroy",
     "psfft_plan_layout", "psfft_plan_set_box",
-    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs", "psfft_gpe_rhs",
+    "psfft_fft3d_r2c", "psfft_fft3d_c2r", "psfft_fft3d_c2r_static", "psfft_hd_rhs", "psfft_mhd_rhs", "psfft_boussinesq_rhs", "psfft_gpe_rhs",
     "psfft_rk_work_bytes", "psfft_rk_step",
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_slab_query", "psfft_slab_r2c_xy", "psfft_slab_z", "psfft_slab_c2r_yx",
@@ -77,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.psfft_plan_set_box.argtypes = [vp, cd, cd, cd]
         L.psfft_fft3d_r2c.argtypes = [vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r.argtypes = [vp, vp, vp, vp, vp]
+        L.psfft_fft3d_c2r_static.argtypes = [vp, vp, vp, vp]
         L.psfft_hd_rhs.argtypes = [vp, vp, vp, cd, vp, vp]
         L.psfft_mhd_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, vp, vp]
         L.psfft_boussinesq_rhs.argtypes = [vp, vp, vp, vp, vp, cd, cd, cd, vp, vp]
@@ -178,6 +179,17 @@ def fft3d_r2c(plan: int, d_real, d_spec, d_work=None, stream=None) -> None:
 
 def fft3d_c2r(plan: int, d_spec, d_real, d_work, stream=None) -> None:
     _check(lib().psfft_fft3d_c2r(plan, _ptr(d_spec), _ptr(d_real), _ptr(d_work), _stream(stream)), "psfft_fft3d_c2r")
+
+
+STATIC_SCRATCH_BYTES = 32 << 20      # PSFFT_STATIC_SCRATCH_BYTES
+E_SCRATCH = -9                       # PSFFT_E_SCRATCH
+
+
+def fft3d_c2r_static(plan: int, d_spec, d_real, stream=None) -> None:
+    """``psfft_fft3d_c2r`` without a caller workspace, for callers that cannot allocate device memory: the
+    workspace is a 32 MiB array inside libpsfft.so (one per GPU, shared by all calls -- calls that overlap on the
+    GPU race; plans with work_bytes_fft above the limit are refused with code -9).  See include/psfft.h."""
+    _check(lib().psfft_fft3d_c2r_static(plan, _ptr(d_spec), _ptr(d_real), _stream(stream)), "psfft_fft3d_c2r_static")
 
 
 def hd_rhs(plan: int, d_uhat, d_rhs, nu: float, d_work, stream=None) -> None:
@@ -383,6 +395,17 @@ class Plan:
         if out is None:
             out = torch.empty((self.batch, self.Nz, self.Ny, self.N), dtype=self.rdtype, device=self.device)
         fft3d_c2r(self.handle, spec, out, self.ensure_work("fft"))
+        return out
+
+    @_on_plan_device
+    def c2r_static(self, spec: torch.Tensor, out: torch.Tensor) -> torch.Tensor:
+        """``c2r`` through ``psfft_fft3d_c2r_static``: the library's built-in 32 MiB workspace instead of this
+        plan's.  ``out`` is required -- this method exists for callers that must not allocate, so it does not."""
+        assert spec.is_cuda and spec.dtype == self.cdtype and spec.is_contiguous()
+        assert spec.numel() == self.batch * self.layout.spec_elems
+        assert out.is_cuda and out.dtype == self.rdtype and out.is_contiguous()
+        assert out.numel() == self.batch * self.layout.real_elems
+        fft3d_c2r_static(self.handle, spec, out)
         return out
 
     @_on_plan_device

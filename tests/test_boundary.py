@@ -57,7 +57,7 @@ def test_error_codes(lib):
     assert lib.psfft_fft3d_r2c(None, None, None, None, None) == -6
     assert lib.psfft_plan_query(1024, psfft.F64, 64, ctypes.byref(lay)) == -7   # batch * Nz > 65535 (y-pass grid)
     assert lib.psfft_plan_query(1024, psfft.F64, 63, ctypes.byref(lay)) == 0
-    for code in (0, -1, -2, -3, -4, -5, -6, -7, -8):
+    for code in (0, -1, -2, -3, -4, -5, -6, -7, -8, -9):
         assert psfft.strerror(code)
     assert "overlap" in psfft.strerror(-8)
     assert "psfft" in psfft.strerror(-2)
