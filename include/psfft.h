@@ -100,7 +100,7 @@ int psfft_plan_create(psfft_plan *plan, int N, int dtype, int batch, void *d_tab
  * each size from the supported list.  Real field [b][z][y][x] (Nx contiguous), half spectrum [b][kz][ky][kx]
  * with ldk = Nx/2 + 1; psfft_fft3d_r2c / c2r work as above (inverse scaled by 1/(Nx Ny Nz)).  layout.N is Nx.
  * Every right-hand-side and Runge-Kutta call works on such a plan (only the *_unfused cross-check variants need a
- * cubic one and return PSFFT_E_SIZE otherwise); spectra are Nx Ny Nz x Fourier coefficient, and
+ * cubic one in the default 2 pi box and return PSFFT_E_SIZE otherwise); spectra are Nx Ny Nz x Fourier coefficient, and
  *   the 2/3 rule is the ellipsoidal truncation in index space, keep iff sum_i (n_i / N_i)^2 < 1/9, evaluated in
  *   integers as 9 sum_i (n_i L / N_i)^2 < L^2 with L = lcm(Nx, Ny, Nz) -- for a cube this is 9 |n|^2 < N^2;
  *   n_i = the integer index p (p < N_i / 2) or p - N_i. */
@@ -252,7 +252,8 @@ int psfft_rk_step(psfft_plan plan, int system, const void *d_y_in, void *d_y_out
  * forward transforms, mask + projection kernel.  Nothing is fused or pruned: every pass touches
  * the dense fields.  Same arguments, same results up to rounding; kept as the second CUDA path that
  * the full-size tests cross-check the fused one against, and as the "before" of DESIGN.md's
- * traffic comparison. */
+ * traffic comparison.  Their kernels use integer wavenumbers on a cube: a plan with Nx != Ny or Ny != Nz, or whose
+ * box psfft_plan_set_box changed to anything but (2 pi, 2 pi, 2 pi), gets PSFFT_E_SIZE. */
 int psfft_hd_rhs_unfused(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu, void *d_work,
                          void *stream);
 int psfft_mhd_rhs_unfused(psfft_plan plan, const void *d_uhat, const void *d_bhat, void *d_rhs_u,

@@ -58,8 +58,16 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
     extra = ["-Xptxas", "-v"] if verbose else []
     extra += list(extra_flags)
 
+    # an object is reused when it was built with the same flags and is newer than everything its unit includes:
+    # its own .cu, every .cuh, and (the boundary unit only) include/psfft.h
+    same_flags = not force and os.path.exists(_stamp()) and open(_stamp()).read() == _flags(extra_flags)
+    headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")]
+
     def compile_one(src: str) -> str:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        deps = [os.path.join(CSRC, src), *headers] + ([os.path.join(INCLUDE, "psfft.h")] if src == "psfft_api.cu" else [])
+        if same_flags and not verbose and os.path.exists(obj) and all(os.path.getmtime(d) < os.path.getmtime(obj) for d in deps):
+            return obj
         cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:

@@ -161,6 +161,8 @@ int fill_layout(int N, int Ny, int Nz, int dtype, int batch, psfft_layout *o)
 }
 
 inline bool cubic(const psfft_layout &l) { return l.Ny == l.N && l.Nz == l.N; }
+// cubic grid in the default 2 pi box (every 2 pi / L_i exactly 1): what the *_unfused kernels assume
+inline bool unit_cube(const Plan *pl) { return cubic(pl->lay) && pl->kf[0] == 1.0 && pl->kf[1] == 1.0 && pl->kf[2] == 1.0; }
 inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 // Live plans.  A handle is looked up here before it is dereferenced, so a destroyed or made-up handle is
@@ -216,7 +218,7 @@ PassArgs args_of(const Plan *pl, void *stream)
     a.kxc = kx_count(a.N);
     a.rx2 = pl->rx2; a.ry2 = pl->ry2; a.rz2 = pl->rz2; a.lim = pl->lim;
     for (int i = 0; i < 3; ++i) a.kf[i] = pl->kf[i];
-    a.unit_cube = cubic(pl->lay) && a.kf[0] == 1.0 && a.kf[1] == 1.0 && a.kf[2] == 1.0;
+    a.unit_cube = unit_cube(pl);
     return a;
 }
 
@@ -552,7 +554,8 @@ static int hd_entry(psfft_plan plan, const void *d_uhat, void *d_rhs, double nu,
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!fused && !cubic(pl->lay)) return PSFFT_E_SIZE;   // the unfused cross-check path needs Nx = Ny = Nz
+    // the unfused cross-check path works in integer wavenumbers on a cube: Nx = Ny = Nz and the default 2 pi box
+    if (!fused && !unit_cube(pl)) return PSFFT_E_SIZE;
     if (!d_uhat || !d_rhs || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_rhs) || misaligned(d_work)) return PSFFT_E_ALIGN;
     {
@@ -576,7 +579,8 @@ static int mhd_entry(psfft_plan plan, const void *d_uhat, const void *d_bhat, vo
 {
     Plan *pl = get(plan);
     if (!pl) return PSFFT_E_PLAN;
-    if (!fused && !cubic(pl->lay)) return PSFFT_E_SIZE;   // the unfused cross-check path needs Nx = Ny = Nz
+    // the unfused cross-check path works in integer wavenumbers on a cube: Nx = Ny = Nz and the default 2 pi box
+    if (!fused && !unit_cube(pl)) return PSFFT_E_SIZE;
     if (!d_uhat || !d_bhat || !d_rhs_u || !d_rhs_b || !d_work) return PSFFT_E_NULL;
     if (misaligned(d_uhat) || misaligned(d_bhat) || misaligned(d_rhs_u) || misaligned(d_rhs_b) || misaligned(d_work))
         return PSFFT_E_ALIGN;

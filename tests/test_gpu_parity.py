@@ -123,6 +123,32 @@ def test_unfused_cross_check_path_needs_a_cubic_plan():
         psfft.hd_rhs_unfused(p.handle, u, torch.empty_like(u), 0.0, p.ensure_work("hd"))
 
 
+def test_unfused_cross_check_path_needs_the_default_box():
+    """The *_unfused kernels use integer wavenumbers: after psfft_plan_set_box to another box they must refuse
+    (PSFFT_E_SIZE) instead of returning the 2 pi-box answer; setting the box back to 2 pi re-enables them."""
+    import math
+    N = 16
+    p = psfft.Plan(N, torch.float64, 1, work="mhd")
+    u = dev(synth.solenoidal_spectrum(N, 3.0, 5, 21))
+    b = dev(synth.solenoidal_spectrum(N, 3.0, 5, 22, tag=1))
+    L = psfft.lib()
+    st = torch.cuda.current_stream().cuda_stream
+    ru, rb = torch.full_like(u, 7.0), torch.full_like(b, 7.0)
+    want = torch.empty_like(u)
+    psfft.hd_rhs_unfused(p.handle, u, want, 0.1, p._work)
+    psfft.plan_set_box(p.handle, 2 * math.pi, 2 * math.pi, math.pi)
+    assert L.psfft_hd_rhs_unfused(p.handle, u.data_ptr(), ru.data_ptr(), 0.1, p._work.data_ptr(), st) == -2
+    assert L.psfft_mhd_rhs_unfused(p.handle, u.data_ptr(), b.data_ptr(), ru.data_ptr(), rb.data_ptr(), 0.1, 0.1,
+                                   p._work.data_ptr(), st) == -2
+    torch.cuda.synchronize()
+    assert bool((ru == 7.0).all()) and bool((rb == 7.0).all())            # nothing was enqueued
+    fused_box = p.hd_rhs(u, 0.1)                                            # the fused call does take the box
+    assert not torch.equal(fused_box, want)
+    psfft.plan_set_box(p.handle, 2 * math.pi, 2 * math.pi, 2 * math.pi)
+    psfft.hd_rhs_unfused(p.handle, u, ru, 0.1, p._work)
+    assert torch.equal(ru, want)
+
+
 def test_degenerate_inputs():
     N = 16
     p = psfft.Plan(N, torch.float64, 1)
