@@ -289,7 +289,11 @@ int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double n
  * same butterfly order per column).  Inverse: psfft_slab_z(dir = +1) on the x-slab, exchange (direct: nothing to do;
  * packed: all-to-all of the contiguous z-ranges [p Mz, (p+1) Mz) of the x-slabs), then psfft_slab_c2r_yx, whose y-pass
  * loads its columns from the blocks.
- * Returns PSFFT_E_SIZE unless 1 <= P <= PSFFT_MAX_RANKS, P divides Nz, P <= ldk, 0 <= rank < P. */
+ * Returns PSFFT_E_SIZE unless 1 <= P <= PSFFT_MAX_RANKS, P divides Nz, P <= ldk, 0 <= rank < P, and (phase calls)
+ * 0 <= zoff and zoff + Mz <= Nz: a block is at most an x-slab of Nz planes, and in direct mode it is another rank's
+ * memory, so a plane range past its end is refused rather than stored.  The overlap check of these calls covers the
+ * planes [zoff, zoff + Mz) of every block as well: the blocks must be disjoint from one another (r2c_xy writes them) and
+ * from d_zspec / d_real_slab (PSFFT_E_OVERLAP otherwise). */
 #define PSFFT_MAX_RANKS 16
 typedef struct psfft_slab_layout {
     int P, rank;

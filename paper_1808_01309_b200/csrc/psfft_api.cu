@@ -186,12 +186,12 @@ struct Span {
     size_t n;
     bool written;
 };
-bool spans_overlap(std::initializer_list<Span> spans)
+bool spans_overlap(const Span *first, const Span *last)
 {
-    for (const Span *a = spans.begin(); a != spans.end(); ++a) {
+    for (const Span *a = first; a != last; ++a) {
         if (!a->p || !a->n) continue;
         const uintptr_t a0 = reinterpret_cast<uintptr_t>(a->p), a1 = a0 + a->n;
-        for (const Span *b = a + 1; b != spans.end(); ++b) {
+        for (const Span *b = a + 1; b != last; ++b) {
             if (!b->p || !b->n || !(a->written || b->written)) continue;
             const uintptr_t b0 = reinterpret_cast<uintptr_t>(b->p), b1 = b0 + b->n;
             if (a0 < b1 && b0 < a1) return true;
@@ -199,6 +199,7 @@ bool spans_overlap(std::initializer_list<Span> spans)
     }
     return false;
 }
+bool spans_overlap(std::initializer_list<Span> spans) { return spans_overlap(spans.begin(), spans.end()); }
 
 PassArgs args_of(const Plan *pl, void *stream)
 {
@@ -797,7 +798,9 @@ static int slab_ranges(const Plan *pl, int P, int rank, psfft_slab_layout *o)
 
 static int slab_xdist(const Plan *pl, const psfft_slab_layout &sl, void *const *blocks, long zoff, XDistArgs *xd)
 {
-    if (zoff < 0) return PSFFT_E_SIZE;
+    // the planes [zoff, zoff + Mz) of every block must exist: a block has at most Nz planes (direct mode: it is the
+    // x-slab of its rank, which may be peer memory -- a store past its end would land in someone else's data)
+    if (zoff < 0 || zoff + sl.Mz > pl->lay.Nz) return PSFFT_E_SIZE;
     memset(xd, 0, sizeof(*xd));
     for (int q = 0; q < sl.P; ++q) {
         if (!blocks[q]) return PSFFT_E_NULL;
@@ -809,6 +812,20 @@ static int slab_xdist(const Plan *pl, const psfft_slab_layout &sl, void *const *
     xd->P = sl.P;
     xd->zoff = zoff;
     return PSFFT_OK;
+}
+
+// Byte ranges a phase-1 / phase-2 call touches: the planes [zoff, zoff + Mz) of every block (written by r2c_xy, only
+// read by c2r_yx) next to the call's other buffers.
+static bool slab_spans_overlap(const Plan *pl, const psfft_slab_layout &sl, void *const *blocks, long zoff, bool blocks_written,
+                               std::initializer_list<Span> others)
+{
+    const size_t cs = pl->lay.dtype == PSFFT_F64 ? 16 : 8;
+    std::vector<Span> v(others);
+    for (int q = 0; q < sl.P; ++q) {
+        const size_t plane = (size_t)pl->lay.Ny * (size_t)(sl.x0[q + 1] - sl.x0[q]) * cs;
+        v.push_back({static_cast<const char *>(blocks[q]) + (size_t)zoff * plane, (size_t)sl.Mz * plane, blocks_written});
+    }
+    return spans_overlap(v.data(), v.data() + v.size());
 }
 
 int psfft_slab_query(psfft_plan plan, int P, int rank, psfft_slab_layout *out)
@@ -832,7 +849,8 @@ int psfft_slab_r2c_xy(psfft_plan plan, int P, int rank, const void *d_real_slab,
     XDistArgs xd;
     rc = slab_xdist(pl, sl, d_blocks, zoff, &xd);
     if (rc) return rc;
-    if (spans_overlap({{d_real_slab, sl.real_bytes, false}, {d_zspec, sl.zspec_bytes, true}})) return PSFFT_E_OVERLAP;
+    if (slab_spans_overlap(pl, sl, d_blocks, zoff, true, {{d_real_slab, sl.real_bytes, false}, {d_zspec, sl.zspec_bytes, true}}))
+        return PSFFT_E_OVERLAP;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     const long nrows = (long)sl.Mz * a.Ny;
@@ -881,7 +899,8 @@ int psfft_slab_c2r_yx(psfft_plan plan, int P, int rank, void *const *d_blocks, l
     XDistArgs xd;
     rc = slab_xdist(pl, sl, d_blocks, zoff, &xd);
     if (rc) return rc;
-    if (spans_overlap({{d_zspec, sl.zspec_bytes, true}, {d_real_slab, sl.real_bytes, true}})) return PSFFT_E_OVERLAP;
+    if (slab_spans_overlap(pl, sl, d_blocks, zoff, false, {{d_zspec, sl.zspec_bytes, true}, {d_real_slab, sl.real_bytes, true}}))
+        return PSFFT_E_OVERLAP;
     pl->launches = 0;
     PassArgs a = args_of(pl, stream);
     const long nrows = (long)sl.Mz * a.Ny;

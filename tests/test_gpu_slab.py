@@ -92,7 +92,19 @@ def test_slab_argument_checks_and_guard_bands():
     bad = (ctypes.c_void_p * P)(blocks[0].data_ptr(), None, blocks[2].data_ptr(), blocks[3].data_ptr())
     assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), bad, 0, st) == -1
     assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), arr, -1, st) == -2          # zoff < 0
+    # planes past the end of a block (here zoff + Mz = 13 + 4 > Nz = 16) would be stores into a peer's memory: refused
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), arr, Nz - lay.Mz + 1, st) == -2
+    assert L.psfft_slab_c2r_yx(plan.handle, P, 1, arr, Nz - lay.Mz + 1, zs.data_ptr(), real.data_ptr(), st) == -2
+    assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), arr, Nz - lay.Mz, st) == 0  # last planes: fine
     assert L.psfft_slab_z(plan.handle, P, 1, 0, blocks[1].data_ptr(), st) == -2                               # dir
+    # the blocks are part of the overlap check: a block on the work buffer, on the input, or two blocks on one another
+    for alias in (zs.data_ptr(), real.data_ptr(), blocks[0].data_ptr()):
+        arr2 = (ctypes.c_void_p * P)(blocks[0].data_ptr(), blocks[1].data_ptr(), alias, blocks[3].data_ptr())
+        assert L.psfft_slab_r2c_xy(plan.handle, P, 1, real.data_ptr(), zs.data_ptr(), arr2, 0, st) == -8
+    arr2 = (ctypes.c_void_p * P)(blocks[0].data_ptr(), blocks[1].data_ptr(), zs.data_ptr(), blocks[3].data_ptr())
+    assert L.psfft_slab_c2r_yx(plan.handle, P, 1, arr2, 0, zs.data_ptr(), real.data_ptr(), st) == -8          # reads what it writes
+    arr2 = (ctypes.c_void_p * P)(blocks[0].data_ptr(), blocks[0].data_ptr(), blocks[2].data_ptr(), blocks[3].data_ptr())
+    assert L.psfft_slab_c2r_yx(plan.handle, P, 1, arr2, 0, zs.data_ptr(), real.data_ptr(), st) == 0           # read-only blocks may alias
     assert L.psfft_slab_r2c_xy(plan.handle, P, 1, zs.data_ptr(), zs.data_ptr(), arr, 0, st) == -8             # overlap
     # guard bands: arena = [guard | zspec | guard | block 0 | guard | ... ]
     G = 512
