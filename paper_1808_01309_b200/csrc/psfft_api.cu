@@ -457,6 +457,9 @@ int psfft_plan_create3(psfft_plan *plan, int N, int Ny, int Nz, int dtype, int b
         auto gcd = [](long x, long y) { while (y) { const long t = x % y; x = y; y = t; } return x; };
         long L = (long)N / gcd(N, Ny) * Ny;
         L = L / gcd(L, Nz) * Nz;
+        // int32 headroom of GeomAny::w2 / keep3 (psfft_rhs.cuh): sum_i (r_i n_i)^2 <= 3 (L/2)^2 with |n_i| <= N_i / 2.
+        // The supported sizes give L <= lcm(2048, 768) = 6144, i.e. 2.8e7; a future size list must not break this.
+        if (3 * (L / 2) * (L / 2) > 0x7fffffffL) { delete pl; return PSFFT_E_SIZE; }
         const long rx = L / N, ry = L / Ny, rz = L / Nz;
         pl->rx2 = (int)(rx * rx); pl->ry2 = (int)(ry * ry); pl->rz2 = (int)(rz * rz);
         pl->lim = (int)((L * L + 8) / 9);

@@ -40,6 +40,17 @@ def test_plan_query_sizes(lib):
     assert lay.work_bytes_mhd + 12 * lay.spec_bytes < 180e9                    # config 5 fits one B200
 
 
+def test_mask_integers_fit_int32_for_every_supported_grid(lib):
+    """DESIGN.md reading G25: the 2/3-rule test 9 sum (n_i L / N_i)^2 < L^2, L = lcm(Nx, Ny, Nz), is evaluated in int32 on
+    the device.  For every triple of supported sizes the largest sum, 3 (L/2)^2, must stay below 2^31."""
+    import math
+    lay = psfft.Layout()
+    sizes = [n for n in range(1, 4097) if lib.psfft_plan_query(n, psfft.F32, 1, ctypes.byref(lay)) == 0]
+    assert sizes == [8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 2048]
+    worst = max(math.lcm(a, b, c) for a in sizes for b in sizes for c in sizes)
+    assert worst == 6144 and 3 * (worst // 2) ** 2 < 2 ** 31 and (worst * worst + 8) // 9 < 2 ** 31
+
+
 def test_error_codes(lib):
     lay = psfft.Layout()
     assert lib.psfft_plan_query(500, psfft.F64, 1, ctypes.byref(lay)) == -2     # unsupported N
