@@ -527,11 +527,32 @@ def slab_rows(torch, psfft, dev, stream, K, timed) -> dict:
     return res
 
 
+def dist_all_ok(ok: bool, device="cpu") -> bool:
+    """True iff EVERY rank says ok (all_reduce MIN of a flag).  Every rank must call it, whether its own set-up worked or
+    not: it is how the ranks agree to skip a collective path before any of them has entered it."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return bool(ok)
+    t = torch.tensor([1 if ok else 0], dtype=torch.int32, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    return bool(int(t.item()))
+
+
+SLAB_WATCHDOG_S = 180   # seconds the N > 1 slab rows may take before the headline is printed without them
+SLAB_RT_TOL = 1e-12     # max |c2r(r2c(x)) - x| of the slab transform on uniform [-1, 1) input (fp64; measured ~4e-16)
+
+
 def slab_multi(torch, psfft, dev, stream, K: int, N: int = 512) -> dict:
     """N > 1 ranks only: the slab-decomposed N^3 fp64 transform ACROSS the ranks (slab.SlabFFT: y-pass scattering
     into a send buffer, one NCCL all_to_all_single, z-pass of the x-slab), timed like everything else
-    (barrier, CUDA events, max over ranks).  Never allowed to take the headline down: any failure is reported as text."""
+    (barrier, CUDA events, max over ranks).  Never allowed to take the headline down: the ranks agree (dist_all_ok) that
+    every one of them has its plan and buffers before any of them enters the all-to-all -- a rank that failed to set up
+    would otherwise leave the others blocked in it -- and run_ours runs this under a watchdog that prints the headline
+    without these rows if they do not come back."""
     import torch.distributed as dist
+    plan = sf = x = None
+    failed = None
     try:
         from paper_1808_01309_b200 import slab
         world, rank = dist.get_world_size(), dist.get_rank()
@@ -539,6 +560,13 @@ def slab_multi(torch, psfft, dev, stream, K: int, N: int = 512) -> dict:
         sf = slab.SlabFFT(plan)
         g = torch.Generator(device=dev).manual_seed(1234 + rank)
         x = torch.rand((sf.lay.Mz, N, N), dtype=torch.float64, device=dev, generator=g) * 2 - 1
+    except Exception as exc:     # out of memory, plan refused, ...: decided together below
+        failed = f"{type(exc).__name__}: {str(exc)[:200]}"
+    if not dist_all_ok(failed is None, dev):
+        if plan is not None:
+            plan.close()
+        return {"failed": failed or "skipped on every rank: another rank could not set up its plan or buffers"}
+    try:
         X = sf.r2c(x)
         back = sf.c2r(X.clone())
         err = float((back - x).abs().max())
@@ -559,9 +587,11 @@ def slab_multi(torch, psfft, dev, stream, K: int, N: int = 512) -> dict:
         res = {"workload": f"{N}^3 fp64, one field, slab-decomposed over {world} ranks (packed mode, NCCL all_to_all_single)",
                "ms_r2c": t_f, "ms_c2r": t_b, "roundtrip_max_abs_err": err, "bytes_sent_per_rank_per_transform": sent,
                "exchange_GBps_per_rank_if_all_of_r2c_were_exchange": sent / (t_f * 1e-3) / 1e9}
+        if not err <= SLAB_RT_TOL:               # also catches NaN
+            res["failed"] = f"round trip c2r(r2c(x)) differs from x by {err:.3e} (> {SLAB_RT_TOL:g}) on rank {rank}"
         plan.close()
         return res
-    except Exception as exc:     # the headline must survive an environment this path has never run on
+    except Exception as exc:     # reported as text; the headline line carries it under slab_multi_failed
         return {"failed": f"{type(exc).__name__}: {str(exc)[:200]}"}
 
 
@@ -594,18 +624,48 @@ def run_ours(args) -> int:
     if world == 1 and not args.no_configs:
         configs = other_configs(torch, psfft, synth, dev, stream, peak, K)
 
-    slab_mg = slab_multi(torch, psfft, dev, stream, K, N) if world > 1 else None
-    if rank != 0:
-        return 0
     line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": m["ms_max"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(N, world), "clocks": m["clk"], "e2e": m["e2e"],
             "gpu_launches": m["launches_per_step"] * K, "launches_per_step": m["launches_per_step"],
-            "roofline": m["roofline"], "fft3d": m["fft3d"], "next_rows": m["next_rows"], "configs": configs, "slab_multi_gpu": slab_mg}
+            "roofline": m["roofline"], "fft3d": m["fft3d"], "next_rows": m["next_rows"], "configs": configs}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(N)
-    print(json.dumps(line), flush=True)
+    if world > 1:
+        print_line_with_guarded_rows(line, rank, lambda: slab_multi(torch, psfft, dev, stream, K, N), SLAB_WATCHDOG_S)
+    elif rank == 0:
+        print(json.dumps(line), flush=True)
     return 0
+
+
+def print_line_with_guarded_rows(line: dict, rank: int, rows_fn, timeout_s: float) -> None:
+    """Print the (already complete) headline line with the N > 1 slab rows added -- or, if rows_fn does not come back
+    within timeout_s, without them.  The slab-decomposed transform across the ranks has never met real multi-GPU
+    hardware; a collective that hangs must not keep the headline from being printed.  On expiry every rank
+    prints-and-exits (code 0) on its own; only rank 0 prints, and always exactly one JSON line."""
+    import threading
+    lock, state = threading.Lock(), {"printed": False}
+
+    def emit(rows):
+        with lock:
+            if state["printed"]:
+                return
+            state["printed"] = True
+            line["slab_multi_gpu"] = rows
+            line["slab_multi_failed"] = rows.get("failed")     # top-level scalar: null = ran and round-tripped
+            if rank == 0:
+                print(json.dumps(line), flush=True)
+
+    def expired():
+        emit({"failed": f"no result after {timeout_s:g} s (a rank is stuck in the exchange); headline unaffected"})
+        os._exit(0)
+
+    dog = threading.Timer(timeout_s, expired)
+    dog.daemon = True
+    dog.start()
+    rows = rows_fn()
+    dog.cancel()
+    emit(rows)
 
 
 def metric_parts(torch, psfft, synth, N, K, W, rank, local, world, dev, stream, peak, peak_src) -> dict:

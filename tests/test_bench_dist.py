@@ -38,6 +38,38 @@ def test_two_rank_gloo_max_and_aggregate(tmp_path):
     assert abs(line["value"] - 2 * 1.0 / 15e-3) < 1e-9
 
 
+AGREE = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import bench
+rank, world = bench.dist_init("gloo")
+a = bench.dist_all_ok(True)                       # every rank fine
+b = bench.dist_all_ok(rank != 1)                  # rank 1 failed its set-up: EVERY rank must learn it and skip
+c = bench.dist_all_ok(rank == 1)                  # rank 0 failed
+bench.dist_barrier()                              # nobody is left behind in a collective
+print(json.dumps({"rank": rank, "a": a, "b": b, "c": c}))
+""" % ROOT
+
+
+def test_ranks_agree_to_skip_a_collective_path_when_one_failed_its_setup(tmp_path):
+    """bench.slab_multi enters its all-to-all only if dist_all_ok says every rank has its plan and buffers."""
+    script = tmp_path / "agree.py"
+    script.write_text(AGREE)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29537", WORLD_SIZE="2")
+    procs = []
+    for r in range(2):
+        e = dict(env, RANK=str(r), LOCAL_RANK=str(r))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=e, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=240) for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    for r, (out, _) in enumerate(outs):
+        got = json.loads(out.strip().splitlines()[-1])
+        assert got == {"rank": r, "a": True, "b": False, "c": False}
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.dist_all_ok(True) is True and bench.dist_all_ok(False) is False      # no process group: own flag
+
+
 def test_reference_arm_non_zero_ranks_exit_without_work():
     env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
@@ -50,3 +82,29 @@ def test_work_ratio():
     import bench
     assert abs(bench.work_ratio(512, 256) - 9.0) < 1e-12
     assert bench.aggregate(20.0, 1.0, 1) == 50.0
+
+
+def test_headline_line_survives_slab_rows_that_hang_or_fail(tmp_path):
+    """bench.print_line_with_guarded_rows: the N > 1 slab rows are added to the one JSON line when they come back, and
+    the line is printed without them (exit code 0, `slab_multi_failed` set) when they never do."""
+    sys.path.insert(0, ROOT)
+    import io
+    from contextlib import redirect_stdout
+    import bench
+    buf = io.StringIO()
+    with redirect_stdout(buf):
+        bench.print_line_with_guarded_rows({"value": 1.0}, 0, lambda: {"ms_r2c": 2.0}, 30.0)
+        bench.print_line_with_guarded_rows({"value": 1.0}, 1, lambda: {"ms_r2c": 2.0}, 30.0)      # rank 1 prints nothing
+        bench.print_line_with_guarded_rows({"value": 1.0}, 0, lambda: {"failed": "RuntimeError: x"}, 30.0)
+    lines = [json.loads(l) for l in buf.getvalue().strip().splitlines()]
+    assert lines == [{"value": 1.0, "slab_multi_gpu": {"ms_r2c": 2.0}, "slab_multi_failed": None},
+                     {"value": 1.0, "slab_multi_gpu": {"failed": "RuntimeError: x"}, "slab_multi_failed": "RuntimeError: x"}]
+    hang = tmp_path / "hang.py"
+    hang.write_text("import sys, time\nsys.path.insert(0, %r)\nimport bench\n"
+                    "bench.print_line_with_guarded_rows({'value': 1.0}, 0, lambda: time.sleep(600), 1.0)\n" % ROOT)
+    r = subprocess.run([sys.executable, str(hang)], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0
+    out = r.stdout.strip().splitlines()
+    assert len(out) == 1
+    got = json.loads(out[0])
+    assert got["value"] == 1.0 and "no result after 1 s" in got["slab_multi_failed"]
