@@ -48,13 +48,20 @@ def test_order_one_is_forward_euler():
     assert np.all(got[:, ~M] == 0)
 
 
-@pytest.mark.parametrize("sys", [0, 1, 2])
+@pytest.mark.parametrize("sys", [0, 1, 2, 3])
 @pytest.mark.parametrize("ord", [2, 3, 4])
 def test_stage_loop_restated_in_numpy(sys, ord):
-    """The stage loop written out with the (separately pinned) right-hand sides."""
+    """The stage loop written out with the (separately pinned) right-hand sides.  sys = 3 (Gross-Pitaevskii,
+    PAPER.md:54-56 Eq. 7) runs with alpha and beta both non-zero and different, and with a third parameter that must
+    be ignored, so rk_rhs cannot take beta from the wrong slot of `par` (the only other CPU pin of that
+    branch has beta = 0)."""
     N, dt, nu, c2, nbv = 12, 0.02, 0.11, 0.07, 1.3
     u = synth.solenoidal_spectrum(N, 2.0, 5, 5, tag=0)
-    if sys == 0:
+    if sys == 3:
+        y = 0.5 * u[:2]                                      # (p^, q^) of psi = p + i q: any two real fields
+        rhs = lambda y: oracle.gpe_rhs(y, nu, c2)            # alpha = 0.11, beta = 0.07
+        assert rel(oracle.gpe_rhs(y, nu, c2), oracle.gpe_rhs(y, nu, nbv)) > 1e-3     # beta matters on this input
+    elif sys == 0:
         y = u
         rhs = lambda y: oracle.hd_rhs(y, nu)
     elif sys == 1:
