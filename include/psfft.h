@@ -232,11 +232,13 @@ int psfft_gpe_rhs(psfft_plan plan, const void *d_psihat, void *d_rhs, double alp
  *     y^(ord) = y_n;   y^(o-1) = M y_n + (dt / o) R(y^(o)),  o = ord, ..., 1;   y_{n+1} = y^(0) ).
  * Each stage is one fused right-hand-side evaluation whose last pass writes M y_n + (dt/o) R instead of
  * R (one more sparse read of y_n in its epilogue); there is no separate update kernel.
- *   system    PSFFT_SYS_HD (y = u^: 3 fields), PSFFT_SYS_MHD (u^, b^: 6), PSFFT_SYS_BOUSSINESQ (u^, theta^: 4)
+ *   system    PSFFT_SYS_HD (y = u^: 3 fields), PSFFT_SYS_MHD (u^, b^: 6), PSFFT_SYS_BOUSSINESQ (u^, theta^: 4),
+ *             PSFFT_SYS_GPE (p^, q^ of psi = p + i q: 2 fields; R = psfft_gpe_rhs)
  *   d_y_in    in   the state y_n, fields contiguous in the order above (not modified)
  *   d_y_out   out  y_{n+1} (dealiased); must not overlap d_y_in
  *   ord       1..4 stages
- *   params    HOST pointer to 3 doubles: { nu, eta (MHD) or kappa (Boussinesq), N_bv }
+ *   params    HOST pointer to 3 doubles: { nu, eta (MHD) or kappa (Boussinesq), N_bv };
+ *             for PSFFT_SYS_GPE { alpha, beta, ignored }
  *   d_work         >= psfft_rk_work_bytes(plan, system) = one state-sized stage buffer + the RHS workspace
  * Returns PSFFT_E_SIZE for a bad system / ord, PSFFT_E_OVERLAP when d_y_in, d_y_out, d_work overlap. */
 #define PSFFT_SYS_HD 0
