@@ -306,7 +306,16 @@ def roofline_of(recs, K: int, ms_step: float, dense_bytes: float, dense_model: s
     achieved = tot[dom][1] / (tot[dom][0] * 1e-3) / 1e9
     moved = sum(v[1] for v in tot.values()) / K
     traffic, traffic_src = ncu_traffic(dom, workload)
-    return {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+    # scalar copies of the nested figures below (a record that keeps only the scalar members of this object still
+    # carries the whole-step fractions and every kernel's own fraction): frac_<kernel> = its algorithmic bytes / its
+    # time / peak, ms_<kernel> = its time per step
+    flat = {"step_bytes_moved_frac": moved / (ms_step * 1e-3) / 1e9 / peak,
+            "step_dense_equiv_frac": dense_bytes / (ms_step * 1e-3) / 1e9 / peak}
+    for k, v in tot.items():
+        short = k[4:] if k.startswith("rhs_") else k
+        flat["frac_" + short] = v[1] / (v[0] * 1e-3) / 1e9 / peak
+        flat["ms_" + short] = v[0] / K
+    return {**flat, "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
             "launches_timed": tot[dom][2], "avg_launch_ms": tot[dom][0] / tot[dom][2],
             "algorithmic_bytes_per_launch": tot[dom][1] / tot[dom][2],
@@ -789,6 +798,11 @@ def metric_parts(torch, psfft, synth, N, K, W, rank, local, world, dev, stream, 
                                  "workload": f"{N}^3 fp64, psi = p + i q as two real fields, alpha = 0.3, beta = 1"}}
         del th, rt
 
+    if fft3d is not None:   # the metric's first clause as scalars of the roofline object, next to the kernel's
+        roofline["fft3d_ms_r2c_plus_c2r"] = fft3d["ms_r2c_plus_c2r"]
+        roofline["fft3d_hbm_frac"] = fft3d["hbm_frac"]
+        roofline["fft3d_ms_r2c"] = fft3d["ms_r2c"]
+        roofline["fft3d_ms_c2r"] = fft3d["ms_c2r"]
     return {"value": value, "ms_max": ms_max, "clk": clk, "e2e": e2e, "launches_per_step": launches_per_step,
             "roofline": roofline, "fft3d": fft3d, "next_rows": next_rows}
 
