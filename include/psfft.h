@@ -272,6 +272,23 @@ int psfft_fft3d_c2r_host(psfft_plan plan, const void *h_spec, void *h_real, void
 int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in,
                       void *d_out, void *d_work, void *stream);
 
+/* psfft_hd_rhs_host that moves only what the method defines (the cost of the
+ * host <-> device transfers is the paper's own concern).  The right-hand side reads its input through the 2/3-rule
+ * mask and its output is exactly zero outside the mask, so of each dense spectral field only the index box around the
+ * retained ellipsoid,
+ *     kx in [0, ceil(Nx/3)),   |ky| < Ny/3,   |kz| < Nz/3        (about 30 % of the field),
+ * has to cross the bus.  Same arguments and same dense layouts as psfft_hd_rhs_host on both sides; per field and
+ * direction the box goes as four cudaMemcpy3DAsync copies (the ky, kz index ranges [0, b] and [N - b, N)), all on
+ * `stream`, which is synchronised before the call returns.  psfft_host_box_bytes = bytes per field and direction.
+ *   h_uhat  in   3 dense spectral fields; only the box is read
+ *   h_rhs   out  3 dense spectral fields; ONLY THE BOX IS WRITTEN.  Everything outside it is an exact zero of the
+ *                result and is never touched: zero the array once before its first use (not once per call)
+ *   d_in, d_out  device staging of 3 spectral fields each; need no initialisation (what lies outside the mask is
+ *                never loaded by the kernels) */
+size_t psfft_host_box_bytes(psfft_plan plan);
+int psfft_hd_rhs_host_box(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in,
+                          void *d_out, void *d_work, void *stream);
+
 /* ---- Slab-decomposed transform over P GPUs (Sec. 2, Fig. 1) ------------------------------------
  * The paper's decomposition: task p of P owns the z-slab of Mz = Nz / P planes.  Forward: (1) local 2D transform
  * (x, y) of the slab, (2) global transpose -- the all-to-all, "the only communication involved" -- (3)

@@ -777,6 +777,68 @@ int psfft_hd_rhs_host(psfft_plan plan, const void *h_uhat, void *h_rhs, double n
     return PSFFT_OK;
 }
 
+// ---- host entry point that moves only the retained box (psfft_hd_rhs_host_box) -----------------------------------
+// Index box around the 2/3-rule ellipsoid: kx in [0, bx), |ky| <= by, |kz| <= bz, from the plan's integer form of the
+// rule (rx2 n^2 < lim on each axis with the other two indices 0).  A superset of the retained modes, and exact on the
+// axes, so nothing the right-hand side reads or writes as non-zero lies outside it.
+struct KeepBox { int bx, by, bz; };
+static KeepBox keep_box(const Plan *pl)
+{
+    auto last = [&](int r2) { long n = 0; while ((long)r2 * (n + 1) * (n + 1) < (long)pl->lim) ++n; return (int)n; };
+    return {last(pl->rx2) + 1, last(pl->ry2), last(pl->rz2)};
+}
+
+// The box of `fields` spectral fields [kz][ky][kx] between two dense arrays of the caller layout (same layout on both
+// sides): per field four 3D copies, one per (ky, kz) index-range quadrant -- indices [0, b] and [N - b, N).
+static int copy_box(const Plan *pl, void *dst, const void *src, int fields, cudaMemcpyKind kind, cudaStream_t st)
+{
+    const size_t cs = pl->lay.dtype == PSFFT_F64 ? 16 : 8, pitch = (size_t)pl->lay.ldk * cs;
+    const KeepBox b = keep_box(pl);
+    const int Ny = pl->lay.Ny, Nz = pl->lay.Nz;
+    for (int f = 0; f < fields; ++f)
+        for (int zq = 0; zq < 2; ++zq)
+            for (int yq = 0; yq < 2; ++yq) {
+                const int z0 = zq ? Nz - b.bz : 0, nz = zq ? b.bz : b.bz + 1;
+                const int y0 = yq ? Ny - b.by : 0, ny = yq ? b.by : b.by + 1;
+                if (nz <= 0 || ny <= 0) continue;
+                cudaMemcpy3DParms p;
+                memset(&p, 0, sizeof(p));
+                p.srcPtr = make_cudaPitchedPtr(const_cast<char *>(off(src, (size_t)f * pl->lay.spec_bytes)), pitch, pitch, (size_t)Ny);
+                p.dstPtr = make_cudaPitchedPtr(off(dst, (size_t)f * pl->lay.spec_bytes), pitch, pitch, (size_t)Ny);
+                p.srcPos = make_cudaPos(0, (size_t)y0, (size_t)z0);
+                p.dstPos = p.srcPos;
+                p.extent = make_cudaExtent((size_t)b.bx * cs, (size_t)ny, (size_t)nz);
+                p.kind = kind;
+                CU(cudaMemcpy3DAsync(&p, st));
+            }
+    return PSFFT_OK;
+}
+
+size_t psfft_host_box_bytes(psfft_plan plan)
+{
+    Plan *pl = get(plan);
+    if (!pl) return 0;
+    const KeepBox b = keep_box(pl);
+    return (size_t)b.bx * (size_t)(2 * b.by + 1) * (size_t)(2 * b.bz + 1) * (pl->lay.dtype == PSFFT_F64 ? 16 : 8);
+}
+
+int psfft_hd_rhs_host_box(psfft_plan plan, const void *h_uhat, void *h_rhs, double nu, void *d_in, void *d_out,
+                          void *d_work, void *stream)
+{
+    Plan *pl = get(plan);
+    if (!pl) return PSFFT_E_PLAN;
+    if (!h_uhat || !h_rhs || !d_in || !d_out) return PSFFT_E_NULL;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    int rc = copy_box(pl, d_in, h_uhat, 3, cudaMemcpyHostToDevice, st);
+    if (rc) return rc;
+    rc = psfft_hd_rhs(plan, d_in, d_out, nu, d_work, stream);
+    if (rc) return rc;
+    rc = copy_box(pl, h_rhs, d_out, 3, cudaMemcpyDeviceToHost, st);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(st));
+    return PSFFT_OK;
+}
+
 // ---- slab-decomposed transform (psfft_slab.cuh) --------------------------------------------------
 static int slab_ranges(const Plan *pl, int P, int rank, psfft_slab_layout *o)
 {

@@ -24,6 +24,7 @@ EXPORTS = [
     "psfft_hd_rhs_unfused", "psfft_mhd_rhs_unfused",
     "psfft_slab_query", "psfft_slab_r2c_xy", "psfft_slab_z", "psfft_slab_c2r_yx",
     "psfft_fft3d_r2c_host", "psfft_fft3d_c2r_host", "psfft_hd_rhs_host",
+    "psfft_hd_rhs_host_box", "psfft_host_box_bytes",
     "psfft_profile_enable", "psfft_profile_reset", "psfft_profile_count", "psfft_profile_get",
     "psfft_kernel_name", "psfft_last_launch_count", "psfft_strerror", "psfft_version",
 ]
@@ -95,6 +96,9 @@ def lib() -> ctypes.CDLL:
         L.psfft_fft3d_r2c_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_fft3d_c2r_host.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.psfft_hd_rhs_host.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
+        L.psfft_hd_rhs_host_box.argtypes = [vp, vp, vp, cd, vp, vp, vp, vp]
+        L.psfft_host_box_bytes.argtypes = [vp]
+        L.psfft_host_box_bytes.restype = sz
         L.psfft_profile_enable.argtypes = [vp, ci]
         L.psfft_profile_reset.argtypes = [vp]
         L.psfft_profile_count.argtypes = [vp]
@@ -275,6 +279,18 @@ def fft3d_c2r_host(plan: int, h_spec, h_real, d_in, d_out, d_work, stream=None) 
 def hd_rhs_host(plan: int, h_uhat, h_rhs, nu: float, d_in, d_out, d_work, stream=None) -> None:
     _check(lib().psfft_hd_rhs_host(plan, _ptr(h_uhat), _ptr(h_rhs), float(nu), _ptr(d_in), _ptr(d_out), _ptr(d_work),
                                    _stream(stream)), "psfft_hd_rhs_host")
+
+
+def hd_rhs_host_box(plan: int, h_uhat, h_rhs, nu: float, d_in, d_out, d_work, stream=None) -> None:
+    """hd_rhs_host copying only the index box around the retained modes (about 30 % of the dense bytes each way).
+    h_rhs must have been zeroed once: only the box is written (include/psfft.h)."""
+    _check(lib().psfft_hd_rhs_host_box(plan, _ptr(h_uhat), _ptr(h_rhs), float(nu), _ptr(d_in), _ptr(d_out),
+                                       _ptr(d_work), _stream(stream)), "psfft_hd_rhs_host_box")
+
+
+def host_box_bytes(plan: int) -> int:
+    """Bytes per spectral field and direction that hd_rhs_host_box copies."""
+    return int(lib().psfft_host_box_bytes(plan))
 
 
 def profile_enable(plan: int, on: bool) -> None:

@@ -531,6 +531,40 @@ def test_host_entry_points():
     assert rel(hr.numpy(), oracle.hd_rhs(uh, 0.0)) < 1e-12
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("shape", [(32, 32, 32), (48, 48, 48), (48, 24, 32), (12, 8, 16)])
+def test_host_box_entry_point_moves_only_the_retained_box(shape, dtype):
+    """psfft_hd_rhs_host_box: the FULL host array equals the oracle's (the array was zeroed once; the call writes the box),
+    nothing outside the box is touched, the staging buffers need no initialisation, and the byte count is the box's."""
+    Nx, Ny, Nz = shape
+    p = psfft.Plan(shape if len(set(shape)) > 1 else Nx, dtype, 1, work="hd")
+    uh = synth.aniso_spectrum(shape, seed=11).astype(CDT[dtype])              # broadband: fills the retained ellipsoid
+    want = oracle.hd_rhs(uh.astype(np.complex128), 0.05)
+    hu = torch.from_numpy(uh).pin_memory()
+    d_in = torch.full((3 * p.layout.spec_elems,), complex(float("nan"), float("nan")), dtype=p.cdtype, device="cuda")
+    d_out = torch.full_like(d_in, complex(float("nan"), float("nan")))
+    hr = torch.zeros_like(hu).pin_memory()
+    psfft.hd_rhs_host_box(p.handle, hu, hr, 0.05, d_in, d_out, p._work)
+    got = hr.numpy()
+    assert rel(got, want) < TOL[dtype]
+    # the box: kx < ceil(Nx / 3), |ky| < Ny / 3, |kz| < Nz / 3 (index ranges [0, b] and [N - b, N))
+    bx, by, bz = (Nx - 1) // 3 + 1, (Ny - 1) // 3, (Nz - 1) // 3
+    inside = np.zeros((Nz, Ny, Nx // 2 + 1), dtype=bool)
+    zi = np.r_[0:bz + 1, Nz - bz:Nz]
+    yi = np.r_[0:by + 1, Ny - by:Ny]
+    inside[np.ix_(zi, yi, np.arange(bx))] = True
+    assert psfft.host_box_bytes(p.handle) == int(inside.sum()) * uh.itemsize
+    assert np.all(want[:, ~inside] == 0)                                       # the oracle agrees that nothing lives outside
+    hr2 = torch.full_like(hu, 7.0).pin_memory()                                 # second call into a marked array
+    psfft.hd_rhs_host_box(p.handle, hu, hr2, 0.05, d_in, d_out, p._work)
+    got2 = hr2.numpy()
+    assert np.all(got2[:, ~inside] == 7.0) and np.array_equal(got2[:, inside], got[:, inside])
+    # and it agrees bit for bit with the dense host entry point
+    hr3 = torch.empty_like(hu).pin_memory()
+    psfft.hd_rhs_host(p.handle, hu, hr3, 0.05, d_in, d_out, p._work)
+    assert np.array_equal(hr3.numpy(), got)
+
+
 # ---- the unfused composition (second CUDA path) ------------------------------------------------------
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
