@@ -3,6 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
+With --gpus N > 1 and no launcher around it (WORLD_SIZE unset) it starts its N ranks itself (launch_ranks); under
+torchrun it is one of the ranks.
+
 One STEP = one pass of the whole hot path over one batch of synthetic input: one Navier-Stokes
 right-hand-side evaluation psfft_hd_rhs at 512^3 fp64 (spectral curl, 6 inverse + 3 forward 3D
 transforms, u x w, 2/3-rule dealias, projection: rows a1-a11 of SURVEY.md §8(a)), input and output
@@ -837,9 +840,26 @@ def main() -> int:
     ap.add_argument("--reference-budget-s", type=float, default=150.0,
                     help="--impl reference: cap on the oracle time of the whole arm (full-size evaluations)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return launch_ranks(args.gpus)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
+
+
+def launch_ranks(n: int) -> int:
+    """`bench.py --gpus N` called WITHOUT a launcher (no WORLD_SIZE in the environment): start the N ranks ourselves,
+    one process per GPU (one task per GPU, bound by the program, not by the caller), by re-running this
+    very command line under torch.distributed.run on 127.0.0.1 with a free port.  Each rank then finds
+    RANK / LOCAL_RANK / WORLD_SIZE in its environment and binds to cuda:LOCAL_RANK (run_ours).  Under an external
+    launcher (the driver's torchrun line) WORLD_SIZE is set and this function is never reached."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 if __name__ == "__main__":

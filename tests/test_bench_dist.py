@@ -108,3 +108,19 @@ def test_headline_line_survives_slab_rows_that_hang_or_fail(tmp_path):
     assert len(out) == 1
     got = json.loads(out[0])
     assert got["value"] == 1.0 and "no result after 1 s" in got["slab_multi_failed"]
+
+
+def test_gpus_2_without_a_launcher_starts_two_ranks(tmp_path):
+    """`bench.py --gpus 2 --impl reference` with NO rank variables in the environment: bench.py launches its two ranks
+    itself (torch.distributed.run on 127.0.0.1); rank 0 runs the oracle arm and prints the one JSON line with n_gpus 2,
+    rank 1 starts, sees it has no work in this arm and exits 0."""
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT", "TORCHELASTIC_RUN_ID")}
+    env["TORCHELASTIC_ERROR_FILE"] = str(tmp_path / "err.json")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--N", "16",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.strip().splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # one line: rank 1 printed nothing
+    got = json.loads(lines[0])
+    assert got["impl"] == "reference" and got["n_gpus"] == 2 and got["value"] > 0
