@@ -10,6 +10,9 @@ where the x-distributed blocks live and moves them:
 * ``SlabFFT``        one rank of a ``torch.distributed`` job, *packed* mode: the y-pass stores into a send buffer laid
                      out as P contiguous slices, ONE ``all_to_all_single`` (NCCL over NVLink on GPUs) delivers the
                      x-slab -- the receive buffer [sender][Mz][Ny][w] is the x-slab [Nz][Ny][w], no unpack.
+* ``DirectSlabFFT``  one rank of a ``torch.distributed`` job on one node, *direct* mode with REAL processes: every rank's
+                     x-slab is mapped into every other rank through CUDA IPC, the y-pass stores / loads go straight
+                     to the owners, a barrier separates the phases; no NCCL needed.
 * ``exchange_forward / exchange_inverse``  the two all-to-alls with their split sizes; pure communication on torch
                      tensors of any device (the world_size-2 gloo test drives them on CPU tensors).
 
@@ -94,6 +97,67 @@ class SlabFFT:
         real = torch.empty((self.lay.Mz, p.Ny, p.N), dtype=p.rdtype, device=p.device)
         psfft.slab_c2r_yx(h, self.P, self.rank, _slice_ptrs(self.sendbuf, self.send), 0, self.zspec, real)
         return real
+
+
+class DirectSlabFFT:
+    """One rank of a ``torch.distributed`` job on ONE node, *direct* mode (psfft.h): the fused compute + exchange path.
+
+    Every rank owns its x-slab [Nz][Ny][w] and exports it to the other ranks through CUDA IPC (the handles travel as
+    pickled objects over the process group -- ``all_gather_object`` -- so the group may be gloo: this mode needs no NCCL
+    at all).  The forward y-pass of a rank then stores each finished column straight into the x-slab of the rank that
+    owns its kx -- over NVLink when that rank sits on another GPU -- so the all-to-all of PAPER.md:76 IS the store
+    pattern of the kernel and overlaps the y-pass tile by tile; the inverse y-pass loads its columns from the peers'
+    x-slabs the same way.  The only synchronisation is a barrier between the two phases (all stores have landed before
+    anyone starts the z-pass; all loads are done before anyone overwrites its x-slab again).
+
+    Buffers (x-slab, phase-1 work buffer, the real output slab) are allocated once, here.  ``plan`` is a psfft.Plan of
+    the GLOBAL grid on this rank's device.  Verified with two processes sharing the one GPU of the test box
+    (tests/test_gpu_slab.py); between different GPUs it relies on CUDA IPC peer mappings and is unmeasured."""
+
+    def __init__(self, plan: "psfft.Plan", group=None):
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        self.plan, self.group = plan, group
+        self.P, self.rank = dist.get_world_size(group), dist.get_rank(group)
+        self.lay = psfft.slab_query(plan.handle, self.P, self.rank)
+        dev, cd = plan.device, plan.cdtype
+        with torch.cuda.device(dev):
+            self.xslab = torch.empty(self.lay.xslab_elems, dtype=cd, device=dev)
+            self.zspec = torch.empty(self.lay.zspec_elems, dtype=cd, device=dev)
+            self.real = torch.empty((self.lay.Mz, plan.Ny, plan.N), dtype=plan.rdtype, device=dev)
+            exported = reduce_tensor(self.xslab)                # (rebuild function, IPC handle + geometry): picklable
+            gathered = [None] * self.P
+            dist.all_gather_object(gathered, exported, group=group)
+            # d_blocks[q]: rank q's x-slab as THIS process addresses it (own buffer; IPC mapping of a peer's)
+            self.blocks = [self.xslab if q == self.rank else fn(*args) for q, (fn, args) in enumerate(gathered)]
+        for q, b in enumerate(self.blocks):
+            assert b.numel() == psfft.slab_query(plan.handle, self.P, q).xslab_elems and b.dtype == cd
+        self._barrier()
+
+    def _barrier(self):
+        import torch.distributed as dist
+        torch.cuda.synchronize(self.plan.device)
+        dist.barrier(group=self.group)
+
+    def r2c(self, real_slab: torch.Tensor) -> torch.Tensor:
+        """real_slab [Mz][Ny][Nx] -> this rank's x-slab [Nz][Ny][w] (the object's own buffer, valid until the next call)."""
+        p, h = self.plan, self.plan.handle
+        with torch.cuda.device(p.device):
+            psfft.slab_r2c_xy(h, self.P, self.rank, real_slab, self.zspec, self.blocks, self.rank * self.lay.Mz)
+            self._barrier()                                     # every rank's stores have landed in every x-slab
+            psfft.slab_z(h, self.P, self.rank, -1, self.xslab)
+        return self.xslab.view(p.Nz, p.Ny, self.lay.w)
+
+    def c2r(self) -> torch.Tensor:
+        """The x-slab held by this object (as r2c left it, or as the caller filled ``self.xslab``; overwritten) ->
+        real z-slab [Mz][Ny][Nx] (the object's own buffer)."""
+        p, h = self.plan, self.plan.handle
+        with torch.cuda.device(p.device):
+            psfft.slab_z(h, self.P, self.rank, +1, self.xslab)
+            self._barrier()                                     # every x-slab holds its inverse z-pass
+            psfft.slab_c2r_yx(h, self.P, self.rank, self.blocks, self.rank * self.lay.Mz, self.zspec, self.real)
+            self._barrier()                                     # all peer loads done: x-slabs may be overwritten again
+        return self.real
 
 
 class VirtualSlabs:

@@ -1,6 +1,8 @@
 """Slab-decomposed transform on ONE GPU: P virtual ranks in direct
 mode -- each rank's y-pass stores straight into the x-slabs of all ranks -- must reproduce the single-GPU transform
 BIT FOR BIT (same kernels, same butterfly order per column), and the oracle within tolerance.  -m gpu."""
+import os
+
 import numpy as np
 import pytest
 
@@ -10,6 +12,7 @@ import oracle  # noqa: E402
 from paper_1808_01309_b200 import psfft, slab, synth  # noqa: E402
 
 pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 TOL = {torch.float64: 1e-12, torch.float32: 2e-5}
 RDT = {torch.float64: np.float64, torch.float32: np.float32}
@@ -229,3 +232,56 @@ def test_packed_mode_for_P_ranks_emulated_on_one_gpu(shape, P):
         rbuf = torch.cat(parts)
         psfft.slab_c2r_yx(plan.handle, P, r, slab._slice_ptrs(rbuf, splits[r][0]), 0, zs, back[r * Mz:(r + 1) * Mz])
     assert torch.equal(back, plan.c2r(single[None])[0])
+
+
+DIRECT_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import numpy as np, torch, torch.distributed as dist
+from paper_1808_01309_b200 import psfft, slab
+rank, P = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(0)                                   # both ranks on the one GPU of the box
+dist.init_process_group("gloo", rank=rank, world_size=P)   # handles and barriers only: direct mode needs no NCCL
+out = {}
+for shape, dtype in (((32, 24, 16), torch.float64), ((48, 16, 32), torch.float32), ((64, 64, 64), torch.float64)):
+    Nx, Ny, Nz = shape
+    plan = psfft.Plan(shape if len(set(shape)) > 1 else Nx, dtype, 1)
+    g = torch.Generator(device="cuda").manual_seed(99)     # the same global field in both processes
+    x = torch.rand((1, Nz, Ny, Nx), dtype=dtype, device="cuda", generator=g) * 2 - 1
+    want = plan.r2c(x)[0]                                  # single-GPU transform of the whole field
+    sf = slab.DirectSlabFFT(plan)
+    Mz, x0 = sf.lay.Mz, sf.lay.x0
+    for rep in range(2):                                   # twice: the barriers make the buffers reusable
+        X = sf.r2c(x[0, rank * Mz:(rank + 1) * Mz].contiguous())
+        fwd = bool(torch.equal(X, want[:, :, x0[rank]:x0[rank + 1]]))
+        back = sf.c2r()
+        inv = bool(torch.equal(back, plan.c2r(want[None].contiguous())[0, rank * Mz:(rank + 1) * Mz]))
+        out[f"{shape}-{dtype}-{rep}"] = [fwd, inv, float((back - x[0, rank * Mz:(rank + 1) * Mz]).abs().max())]
+    del sf
+    dist.barrier()
+print(json.dumps({"rank": rank, "results": out}))
+dist.destroy_process_group()
+""" % ROOT
+
+
+def test_direct_mode_with_two_real_processes_sharing_the_gpu(tmp_path):
+    """slab.DirectSlabFFT: two PROCESSES (gloo group for handles and barriers), both on cuda:0, each exporting its x-slab
+    to the other through CUDA IPC; rank p's y-pass stores straight into the peer's x-slab.  Each rank's x-slab equals the
+    matching kx range of psfft_fft3d_r2c of the whole field BIT FOR BIT, and the inverse equals psfft_fft3d_c2r's
+    planes bit for bit."""
+    import json
+    import subprocess
+    import sys
+    script = tmp_path / "direct_worker.py"
+    script.write_text(DIRECT_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29541", WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, str(script)], env=dict(env, RANK=str(r), LOCAL_RANK=str(r)),
+                              stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True) for r in range(2)]
+    outs = [p.communicate(timeout=600) for p in procs]
+    assert all(p.returncode == 0 for p in procs), [o[1][-1500:] for o in outs]
+    for r, (out, _) in enumerate(outs):
+        got = json.loads(out.strip().splitlines()[-1])
+        assert got["rank"] == r and len(got["results"]) == 6
+        for key, (fwd, inv, err) in got["results"].items():
+            assert fwd and inv, (r, key)
+            assert err < (1e-5 if "float32" in key else 1e-13), (r, key, err)
