@@ -80,21 +80,25 @@ class SlabFFT:
         self.sendbuf = torch.empty(self.lay.zspec_elems, dtype=cd, device=dev)   # sum of the slices = Mz Ny ldk
         self.send, self.recv = forward_splits(plan.Nz, plan.Ny, plan.ldk, self.P, self.rank)
 
-    def r2c(self, real_slab: torch.Tensor) -> torch.Tensor:
-        """real_slab [Mz][Ny][Nx] -> this rank's x-slab [Nz][Ny][w]."""
+    def r2c(self, real_slab: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        """real_slab [Mz][Ny][Nx] -> this rank's x-slab [Nz][Ny][w].  `out`: a flat complex buffer of xslab_elems to
+        receive it (a time loop passes the same one every step); allocated here when omitted."""
         p, h = self.plan, self.plan.handle
-        xslab = torch.empty(self.lay.xslab_elems, dtype=p.cdtype, device=p.device)
+        xslab = out if out is not None else torch.empty(self.lay.xslab_elems, dtype=p.cdtype, device=p.device)
+        assert xslab.numel() == self.lay.xslab_elems and xslab.dtype == p.cdtype and xslab.is_contiguous()
+        xslab = xslab.view(-1)
         psfft.slab_r2c_xy(h, self.P, self.rank, real_slab, self.zspec, _slice_ptrs(self.sendbuf, self.send), 0)
         exchange_forward(self.sendbuf, xslab, p.Nz, p.Ny, p.ldk, self.group)
         psfft.slab_z(h, self.P, self.rank, -1, xslab)
         return xslab.view(p.Nz, p.Ny, self.lay.w)
 
-    def c2r(self, xslab: torch.Tensor) -> torch.Tensor:
-        """x-slab [Nz][Ny][w] (overwritten) -> real z-slab [Mz][Ny][Nx]."""
+    def c2r(self, xslab: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        """x-slab [Nz][Ny][w] (overwritten) -> real z-slab [Mz][Ny][Nx] (into `out` when given)."""
         p, h = self.plan, self.plan.handle
         psfft.slab_z(h, self.P, self.rank, +1, xslab)
         exchange_inverse(xslab.reshape(-1), self.sendbuf, p.Nz, p.Ny, p.ldk, self.group)
-        real = torch.empty((self.lay.Mz, p.Ny, p.N), dtype=p.rdtype, device=p.device)
+        real = out if out is not None else torch.empty((self.lay.Mz, p.Ny, p.N), dtype=p.rdtype, device=p.device)
+        assert real.numel() == self.lay.real_elems and real.dtype == p.rdtype and real.is_contiguous()
         psfft.slab_c2r_yx(h, self.P, self.rank, _slice_ptrs(self.sendbuf, self.send), 0, self.zspec, real)
         return real
 

@@ -161,6 +161,13 @@ def test_packed_mode_class_under_torch_distributed_world_size_1():
         assert torch.equal(X, single)
         back = sf.c2r(X.clone())
         assert torch.equal(back, plan.c2r(single[None])[0])
+        # caller-owned result buffers (what a time loop passes every step): same bits, and it is those buffers that come back
+        xbuf = torch.full((sf.lay.xslab_elems,), complex(float("nan"), 0.0), dtype=torch.complex128, device="cuda")
+        rbuf = torch.full_like(xd, float("nan"))
+        X2 = sf.r2c(xd, out=xbuf)
+        assert X2.data_ptr() == xbuf.data_ptr() and torch.equal(X2, single)
+        back2 = sf.c2r(X2, out=rbuf)
+        assert back2.data_ptr() == rbuf.data_ptr() and torch.equal(back2, back)
     finally:
         dist.destroy_process_group()
 
